@@ -1,0 +1,400 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix.
+
+None of these compares the oracle with itself or with the CUDA path: each checks a closed form, an
+exact solution, an invariant or a special case that a plausible mistake in the oracle would break.
+All run on the CPU (-m "not gpu").
+"""
+import os
+
+import numpy as np
+import pytest
+
+import exact_riemann
+from helpers import (leaf_totals, oracle_for, problem_from_tree, small_amr_tree, smooth_fields)
+from oracle import lib
+from oracle.binding import hllc
+from sfh_inputs import Tree, prim_to_cons, unblockify, uniform_tree
+from sfh_inputs.configs import cell_centres, sod, Problem
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def run_to(m, T):
+    while m.t.value < T * (1 - 1e-14):
+        dt = m.cfl_dt()
+        m.advance(1, 0, min(dt, T - m.t.value))
+
+
+def prims(U, gamma):
+    rho = U[:, 0]
+    v = [U[:, 1 + d] / rho for d in range(3)]
+    P = (gamma - 1.0) * (U[:, 4] - 0.5 * rho * (v[0] ** 2 + v[1] ** 2 + v[2] ** 2))
+    return rho, v, P
+
+
+# ------------------------------------------------------------------ P1 exact Riemann solution
+def test_p1_exact_solver_reproduces_textbook_star_state():
+    gold = np.loadtxt(os.path.join(GOLD, "sod_star_gamma1p4.txt"))
+    ps, us, rsl, rsr = exact_riemann.star_state(1.0, 0.0, 1.0, 0.125, 0.0, 0.1, 1.4)
+    assert np.allclose([ps, us, rsl, rsr], gold, rtol=0, atol=6e-6)
+    # independent identity: Rankine-Hugoniot mass flux across the right shock
+    g = 1.4
+    S = 0.0 + np.sqrt(g * 0.1 / 0.125) * np.sqrt((g + 1) / (2 * g) * ps / 0.1 + (g - 1) / (2 * g))
+    assert abs(0.125 * (0.0 - S) - rsr * (us - S)) < 1e-12
+
+
+@pytest.mark.parametrize("gamma,T", [(1.4, 0.2), (5.0 / 3.0, 0.15)])
+def test_p1_sod_converges_to_exact_solution(gamma, T):
+    """Oracle L1 error against the exact Riemann solution falls monotonically with resolution
+    (C1 of BASELINE.json with gamma=1.4; the paper's own variant gamma=5/3)."""
+    errs = []
+    for nb in (4, 8, 16):
+        p = sod(nb=nb, gamma=gamma, slab=True)
+        m = oracle_for(p)
+        run_to(m, T)
+        assert m.status() == 0
+        U = m.get_state()
+        rho, v, P = prims(U, gamma)
+        x = (np.arange(nb * 8) + 0.5) / (nb * 8)
+        re, ue, pe = exact_riemann.sample((x - 0.5) / T, 1.0, 0.0, 1.0, 0.125, 0.0, 0.1, gamma)
+        rho1d = unblockify(rho, p.nb0)[3, 4, :]
+        u1d = unblockify(v[0], p.nb0)[3, 4, :]
+        p1d = unblockify(P, p.nb0)[3, 4, :]
+        errs.append([np.abs(rho1d - re).mean(), np.abs(u1d - ue).mean(), np.abs(p1d - pe).mean()])
+    errs = np.array(errs)
+    assert (errs[1] < 0.7 * errs[0]).all() and (errs[2] < 0.7 * errs[1]).all(), errs
+    assert errs[2, 0] < 8e-3 and errs[2, 1] < 1.5e-2 and errs[2, 2] < 7e-3, errs
+
+
+# ------------------------------------------------------------------ P2 HLLC identities
+def phys_flux(W, d, gamma):
+    rho, v, P = W[0], W[1:4], W[4]
+    E = P / (gamma - 1) + 0.5 * rho * (v @ v)
+    F = np.empty(5)
+    F[0] = rho * v[d]
+    F[1:4] = rho * v[d] * v
+    F[1 + d] += P
+    F[4] = v[d] * (E + P)
+    return F
+
+
+def test_p2_hllc_consistency_and_upwinding():
+    rng = np.random.default_rng(7)
+    for gamma in (1.4, 5.0 / 3.0, 1.0001):
+        for d in range(3):
+            for _ in range(20):
+                W = np.array([rng.uniform(0.1, 3), *rng.normal(0, 2, 3), rng.uniform(0.1, 3)])
+                F = hllc(W, W, d, gamma)
+                assert np.allclose(F, phys_flux(W, d, gamma), rtol=1e-13, atol=1e-13)
+            # supersonic to the right / left: pure upwind flux
+            WL = np.array([1.0, 0.3, -0.2, 0.1, 1.0])
+            WR = np.array([0.5, -0.1, 0.4, 0.2, 0.7])
+            WL[1 + d] = 9.0
+            WR[1 + d] = 8.0
+            assert np.allclose(hllc(WL, WR, d, gamma), phys_flux(WL, d, gamma), rtol=1e-14)
+            WL[1 + d] = -8.0
+            WR[1 + d] = -9.0
+            assert np.allclose(hllc(WL, WR, d, gamma), phys_flux(WR, d, gamma), rtol=1e-14)
+
+
+def test_p2_hllc_stationary_contact_flux_is_exact():
+    for d in range(3):
+        WL = np.array([1.0, 0.0, 0.0, 0.0, 0.7])
+        WR = np.array([0.013, 0.0, 0.0, 0.0, 0.7])
+        F = hllc(WL, WR, d, 1.4)
+        expect = np.zeros(5)
+        expect[1 + d] = 0.7
+        assert (F == expect).all()          # bitwise: distinguishes HLLC from HLL
+
+
+def test_p2_hllc_mirror_antisymmetry_and_axis_permutation():
+    rng = np.random.default_rng(11)
+    for _ in range(50):
+        WL = np.array([rng.uniform(0.1, 3), *rng.normal(0, 1.5, 3), rng.uniform(0.1, 3)])
+        WR = np.array([rng.uniform(0.1, 3), *rng.normal(0, 1.5, 3), rng.uniform(0.1, 3)])
+        F = hllc(WL, WR, 0, 1.4)
+        ml, mr = WR.copy(), WL.copy()
+        ml[1] *= -1
+        mr[1] *= -1
+        Fm = hllc(ml, mr, 0, 1.4)
+        sign = np.array([-1, 1, -1, -1, -1.0])
+        assert np.allclose(Fm, sign * F, rtol=1e-13, atol=1e-14)
+        # y-face flux of the state with (vx,vy,vz) -> (vz,vx,vy) equals the permuted x-face flux
+        perm = lambda W: np.array([W[0], W[3], W[1], W[2], W[4]])
+        Fy = hllc(perm(WL), perm(WR), 1, 1.4)
+        assert np.allclose(Fy, perm(F), rtol=1e-14, atol=1e-15)
+
+
+def test_p2_stationary_contact_preserved_exactly_by_the_full_scheme():
+    t = uniform_tree((4, 1, 1), 0)
+    level, ijk = t.block_list()
+    X, Y, Z = cell_centres(level, ijk, t.nb0)
+    rho = np.where((X > 0.25) & (X < 0.75), 1.0, 0.05)
+    z = np.zeros_like(rho)
+    U = prim_to_cons(rho, z, z, z, np.full_like(rho, 0.6), 1.4)
+    p = Problem("contact", t.nb0, 0, ((0, 0),) * 3, (1.0, 0.25, 0.25), 1.4, 0.4, 0, 5, level, ijk, U)
+    m = oracle_for(p)
+    m.advance(5, 0)
+    assert (m.get_state() == U).all()
+
+
+# ------------------------------------------------------------------ P3 conservation incl. reflux
+def hot_fields(factor, centre=0.5):
+    """smooth_fields with the pressure scaled by `factor` in a spot at (centre,)*3: a hot spot inside
+    the refined patch (centre 0.5) forces n = 2, one in coarse-only territory (centre 0.1) gives n = 0."""
+    def f(X, Y, Z):
+        rho, vx, vy, vz, P = smooth_fields(X, Y, Z)
+        r2 = (X - centre) ** 2 + (Y - centre) ** 2 + (Z - centre) ** 2
+        P = P * (1.0 + (factor - 1.0) * np.exp(-r2 / 0.01))
+        return rho, vx, vy, vz, P
+    return f
+
+
+@pytest.mark.parametrize("mode,factor,centre,expect_sub", [(0, 1.0, 0.5, None), (1, 1.0, 0.5, (1, 2, 4)), (1, 40.0, 0.5, None),
+                                                          (1, 0.02, 0.5, None), (1, 60.0, 0.1, None)])
+def test_p3_conservation_to_roundoff_with_flux_correction(mode, factor, centre, expect_sub):
+    t = small_amr_tree(4, 2)
+    p = problem_from_tree(t, mode=mode, fields=hot_fields(factor, centre))
+    m = oracle_for(p)
+    m.restrict_all(0)
+    leaf = m.is_leaf()
+    h0 = m.cell_width(0)
+    tot0 = leaf_totals(leaf, m.get_state(), p.level, h0)
+    scale = np.array([tot0[0], tot0[0], tot0[0], tot0[0], tot0[4]])
+    for step in range(2):
+        m.advance(1, mode)
+        tot = leaf_totals(leaf, m.get_state(), p.level, h0)
+        assert (np.abs(tot - tot0) / scale < 2e-14).all(), (tot - tot0) / scale
+    assert m.status() == 0
+    if expect_sub:
+        assert tuple(m.nupd // m.nupd[0]) == expect_sub
+
+
+def test_p3_subcycling_exponents_0_1_2_are_exercised():
+    seen = set()
+    for factor, centre in ((1.0, 0.5), (40.0, 0.5), (0.02, 0.5), (60.0, 0.1)):
+        t = small_amr_tree(4, 2)
+        p = problem_from_tree(t, mode=1, fields=hot_fields(factor, centre))
+        m = oracle_for(p)
+        m.restrict_all(0)
+        m.advance(1, 1)
+        seen.add(int(m.nupd[1] // m.nupd[0]))
+        seen.add(int(m.nupd[2] // m.nupd[1]))
+    assert {1, 2, 4} <= seen, seen
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_p3_conservation_breaks_without_reflux(mode):
+    t = small_amr_tree(4, 2)
+    p = problem_from_tree(t, mode=mode)
+    m = oracle_for(p)
+    m.set_reflux(0)
+    m.restrict_all(0)
+    leaf = m.is_leaf()
+    h0 = m.cell_width(0)
+    tot0 = leaf_totals(leaf, m.get_state(), p.level, h0)
+    m.advance(1, mode)
+    tot = leaf_totals(leaf, m.get_state(), p.level, h0)
+    assert abs(tot[0] - tot0[0]) / tot0[0] > 1e-9      # the conservation test has teeth
+
+
+# ------------------------------------------------------------------ P4 uniform == fully refined
+def test_p4_uniform_equals_fully_refined_bitwise():
+    tf = uniform_tree((4, 4, 4), 0)
+    pf = problem_from_tree(tf)
+    mu = oracle_for(pf)
+    tr = uniform_tree((2, 2, 2), 1, fully_refined_to=1)
+    pr = problem_from_tree(tr)
+    lev, ijk = tr.block_list()
+    fine = lev == 1
+    assert (ijk[fine] == pf.ijk).all()
+    U = pr.U.copy()
+    U[fine] = pf.U
+    mr = oracle_for(pr, U)
+    mr.restrict_all(0)
+    dt = 0.8 * mu.cfl_dt()
+    for _ in range(2):
+        mu.advance(1, 0, dt)
+        mr.advance(1, 0, dt)
+    assert (mr.get_state()[fine] == mu.get_state()).all()
+
+
+# ------------------------------------------------------------------ P5 mirror symmetry, axis permutation
+def sym_fields(X, Y, Z):
+    rho, vx, vy, vz, P = smooth_fields(X, Y, Z)
+    Xm = 1.0 - X
+    r2, a2, b2, c2, P2 = smooth_fields(Xm, Y, Z)
+    return 0.5 * (rho + r2), 0.5 * (vx - a2), 0.5 * (vy + b2), 0.5 * (vz + c2), 0.5 * (P + P2)
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_p5_mirror_symmetry_about_x(mode):
+    t = small_amr_tree(4, 2)
+    p = problem_from_tree(t, mode=mode, fields=sym_fields)
+    m = oracle_for(p)
+    m.restrict_all(0)
+    m.advance(2, mode)
+    U = m.get_state()
+    index = {(l, *c): b for b, (l, c) in enumerate(zip(p.level, map(tuple, p.ijk)))}
+    sign = np.array([1, -1, 1, 1, 1.0])[:, None, None, None]
+    worst = 0.0
+    for b in range(p.nblocks):
+        l, (bx, by, bz) = p.level[b], p.ijk[b]
+        bm = index[(l, (4 << l) - 1 - bx, by, bz)]
+        worst = max(worst, np.abs(U[b] - sign * U[bm][:, :, :, ::-1]).max())
+    assert worst < 1e-13, worst
+
+
+def test_p5_sod_along_y_and_z_reproduces_x_profile():
+    prof = []
+    for axis in range(3):
+        p = sod(nb=4, axis=axis, slab=True)
+        m = oracle_for(p)
+        m.advance(10, 0)
+        U = m.get_state()
+        rho = unblockify(U[:, 0], p.nb0)          # [z,y,x]
+        mom = unblockify(U[:, 1 + axis], p.nb0)
+        take = [3, 3, 3]
+        take[2 - axis] = slice(None)
+        prof.append((rho[tuple(take)], mom[tuple(take)]))
+    for a in (1, 2):
+        assert np.abs(prof[a][0] - prof[0][0]).max() < 1e-14
+        assert np.abs(prof[a][1] - prof[0][1]).max() < 1e-14
+
+
+# ------------------------------------------------------------------ P6 free stream
+@pytest.mark.parametrize("mode", [0, 1])
+def test_p6_free_stream_preserved(mode):
+    t = small_amr_tree(4, 2)
+    f = lambda X, Y, Z: (np.full_like(X, 1.3), np.full_like(X, 0.7), np.full_like(X, -0.4), np.full_like(X, 0.2), np.full_like(X, 0.9))
+    p = problem_from_tree(t, mode=mode, fields=f)
+    m = oracle_for(p)
+    m.restrict_all(0)
+    m.advance(2, mode)
+    d = np.abs(m.get_state() - p.U).max()
+    assert d == 0.0 if mode == 0 else d < 1e-15
+
+
+# ------------------------------------------------------------------ P7 eq. (16)-(17)
+def test_p7_time_interpolation_closed_forms():
+    L = lib()
+    f = L.orc_time_interp
+    rng = np.random.default_rng(3)
+    for _ in range(50):
+        U0, Uh, U1 = rng.normal(0, 2, 3)
+        assert f(U0, Uh, U1, 0.0) == U0
+        assert abs(f(U0, Uh, U1, 1.0) - U1) < 1e-14
+        assert abs(f(U0, Uh, U1, 0.5) - (0.25 * U0 + 0.5 * Uh + 0.25 * U1)) < 1e-14
+        eps = 1e-7
+        assert abs((f(U0, Uh, U1, eps) - U0) / eps - 2.0 * (Uh - U0)) < 1e-5
+        # exact for data linear in time
+        a, b = rng.normal(0, 1, 2)
+        for tau in (0.125, 0.3, 0.75):
+            assert abs(f(a, a + 0.5 * b, a + b, tau) - (a + tau * b)) < 1e-14
+
+
+# ------------------------------------------------------------------ P8 eq. (14)-(15)
+def test_p8_substep_exponent_table():
+    f = lib().orc_substep_exponent
+    table = [(1.0, 1.0, 0), (1.0, 2.0, 0), (1.0, 0.5, 1), (1.0, 0.51, 1), (1.0, 0.49, 2), (1.0, 0.25, 2),
+             (1.0, 0.1, 4), (0.3, 0.3, 0), (0.3, 0.1499, 2), (3e-4, 1e-4, 2)]
+    for dtH, dtc, n in table:
+        assert f(dtH, dtc) == n, (dtH, dtc, n)
+        assert dtH * 2.0 ** -n <= dtc and (n == 0 or dtH * 2.0 ** -(n - 1) > dtc)
+
+
+# ------------------------------------------------------------------ P9 prolongation / restriction
+def two_level_tree(periodic):
+    t = Tree((4, 4, 4), 1, periodic)
+    f0 = np.zeros_like(t.exists[0])
+    f0[0, 0, 0] = True            # one refined corner block so level 1 exists; queries go elsewhere
+    t.refine(0, f0)
+    return t
+
+
+def test_p9_prolongation_is_conservative_linear_exact_and_positive():
+    t = two_level_tree((False, False, False))
+    level, ijk = t.block_list()
+    rng = np.random.default_rng(5)
+    # (a) random positive coarse data: mean of 8 children = parent, children stay positive
+    p = problem_from_tree(t, fields=lambda X, Y, Z: (rng.uniform(0.01, 5, X.shape),) * 1 + (0 * X, 0 * X, 0 * X, 1 + 0 * X))
+    m = oracle_for(p)
+    for (I, J, K) in [(9, 10, 11), (17, 5, 20), (25, 25, 25)]:
+        kids = np.array([m.get(1, 2 * I + a, 2 * J + b, 2 * K + c) for c in (0, 1) for b in (0, 1) for a in (0, 1)])
+        parent = m.get(0, I, J, K)
+        assert np.abs(kids.mean(axis=0) - parent).max() < 1e-14
+        assert (kids[:, 0] > 0).all()
+        nb = [m.get(0, I + a, J + b, K + c)[0] for a, b, c in [(1, 0, 0), (-1, 0, 0), (0, 1, 0), (0, -1, 0), (0, 0, 1), (0, 0, -1), (0, 0, 0)]]
+        assert kids[:, 0].min() >= min(nb) - 1e-14 and kids[:, 0].max() <= max(nb) + 1e-14
+    # (b) linear field: prolongation reproduces it exactly at fine cell centres
+    lin = lambda X, Y, Z: (2.0 + 0.5 * X - 0.25 * Y + 0.125 * Z, 0 * X, 0 * X, 0 * X, 1 + 0 * X)
+    p = problem_from_tree(t, fields=lin)
+    m = oracle_for(p)
+    for (I, J, K) in [(20, 21, 22), (33, 18, 40), (50, 50, 50)]:
+        x, y, z = (I + 0.5) / 64, (J + 0.5) / 64, (K + 0.5) / 64
+        val = m.get(1, I, J, K)[0]
+        assert abs(val - (2.0 + 0.5 * x - 0.25 * y + 0.125 * z)) < 1e-14
+    # (c) restriction of the prolonged values is the identity (checked through (a))
+
+
+def test_p9_restriction_is_the_mean_of_eight_children():
+    t = uniform_tree((2, 2, 2), 1, fully_refined_to=1)
+    rng = np.random.default_rng(9)
+    p = problem_from_tree(t, fields=lambda X, Y, Z: (rng.uniform(0.5, 2, X.shape), 0 * X, 0 * X, 0 * X, 1 + 0 * X))
+    m = oracle_for(p)
+    m.restrict_all(0)
+    U = m.get_state()
+    fine = p.level == 1
+    rho_f = unblockify(U[fine][:, 0], (4, 4, 4))
+    rho_c = unblockify(U[~fine][:, 0], (2, 2, 2))
+    mean8 = rho_f.reshape(16, 2, 16, 2, 16, 2).mean(axis=(1, 3, 5))
+    assert np.abs(mean8 - rho_c).max() < 1e-15
+
+
+# ------------------------------------------------------------------ P10 1-D invariance (bitwise)
+def test_p10_one_dimensional_problem_stays_one_dimensional():
+    p = sod(nb=4)
+    m = oracle_for(p)
+    m.advance(20, 0)
+    U = m.get_state()
+    assert (U[:, 2] == 0).all() and (U[:, 3] == 0).all()
+    for v in (0, 1, 4):
+        f = unblockify(U[:, v], p.nb0)
+        assert (f == f[0:1, 0:1, :]).all()
+
+
+# ------------------------------------------------------------------ P11 contact advection
+def test_p11_contact_advection_keeps_velocity_and_pressure_uniform():
+    t = uniform_tree((4, 4, 4), 0)
+    f = lambda X, Y, Z: (1.0 + 0.8 * np.exp(-((X - 0.5) ** 2 + (Y - 0.5) ** 2 + (Z - 0.5) ** 2) / 0.02),
+                         np.full_like(X, 0.7), np.full_like(X, -0.3), np.full_like(X, 0.45), np.full_like(X, 1.1))
+    p = problem_from_tree(t, fields=f)
+    m = oracle_for(p)
+    m.advance(5, 0)
+    U = m.get_state()
+    rho, v, P = prims(U, p.gamma)
+    assert np.abs(v[0] - 0.7).max() < 1e-13 and np.abs(v[1] + 0.3).max() < 1e-13 and np.abs(v[2] - 0.45).max() < 1e-13
+    assert np.abs(P - 1.1).max() < 1e-12
+    assert np.abs(rho - f(*cell_centres(p.level, p.ijk, p.nb0))[0]).max() > 1e-3   # and the pulse did move
+
+
+# ------------------------------------------------------------------ P12 second-order convergence
+def test_p12_second_order_convergence_on_a_sound_wave():
+    gamma, A = 1.4, 1e-5
+    errs = []
+    for nb in (2, 4, 8):
+        t = uniform_tree((nb, 1, 1), 0)
+        level, ijk = t.block_list()
+        X, _, _ = cell_centres(level, ijk, t.nb0)
+        s = np.sin(2 * np.pi * X)
+        rho0, P0 = 1.0, 1.0 / gamma                  # c0 = 1
+        U = prim_to_cons(rho0 * (1 + A * s), A * s, 0 * s, 0 * s, P0 * (1 + gamma * A * s), gamma)
+        p = Problem("wave", t.nb0, 0, ((0, 0),) * 3, (1.0, 1.0 / nb, 1.0 / nb), gamma, 0.4, 0, 0, level, ijk, U)
+        m = oracle_for(p)
+        T = 0.25
+        run_to(m, T)
+        rho = unblockify(m.get_state()[:, 0], p.nb0)[0, 0, :]
+        x = (np.arange(nb * 8) + 0.5) / (nb * 8)
+        exact = rho0 * (1 + A * np.sin(2 * np.pi * (x - T)))
+        errs.append(np.abs(rho - exact).mean() / A)
+    assert errs[0] / errs[1] > 3.0 and errs[1] / errs[2] > 3.0, errs
