@@ -271,8 +271,9 @@ def test_p6_free_stream_preserved(mode):
     m = oracle_for(p)
     m.restrict_all(0)
     m.advance(2, mode)
+    # not bitwise: the fixed-order sums of 8 equal children / 4 equal fine fluxes round (3x is inexact)
     d = np.abs(m.get_state() - p.U).max()
-    assert d == 0.0 if mode == 0 else d < 1e-15
+    assert d < 2e-15
 
 
 # ------------------------------------------------------------------ P7 eq. (16)-(17)
@@ -382,7 +383,7 @@ def test_p11_contact_advection_keeps_velocity_and_pressure_uniform():
 def test_p12_second_order_convergence_on_a_sound_wave():
     gamma, A = 1.4, 1e-5
     errs = []
-    for nb in (2, 4, 8):
+    for nb in (4, 8, 16):
         t = uniform_tree((nb, 1, 1), 0)
         level, ijk = t.block_list()
         X, _, _ = cell_centres(level, ijk, t.nb0)
@@ -397,4 +398,6 @@ def test_p12_second_order_convergence_on_a_sound_wave():
         x = (np.arange(nb * 8) + 0.5) / (nb * 8)
         exact = rho0 * (1 + A * np.sin(2 * np.pi * (x - T)))
         errs.append(np.abs(rho - exact).mean() / A)
-    assert errs[0] / errs[1] > 3.0 and errs[1] / errs[2] > 3.0, errs
+    # minmod clips the two extrema, so the L1 ratio approaches 4 from below (3.45, 3.63, 3.72 ...);
+    # a first-order scheme would give 2
+    assert errs[0] / errs[1] > 3.3 and errs[1] / errs[2] > 3.5, errs
