@@ -1,0 +1,177 @@
+/* sfh.h — C ABI of libsfh: the per-step hydrodynamics update on octree block-structured AMR grids
+ * of arxiv/paper_2604_21438 (SFUMATO#), B200 (sm_100a) only.
+ *
+ * What the calls compute is defined by PAPER.md (cited per call as PAPER.md:<line>) and, where the
+ * paper is silent, by the readings R1..R28 of DESIGN.md.  There is no CPU fallback: every call that
+ * touches field data launches CUDA kernels on the caller's stream and returns SFH_ECUDA when no
+ * device is usable.
+ *
+ * Conventions
+ *   - Blocks: N^3 = 8^3 cells, fixed; level l has cell width h_l = box_len[0] / (nb0[0]*8*2^l)
+ *     (PAPER.md:96).  A block of level l has integer coordinates (bx,by,bz) in [0, nb0_d * 2^l);
+ *     child c = cx + 2 cy + 4 cz of (bx,by,bz) is (2bx+cx, 2by+cy, 2bz+cz) at level l+1.
+ *     EVERY block of every level holds data and is updated, covered (non-leaf) blocks too.
+ *   - Conserved variables, in this order: rho, rho*vx, rho*vy, rho*vz, rho*E with
+ *     rho*E = P/(gamma-1) + rho |v|^2 / 2 (eq. 1-3; eq. 8).  fp64.
+ *   - "Caller layout" of a state: double U[nblocks][5][8][8][8], indexed [block][var][k][j][i]
+ *     (i = x fastest), blocks in the order given to sfh_create_mesh, INTERIOR cells only.
+ *   - Internal layout: interior-only blocks in the library's own order (level-major, Morton within
+ *     a level); ghost values are never stored for same-level neighbours (the stage kernels gather
+ *     them from the neighbours' interiors through the neighbour map); only ghost slabs on
+ *     coarse-fine faces are materialised (in the work buffer) by sfh_fill_ghosts.
+ *   - Three state copies ("roles"): 0 = U^n, 1 = U^{n+1/2}, 2 = U^{n+1} (values "at
+ *     the current, previous, and half timesteps" are kept for temporal interpolation).
+ *   - Pointers: "host" = ordinary host memory, "device" = CUDA device memory of the current
+ *     device.  `stream` is a cudaStream_t passed as void* (NULL = default stream).  Calls are
+ *     asynchronous on that stream unless they return a host scalar (noted per call).
+ *   - Ownership: the caller owns state and work buffers and the stream; the library owns the mesh
+ *     tables (host and device).  A mesh is immutable after creation.
+ *   - Errors: every int call returns SFH_OK (0) or a negative code; nothing throws or aborts
+ *     across the ABI; sfh_last_error() returns a text for the calling thread's last failure.
+ *     Non-positive density or pressure is reported by sfh_status, never floored (reading R28).
+ */
+#ifndef SFH_H_
+#define SFH_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SFH_OK 0
+#define SFH_EINVAL (-1) /* bad argument                                   */
+#define SFH_EMESH (-2)  /* block list is not a valid, properly nested octree */
+#define SFH_ENOMEM (-3) /* host or device allocation failed                */
+#define SFH_ECUDA (-4)  /* CUDA runtime/driver error (text in sfh_last_error) */
+#define SFH_ESTATE (-5) /* mesh not bound to state/work buffers            */
+
+typedef struct sfh_mesh sfh_mesh; /* opaque, library-owned */
+
+typedef struct {
+  int32_t nb0[3];     /* root (level-0) blocks per axis */
+  int32_t ncell;      /* cells per block edge; only 8 is supported */
+  int32_t nghost;     /* ghost layers; only 2 is supported     */
+  int32_t max_level;  /* finest level that may hold blocks (0 = uniform grid)                    */
+  int32_t bc[3][2];   /* per axis, low/high face: 0 periodic, 1 outflow (zero gradient, R1)      */
+  double box_len[3];  /* physical size; cells are cubes of h_0 = box_len[0]/(nb0[0]*8)           */
+  double gamma;       /* ideal-gas exponent of eq. (8)      */
+  double cfl;         /* CFL number used by sfh_cfl_dt / sfh_advance                             */
+} sfh_config;
+
+/* ---- mesh: octree block table and neighbour map -------------------------- */
+
+/* Builds the block table (level, coordinates, parent, first child), the 27-entry same-level
+ * neighbour map, the per-face halo sources, and the flux-register maps on the HOST.  `level`
+ * [nblocks] and `ijk` [nblocks][3] are host arrays.  Validates: levels/coordinates in range, no
+ * duplicates, every block of level > 0 has its parent and all 7 siblings, and proper nesting over
+ * all 26 neighbours (a neighbour position inside the domain holds a block of the same level or
+ * its parent exists, reading R25); violations give SFH_EMESH.  Needs no GPU. */
+int sfh_create_mesh(const sfh_config* cfg, int64_t nblocks, const int32_t* level, const int32_t* ijk,
+                    sfh_mesh** out);
+int sfh_destroy_mesh(sfh_mesh* m);
+
+int64_t sfh_num_blocks(const sfh_mesh* m);
+/* Blocks of `level` occupy library slots [first, first+count). */
+int sfh_level_range(const sfh_mesh* m, int level, int64_t* first, int64_t* count);
+/* perm[s] = caller index of the block stored in library slot s (host array [nblocks]). */
+int sfh_block_order(const sfh_mesh* m, int64_t* perm);
+/* Number of coarse-fine block faces (fine side; one ghost slab and one flux register each) and of
+ * coarse-leaf faces that receive a flux correction. */
+int sfh_num_faces(const sfh_mesh* m, int64_t* n_fine_faces, int64_t* n_coarse_faces);
+/* Cell width of a level. */
+double sfh_cell_width(const sfh_mesh* m, int level);
+
+/* Bytes of ONE state copy in the internal layout, and of the work buffer (coarse-fine ghost
+ * slabs, flux registers, reduction scratch). */
+int64_t sfh_state_bytes(const sfh_mesh* m);
+int64_t sfh_work_bytes(const sfh_mesh* m);
+
+/* Attaches caller-owned DEVICE buffers (each state buffer >= sfh_state_bytes, work >=
+ * sfh_work_bytes, all 256-byte aligned), uploads the mesh tables and creates the TMA tensor maps
+ * of the three state buffers.  Synchronous.  The work buffer is zeroed. */
+int sfh_bind(sfh_mesh* m, void* d_state0, void* d_state1, void* d_state2, void* d_work);
+
+/* Copies a DEVICE state in caller layout into / out of role `which` (0,1,2) of every level.
+ * sfh_get_state(which=0) after sfh_advance returns U at the new time. */
+int sfh_set_state(sfh_mesh* m, int which, const double* d_U, void* stream);
+int sfh_get_state(sfh_mesh* m, int which, double* d_U, void* stream);
+
+/* ---- the hot path ------------------------------------------------------------------------------ */
+
+/* Ghost fill of role `which` on `level` (-1: every level, coarse to fine).
+ * Same-level ("sibling") ghosts and outflow ghosts are not stored: the hydro stage kernels gather
+ * them.  This call computes the ghost slabs of every block face of the level whose neighbour is
+ * one level coarser: slope-limited linear prolongation of the coarse data (reading R3), which are
+ *   interp = 0: role `which` of level-1 (synchronous mode: both levels at the same time);
+ *   interp = 1: the quadratic time interpolation of eq. (16)-(17) of roles
+ *               0, 1, 2 of level-1 at tau = (t - t^n)/(t^{n+1} - t^n) of the COARSE step.
+ * Asynchronous. */
+int sfh_fill_ghosts(sfh_mesh* m, int level, int which, int interp, double tau, void* stream);
+
+/* Writes ghosted blocks double G[nblocks][5][12][12][12] (caller block order, DEVICE) of role
+ * `which`: interiors, and the 6 face halos exactly as the stage kernels see them (same-level
+ * gather, outflow copy, or the coarse-fine slabs last written by sfh_fill_ghosts); edge and
+ * corner ghost cells, which no stage reads, are set to NaN.  For parity tests of the ghost fill. */
+int sfh_get_ghosted(sfh_mesh* m, int which, double* d_G, void* stream);
+
+/* CFL time step (reading R16): dt = cfl * h_l / max over all cells of level l of
+ * (max_d |v_d| + c_s), c_s = sqrt(gamma P / rho), from role 0; level = -1: minimum over levels
+ * ("grid-level reductions").  Warp-shuffle + atomic-max reduction
+ * (exact).  Returns the value in *dt_host: synchronises the stream. */
+int sfh_cfl_dt(sfh_mesh* m, int level, double* dt_host, void* stream);
+
+/* One predictor-corrector update of `level` (-1: every level) by dt   (R8-R14):
+ *   zero the flux registers of the (level, level+1) interface;
+ *   predictor: U^{n+1/2} = U^n - dt/(2h) sum_d dF_d, first-order HLLC fluxes      (role 0 -> 1);
+ *   sfh_fill_ghosts(level, which=1, interp, tau + dtau/2);
+ *   corrector: minmod-limited linear reconstruction of primitives of U^{n+1/2}, HLLC flux
+ *              (PAPER.md:126), U^{n+1} = U^n - dt/h sum_d dF_d                    (roles 0,1 -> 2);
+ *   flux-register accumulate: fine side += dt*F, coarse leaf side stores F.
+ * The caller must have called sfh_fill_ghosts(level, 0, interp, tau) before.  tau = time fraction
+ * of the start of this step within the parent-level step, dtau = dt/dt_parent (both ignored when
+ * interp = 0).  Asynchronous.  Does not rotate the roles (see sfh_end_step). */
+int sfh_hydro_step(sfh_mesh* m, int level, double dt, int interp, double tau, double dtau, void* stream);
+
+/* Flux correction of `coarse_level` after level+1 has reached the same time:
+ *   restriction: every covered cell of role 2 of coarse_level = mean of its 8 children (role 0 of
+ *                level+1, i.e. after that level's sfh_end_step);
+ *   reflux: each leaf cell of coarse_level on a coarse-fine face gets
+ *           U -= (s/h) (1/4 sum_{2x2} R_fine - dt_coarse F_coarse), s = +1/-1 for its upper/lower face.
+ * Fixed summation order, no floating-point atomics.  Asynchronous. */
+int sfh_flux_correct(sfh_mesh* m, int coarse_level, double dt_coarse, void* stream);
+
+/* Restriction alone (a8): covered cells of role `dst_role` of coarse_level = mean of the 8 children
+ * in role `src_role` of coarse_level+1.  Used to make initial data consistent.  Asynchronous. */
+int sfh_restrict(sfh_mesh* m, int coarse_level, int src_role, int dst_role, void* stream);
+
+/* Ends the step of `level` (-1: all): role 0 <-> role 2 (U^n := U^{n+1}).  Host-side pointer
+ * rotation, no data movement. */
+int sfh_end_step(sfh_mesh* m, int level);
+
+/* Level driver.  mode 0 = synchronous: all levels advance with a common dt =
+ * dt_fixed if > 0 else the minimum CFL step over levels, computed on the device without a host
+ * round trip.  mode 1 = adaptive: Berger-Colella recursion; the step of level l+1 is
+ * dt_l 2^-n with n = min{m >= 0 : dt_l 2^-m <= dt_CFL^{l+1}} (eq. 14-15); level 0 uses dt_fixed if
+ * > 0 else its CFL step.  Adds the elapsed time to *t_host and the number of updates of each level
+ * to nupd_host[0..max_level] (either may be NULL).  Synchronises the stream before returning. */
+int sfh_advance(sfh_mesh* m, int ncoarse_steps, int mode, double dt_fixed, double* t_host,
+                int64_t* nupd_host, void* stream);
+
+/* End-to-end convenience: h_in (HOST, caller layout) -> device role 0, sfh_advance, role 0 -> h_out
+ * (HOST).  Host buffers should be pinned for full PCIe speed.  Synchronous. */
+int sfh_advance_host(sfh_mesh* m, const double* h_in, double* h_out, int ncoarse_steps, int mode,
+                     double dt_fixed, double* t_host, void* stream);
+
+/* Number of interior cells of role `which` with rho <= 0, P <= 0 or NaN (all blocks).  Synchronises. */
+int sfh_status(sfh_mesh* m, int which, int64_t* n_bad_cells, void* stream);
+
+/* Kernels launched by this library since the mesh was created (for bench.py's gpu_launches). */
+int64_t sfh_launch_count(const sfh_mesh* m);
+
+const char* sfh_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SFH_H_ */

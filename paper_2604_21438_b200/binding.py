@@ -1,0 +1,245 @@
+"""ctypes binding of libsfh.so (include/sfh.h).  Argument marshalling only."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+
+from . import build as _build
+
+N, NV = 8, 5
+BLK = NV * N * N * N
+HERE = os.path.dirname(os.path.abspath(__file__))
+HEADER = os.path.join(os.path.dirname(HERE), "include", "sfh.h")
+
+ERRORS = {-1: "SFH_EINVAL", -2: "SFH_EMESH", -3: "SFH_ENOMEM", -4: "SFH_ECUDA", -5: "SFH_ESTATE"}
+
+
+class SfhError(RuntimeError):
+    def __init__(self, code, text):
+        super().__init__("%s (%d): %s" % (ERRORS.get(code, "SFH_E?"), code, text))
+        self.code = code
+
+
+class SfhConfig(C.Structure):
+    _fields_ = [("nb0", C.c_int32 * 3), ("ncell", C.c_int32), ("nghost", C.c_int32), ("max_level", C.c_int32),
+                ("bc", (C.c_int32 * 2) * 3), ("box_len", C.c_double * 3), ("gamma", C.c_double), ("cfl", C.c_double)]
+
+
+def library_path():
+    return _build.lib_path()
+
+
+def declared_symbols():
+    """Names of the functions include/sfh.h declares."""
+    text = open(HEADER).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(sfh_[a-z_0-9]+)\s*\(", text)))
+
+
+_lib = None
+
+
+def load_library(path=None):
+    """Loads libsfh.so (building it with nvcc if it is missing or stale).  Raises if that fails:
+    there is no fallback implementation."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    if path is None:
+        path = _build.build()
+    L = C.CDLL(path)
+    vp, i64, i32, dbl = C.c_void_p, C.c_int64, C.c_int, C.c_double
+    sig = {
+        "sfh_create_mesh": (i32, [C.POINTER(SfhConfig), i64, vp, vp, C.POINTER(vp)]),
+        "sfh_destroy_mesh": (i32, [vp]),
+        "sfh_num_blocks": (i64, [vp]),
+        "sfh_level_range": (i32, [vp, i32, C.POINTER(i64), C.POINTER(i64)]),
+        "sfh_block_order": (i32, [vp, vp]),
+        "sfh_num_faces": (i32, [vp, C.POINTER(i64), C.POINTER(i64)]),
+        "sfh_cell_width": (dbl, [vp, i32]),
+        "sfh_state_bytes": (i64, [vp]),
+        "sfh_work_bytes": (i64, [vp]),
+        "sfh_bind": (i32, [vp, vp, vp, vp, vp]),
+        "sfh_set_state": (i32, [vp, i32, vp, vp]),
+        "sfh_get_state": (i32, [vp, i32, vp, vp]),
+        "sfh_fill_ghosts": (i32, [vp, i32, i32, i32, dbl, vp]),
+        "sfh_get_ghosted": (i32, [vp, i32, vp, vp]),
+        "sfh_cfl_dt": (i32, [vp, i32, C.POINTER(dbl), vp]),
+        "sfh_hydro_step": (i32, [vp, i32, dbl, i32, dbl, dbl, vp]),
+        "sfh_flux_correct": (i32, [vp, i32, dbl, vp]),
+        "sfh_restrict": (i32, [vp, i32, i32, i32, vp]),
+        "sfh_end_step": (i32, [vp, i32]),
+        "sfh_advance": (i32, [vp, i32, i32, dbl, C.POINTER(dbl), vp, vp]),
+        "sfh_advance_host": (i32, [vp, vp, vp, i32, i32, dbl, C.POINTER(dbl), vp]),
+        "sfh_status": (i32, [vp, i32, C.POINTER(i64), vp]),
+        "sfh_launch_count": (i64, [vp]),
+        "sfh_last_error": (C.c_char_p, []),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(L, name)
+        fn.restype = res
+        fn.argtypes = args
+    if path == _build.lib_path():
+        _lib = L
+    return L
+
+
+def _stream():
+    import torch
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+class Mesh:
+    """An octree block mesh bound to three device state buffers and a work buffer (torch tensors).
+
+    level[nb], ijk[nb,3]: the caller's block list; states cross this interface in caller layout
+    double [nb][5][8][8][8] (interior cells, [block][var][k][j][i])."""
+
+    def __init__(self, nb0, max_level, bc, box_len, gamma, cfl, level, ijk, device="cuda:0", bind=True, lib=None):
+        self.L = lib or load_library()
+        self.level = np.ascontiguousarray(level, dtype=np.int32)
+        self.ijk = np.ascontiguousarray(ijk, dtype=np.int32).reshape(-1, 3)
+        self.nb = len(self.level)
+        cfg = SfhConfig()
+        for d in range(3):
+            cfg.nb0[d] = int(nb0[d])
+            cfg.box_len[d] = float(box_len[d])
+            for s in range(2):
+                cfg.bc[d][s] = int(bc[d][s])
+        cfg.ncell, cfg.nghost, cfg.max_level = N, 2, int(max_level)
+        cfg.gamma, cfg.cfl = float(gamma), float(cfl)
+        self.cfg = cfg
+        self.max_level = int(max_level)
+        self.h = C.c_void_p()
+        self._chk(self.L.sfh_create_mesh(C.byref(cfg), self.nb, self.level.ctypes.data, self.ijk.ctypes.data,
+                                         C.byref(self.h)))
+        self.t = C.c_double(0.0)
+        self.nupd = np.zeros(self.max_level + 1, dtype=np.int64)
+        self.device = device
+        self.bound = False
+        if bind:
+            self.bind()
+
+    @classmethod
+    def from_problem(cls, p, **kw):
+        return cls(p.nb0, p.max_level, p.bc, p.box_len, p.gamma, p.cfl, p.level, p.ijk, **kw)
+
+    def __del__(self):
+        if getattr(self, "h", None) and self.h.value:
+            self.L.sfh_destroy_mesh(self.h)
+            self.h = C.c_void_p()
+
+    def _chk(self, rc):
+        if rc != 0:
+            raise SfhError(rc, self.L.sfh_last_error().decode())
+
+    # ---- host-only queries
+    def level_range(self, l):
+        a, b = C.c_int64(), C.c_int64()
+        self._chk(self.L.sfh_level_range(self.h, l, C.byref(a), C.byref(b)))
+        return a.value, b.value
+
+    def block_order(self):
+        perm = np.zeros(self.nb, dtype=np.int64)
+        self._chk(self.L.sfh_block_order(self.h, perm.ctypes.data))
+        return perm
+
+    def num_faces(self):
+        a, b = C.c_int64(), C.c_int64()
+        self._chk(self.L.sfh_num_faces(self.h, C.byref(a), C.byref(b)))
+        return a.value, b.value
+
+    def cell_width(self, l):
+        return self.L.sfh_cell_width(self.h, l)
+
+    def state_bytes(self):
+        return self.L.sfh_state_bytes(self.h)
+
+    def work_bytes(self):
+        return self.L.sfh_work_bytes(self.h)
+
+    def launch_count(self):
+        return self.L.sfh_launch_count(self.h)
+
+    # ---- device
+    def bind(self):
+        import torch
+        if not torch.cuda.is_available():
+            raise SfhError(-4, "no CUDA device: libsfh has no CPU fallback")
+        dev = torch.device(self.device)
+        torch.cuda.set_device(dev)
+        self.state = [torch.empty(self.state_bytes() // 8, dtype=torch.float64, device=dev) for _ in range(3)]
+        self.work = torch.empty(self.work_bytes() // 8, dtype=torch.float64, device=dev)
+        torch.cuda.synchronize()
+        self._chk(self.L.sfh_bind(self.h, self.state[0].data_ptr(), self.state[1].data_ptr(),
+                                  self.state[2].data_ptr(), self.work.data_ptr()))
+        self.bound = True
+
+    def _dev_state(self, U):
+        import torch
+        if isinstance(U, np.ndarray):
+            U = torch.from_numpy(np.ascontiguousarray(U, dtype=np.float64))
+        U = U.to(device=self.device, dtype=torch.float64).contiguous()
+        assert U.numel() == self.nb * BLK, "state must be [nb][5][8][8][8]"
+        return U
+
+    def set_state(self, U, which=0):
+        U = self._dev_state(U)
+        self._chk(self.L.sfh_set_state(self.h, which, U.data_ptr(), _stream()))
+        import torch
+        torch.cuda.current_stream().synchronize()   # U may be a temporary
+
+    def get_state(self, which=0):
+        """torch tensor [nb][5][8][8][8] on the device."""
+        import torch
+        out = torch.empty((self.nb, NV, N, N, N), dtype=torch.float64, device=self.device)
+        self._chk(self.L.sfh_get_state(self.h, which, out.data_ptr(), _stream()))
+        return out
+
+    def get_ghosted(self, which=0):
+        import torch
+        out = torch.empty((self.nb, NV, N + 4, N + 4, N + 4), dtype=torch.float64, device=self.device)
+        self._chk(self.L.sfh_get_ghosted(self.h, which, out.data_ptr(), _stream()))
+        return out
+
+    def fill_ghosts(self, level=-1, which=0, interp=0, tau=0.0):
+        self._chk(self.L.sfh_fill_ghosts(self.h, level, which, interp, tau, _stream()))
+
+    def cfl_dt(self, level=-1):
+        dt = C.c_double()
+        self._chk(self.L.sfh_cfl_dt(self.h, level, C.byref(dt), _stream()))
+        return dt.value
+
+    def hydro_step(self, level, dt, interp=0, tau=0.0, dtau=0.0):
+        self._chk(self.L.sfh_hydro_step(self.h, level, dt, interp, tau, dtau, _stream()))
+
+    def flux_correct(self, coarse_level, dt_coarse):
+        self._chk(self.L.sfh_flux_correct(self.h, coarse_level, dt_coarse, _stream()))
+
+    def restrict(self, coarse_level, src_role=0, dst_role=0):
+        self._chk(self.L.sfh_restrict(self.h, coarse_level, src_role, dst_role, _stream()))
+
+    def restrict_all(self, role=0):
+        for l in range(self.max_level - 1, -1, -1):
+            self.restrict(l, role, role)
+
+    def end_step(self, level=-1):
+        self._chk(self.L.sfh_end_step(self.h, level))
+
+    def advance(self, nsteps, mode=0, dt_fixed=0.0):
+        self._chk(self.L.sfh_advance(self.h, nsteps, mode, dt_fixed, C.byref(self.t), self.nupd.ctypes.data,
+                                     _stream()))
+        return self.t.value
+
+    def advance_host(self, h_in, h_out, nsteps, mode=0, dt_fixed=0.0):
+        """h_in, h_out: host tensors/arrays in caller layout (pinned for full PCIe speed)."""
+        pin = h_in.data_ptr() if hasattr(h_in, "data_ptr") else h_in.ctypes.data
+        pout = h_out.data_ptr() if hasattr(h_out, "data_ptr") else h_out.ctypes.data
+        self._chk(self.L.sfh_advance_host(self.h, pin, pout, nsteps, mode, dt_fixed, C.byref(self.t), _stream()))
+        return self.t.value
+
+    def status(self, which=0):
+        n = C.c_int64()
+        self._chk(self.L.sfh_status(self.h, which, C.byref(n), _stream()))
+        return n.value

@@ -1,0 +1,557 @@
+// sfh_api.cu — the C ABI of libsfh (include/sfh.h): mesh handle, role rotation, level drivers.
+// Every step of the hot path runs in the kernels of sfh_kernels*.cu; this file only sequences them.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "sfh_kernels.cuh"
+
+using namespace sfh;
+
+namespace sfh {
+static thread_local std::string g_err;
+void set_error(const std::string& s) { g_err = s; }
+}  // namespace sfh
+
+struct sfh_mesh {
+  HostMesh hm;
+  bool bound = false;
+  char* dev_tables = nullptr;
+  int32_t *d_face_src = nullptr, *d_fslot = nullptr, *d_nbr27 = nullptr, *d_parent = nullptr, *d_child0 = nullptr,
+          *d_coord = nullptr, *d_cf_block = nullptr, *d_cf_face = nullptr, *d_fh_src = nullptr,
+          *d_restrict_list = nullptr, *d_reflux_list = nullptr;
+  int64_t* d_perm = nullptr;
+  double* state[3] = {nullptr, nullptr, nullptr};
+  double *ghost = nullptr, *R = nullptr, *FH = nullptr;
+  unsigned long long* smax = nullptr;   // [MAX_LEVELS] bit patterns of the per-level maximum speed
+  double *dt_dev = nullptr, *t_dev = nullptr;
+  unsigned long long* nbad = nullptr;
+  int role[MAX_LEVELS][3];              // role -> physical state buffer, per level
+  TensorMaps tm[3];                     // per physical state buffer
+  int64_t launches = 0;
+};
+
+namespace {
+
+constexpr size_t ALIGN = 256;
+inline size_t up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
+
+struct WorkLayout {
+  size_t ghost, R, FH, scalars, total;
+};
+WorkLayout work_layout(const HostMesh& hm) {
+  WorkLayout w;
+  const size_t ncf = hm.cf_block.size();
+  w.ghost = 0;
+  w.R = up(w.ghost + ncf * SLAB * 8);
+  w.FH = up(w.R + ncf * REG * 8);
+  w.scalars = up(w.FH + size_t(hm.nfh) * REG * 8);
+  w.total = w.scalars + 4096;
+  return w;
+}
+
+int fail(int code, const std::string& what) {
+  set_error(what);
+  return code;
+}
+int cuda_fail(cudaError_t e, const char* where) {
+  set_error(std::string(where) + ": " + cudaGetErrorString(e));
+  return SFH_ECUDA;
+}
+#define CU(call, where)                                    \
+  do {                                                     \
+    cudaError_t e_ = (call);                               \
+    if (e_ != cudaSuccess) return cuda_fail(e_, where);    \
+  } while (0)
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// Tensor maps of one state buffer seen as a 4-D fp64 tensor [5*nb][8][8][8] (innermost = x); one map
+// per face axis, whose box is the two-layer slab {2,8,8,5}, {8,2,8,5} or {8,8,2,5}.
+int make_tensor_maps(void* base, int64_t nb, TensorMaps& out) {
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  CU(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres), "cudaGetDriverEntryPoint");
+  if (!fn || qres != cudaDriverEntryPointSuccess) return fail(SFH_ECUDA, "cuTensorMapEncodeTiled not available");
+  EncodeTiledFn encode = reinterpret_cast<EncodeTiledFn>(fn);
+  const cuuint64_t dims[4] = {N, N, N, cuuint64_t(NV) * cuuint64_t(nb)};
+  const cuuint64_t strides[3] = {N * 8, N * N * 8, N * N * N * 8};
+  const cuuint32_t estr[4] = {1, 1, 1, 1};
+  for (int axis = 0; axis < 3; ++axis) {
+    cuuint32_t box[4] = {N, N, N, NV};
+    box[axis] = NG;
+    const CUresult r = encode(&out.ax[axis], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                              CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+      char buf[96];
+      snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled failed (CUresult %d)", int(r));
+      return fail(SFH_ECUDA, buf);
+    }
+  }
+  return SFH_OK;
+}
+
+inline cudaStream_t S(void* s) { return reinterpret_cast<cudaStream_t>(s); }
+inline double* role_buf(const sfh_mesh* m, int l, int r) { return m->state[m->role[l][r]]; }
+
+int check_bound(const sfh_mesh* m) {
+  if (!m) return fail(SFH_EINVAL, "null mesh");
+  if (!m->bound) return fail(SFH_ESTATE, "mesh is not bound to state/work buffers (sfh_bind)");
+  return SFH_OK;
+}
+int check_level(const sfh_mesh* m, int level) {
+  if (level < -1 || level >= m->hm.nlev) return fail(SFH_EINVAL, "level out of range");
+  return SFH_OK;
+}
+
+struct Dt {   // a step known on the host, or to be read from device memory
+  double host;
+  const double* dev;
+};
+
+int fill_level(sfh_mesh* m, int l, int which, int interp, double tau, cudaStream_t st) {
+  const HostMesh& hm = m->hm;
+  if (l == 0 || hm.cf_count[l] == 0) return SFH_OK;
+  ProlongParams p;
+  if (interp) { p.C0 = role_buf(m, l - 1, 0); p.C1 = role_buf(m, l - 1, 1); p.C2 = role_buf(m, l - 1, 2); }
+  else { p.C0 = p.C1 = p.C2 = role_buf(m, l - 1, which); }
+  p.ghost = m->ghost;
+  p.cf_block = m->d_cf_block; p.cf_face = m->d_cf_face; p.parent = m->d_parent; p.coord = m->d_coord;
+  p.nbr27 = m->d_nbr27;
+  p.first = int(hm.cf_first[l]); p.count = int(hm.cf_count[l]);
+  p.interp = interp; p.tau = tau;
+  CU(launch_prolong(p, st), "prolong_kernel");
+  m->launches += 1;
+  return SFH_OK;
+}
+
+int stage_level(sfh_mesh* m, int l, int stage, Dt dt, cudaStream_t st) {
+  const HostMesh& hm = m->hm;
+  if (hm.lev_count[l] == 0) return SFH_OK;
+  StageParams p;
+  const int src_role = stage == 0 ? 0 : 1;
+  p.Usrc = role_buf(m, l, src_role);
+  p.Un = role_buf(m, l, 0);
+  p.Udst = role_buf(m, l, stage == 0 ? 1 : 2);
+  p.ghost = m->ghost; p.R = m->R; p.FH = m->FH;
+  p.face_src = m->d_face_src; p.fslot = m->d_fslot;
+  p.dt_dev = dt.dev; p.dt = dt.host; p.h = hm.h[l]; p.gamma = hm.cfg.gamma;
+  p.first = int(hm.lev_first[l]); p.count = int(hm.lev_count[l]);
+  p.use_regs = stage == 1 && (hm.cf_count[l] > 0 || hm.reflux_count[l] > 0);
+  CU(launch_stage(stage, m->tm[m->role[l][src_role]], p, st), "stage_kernel");
+  m->launches += 1;
+  return SFH_OK;
+}
+
+int zero_fine_registers(sfh_mesh* m, int coarse_level, cudaStream_t st) {   // registers of (l, l+1)
+  const HostMesh& hm = m->hm;
+  const int lf = coarse_level + 1;
+  if (lf >= hm.nlev || hm.cf_count[lf] == 0) return SFH_OK;
+  CU(cudaMemsetAsync(m->R + size_t(hm.cf_first[lf]) * REG, 0, size_t(hm.cf_count[lf]) * REG * 8, st), "memset R");
+  return SFH_OK;
+}
+
+int hydro_level(sfh_mesh* m, int l, Dt dt, int interp, double tau, double dtau, cudaStream_t st) {
+  int rc;
+  if ((rc = zero_fine_registers(m, l, st))) return rc;
+  if ((rc = stage_level(m, l, 0, dt, st))) return rc;
+  if ((rc = fill_level(m, l, 1, interp, tau + 0.5 * dtau, st))) return rc;
+  return stage_level(m, l, 1, dt, st);
+}
+
+int flux_correct_level(sfh_mesh* m, int lc, Dt dt, cudaStream_t st) {
+  const HostMesh& hm = m->hm;
+  if (lc + 1 >= hm.nlev || hm.lev_count[lc + 1] == 0) return SFH_OK;
+  CU(launch_restrict(role_buf(m, lc + 1, 0), role_buf(m, lc, 2), m->d_restrict_list + hm.restrict_first[lc],
+                     m->d_child0, int(hm.restrict_count[lc]), st), "restrict_kernel");
+  m->launches += hm.restrict_count[lc] > 0;
+  CU(launch_reflux(role_buf(m, lc, 2), m->R, m->FH, m->d_reflux_list + hm.reflux_first[lc], m->d_fslot, m->d_fh_src,
+                   int(hm.reflux_count[lc]), hm.h[lc], dt.host, dt.dev, st), "reflux_kernel");
+  m->launches += hm.reflux_count[lc] > 0;
+  return SFH_OK;
+}
+
+void rotate(sfh_mesh* m, int l) { std::swap(m->role[l][0], m->role[l][2]); }
+
+int max_speed_level(sfh_mesh* m, int l, cudaStream_t st) {
+  const HostMesh& hm = m->hm;
+  CU(launch_max_speed(role_buf(m, l, 0), int(hm.lev_first[l]), int(hm.lev_count[l]), hm.cfg.gamma, m->smax + l, st),
+     "max_speed_kernel");
+  m->launches += hm.lev_count[l] > 0;
+  return SFH_OK;
+}
+
+int cfl_host(sfh_mesh* m, int level, double* dt_out, cudaStream_t st) {
+  const HostMesh& hm = m->hm;
+  int rc;
+  for (int l = 0; l < hm.nlev; ++l)
+    if ((level < 0 || level == l) && (rc = max_speed_level(m, l, st))) return rc;
+  unsigned long long bits[MAX_LEVELS];
+  CU(cudaMemcpyAsync(bits, m->smax, sizeof bits, cudaMemcpyDeviceToHost, st), "memcpy smax");
+  CU(cudaStreamSynchronize(st), "cudaStreamSynchronize");
+  double dt = INFINITY;
+  for (int l = 0; l < hm.nlev; ++l)
+    if ((level < 0 || level == l) && hm.lev_count[l] > 0) {
+      double s;
+      std::memcpy(&s, &bits[l], 8);
+      dt = std::fmin(dt, hm.cfg.cfl * hm.h[l] / s);
+    }
+  *dt_out = dt;
+  return SFH_OK;
+}
+
+// eq. (14)-(15): smallest n >= 0 with dtH 2^-n <= dt_cfl (reading R18)
+int substep_exponent(double dtH, double dt_cfl) {
+  int n = 0;
+  while (n < 30 && std::ldexp(dtH, -n) > dt_cfl) ++n;
+  return n;
+}
+
+int advance_adaptive(sfh_mesh* m, int l, double dt, double tau, double dtau, int64_t* nupd, cudaStream_t st) {
+  const HostMesh& hm = m->hm;
+  const int interp = l > 0;
+  int rc;
+  if ((rc = fill_level(m, l, 0, interp, tau, st))) return rc;
+  if ((rc = hydro_level(m, l, Dt{dt, nullptr}, interp, tau, dtau, st))) return rc;
+  if (nupd) nupd[l] += 1;
+  if (l + 1 < hm.nlev && hm.lev_count[l + 1] > 0) {
+    double dtc;
+    if ((rc = cfl_host(m, l + 1, &dtc, st))) return rc;
+    const int n = substep_exponent(dt, dtc);
+    const double dtf = std::ldexp(dt, -n);
+    const int nsub = 1 << n;
+    for (int s = 0; s < nsub; ++s)
+      if ((rc = advance_adaptive(m, l + 1, dtf, double(s) / double(nsub), dtf / dt, nupd, st))) return rc;
+    if ((rc = flux_correct_level(m, l, Dt{dt, nullptr}, st))) return rc;
+  }
+  rotate(m, l);
+  return SFH_OK;
+}
+
+int step_sync(sfh_mesh* m, double dt_fixed, cudaStream_t st) {
+  const HostMesh& hm = m->hm;
+  int rc;
+  Dt dt{dt_fixed, nullptr};
+  if (!(dt_fixed > 0.0)) {
+    LevelInfo li;
+    li.nlev = hm.nlev;
+    for (int l = 0; l < hm.nlev; ++l) {
+      li.h[l] = hm.h[l];
+      li.has[l] = hm.lev_count[l] > 0;
+      if ((rc = max_speed_level(m, l, st))) return rc;
+    }
+    CU(launch_dt_finalize(m->smax, li, hm.cfg.cfl, m->dt_dev, m->t_dev, st), "dt_finalize_kernel");
+    m->launches += 1;
+    dt = Dt{0.0, m->dt_dev};
+  }
+  for (int l = 0; l < hm.nlev; ++l) if ((rc = zero_fine_registers(m, l, st))) return rc;
+  for (int l = 0; l < hm.nlev; ++l) if ((rc = fill_level(m, l, 0, 0, 0.0, st))) return rc;
+  for (int l = 0; l < hm.nlev; ++l) if ((rc = stage_level(m, l, 0, dt, st))) return rc;
+  for (int l = 0; l < hm.nlev; ++l) if ((rc = fill_level(m, l, 1, 0, 0.0, st))) return rc;
+  for (int l = 0; l < hm.nlev; ++l) if ((rc = stage_level(m, l, 1, dt, st))) return rc;
+  for (int l = hm.nlev - 1; l >= 0; --l) {
+    if ((rc = flux_correct_level(m, l, dt, st))) return rc;
+    rotate(m, l);
+  }
+  return SFH_OK;
+}
+
+}  // namespace
+
+// =====================================================================================================
+extern "C" {
+
+const char* sfh_last_error(void) { return g_err.c_str(); }
+
+int sfh_create_mesh(const sfh_config* cfg, int64_t nblocks, const int32_t* level, const int32_t* ijk,
+                    sfh_mesh** out) {
+  if (!cfg || !out) return fail(SFH_EINVAL, "null argument");
+  *out = nullptr;
+  sfh_mesh* m = new (std::nothrow) sfh_mesh;
+  if (!m) return fail(SFH_ENOMEM, "out of host memory");
+  std::string err;
+  int rc;
+  try {
+    rc = build_host_mesh(*cfg, nblocks, level, ijk, m->hm, err);
+  } catch (const std::bad_alloc&) {
+    delete m;
+    return fail(SFH_ENOMEM, "out of host memory");
+  }
+  if (rc != SFH_OK) {
+    delete m;
+    return fail(rc, err);
+  }
+  for (int l = 0; l < MAX_LEVELS; ++l) for (int r = 0; r < 3; ++r) m->role[l][r] = r;
+  *out = m;
+  return SFH_OK;
+}
+
+int sfh_destroy_mesh(sfh_mesh* m) {
+  if (!m) return SFH_OK;
+  if (m->dev_tables) cudaFree(m->dev_tables);
+  delete m;
+  return SFH_OK;
+}
+
+int64_t sfh_num_blocks(const sfh_mesh* m) { return m ? m->hm.nb : 0; }
+
+int sfh_level_range(const sfh_mesh* m, int level, int64_t* first, int64_t* count) {
+  if (!m || level < 0 || level >= m->hm.nlev) return fail(SFH_EINVAL, "level out of range");
+  if (first) *first = m->hm.lev_first[level];
+  if (count) *count = m->hm.lev_count[level];
+  return SFH_OK;
+}
+
+int sfh_block_order(const sfh_mesh* m, int64_t* perm) {
+  if (!m || !perm) return fail(SFH_EINVAL, "null argument");
+  std::memcpy(perm, m->hm.perm.data(), sizeof(int64_t) * size_t(m->hm.nb));
+  return SFH_OK;
+}
+
+int sfh_num_faces(const sfh_mesh* m, int64_t* n_fine_faces, int64_t* n_coarse_faces) {
+  if (!m) return fail(SFH_EINVAL, "null mesh");
+  if (n_fine_faces) *n_fine_faces = int64_t(m->hm.cf_block.size());
+  if (n_coarse_faces) *n_coarse_faces = m->hm.nfh;
+  return SFH_OK;
+}
+
+double sfh_cell_width(const sfh_mesh* m, int level) {
+  if (!m || level < 0 || level >= m->hm.nlev) return 0.0;
+  return m->hm.h[level];
+}
+
+int64_t sfh_state_bytes(const sfh_mesh* m) { return m ? int64_t(up(size_t(m->hm.nb) * BLK * 8)) : 0; }
+int64_t sfh_work_bytes(const sfh_mesh* m) { return m ? int64_t(work_layout(m->hm).total) : 0; }
+int64_t sfh_launch_count(const sfh_mesh* m) { return m ? m->launches : 0; }
+
+int sfh_bind(sfh_mesh* m, void* d_state0, void* d_state1, void* d_state2, void* d_work) {
+  if (!m || !d_state0 || !d_state1 || !d_state2 || !d_work) return fail(SFH_EINVAL, "null argument");
+  void* ptrs[4] = {d_state0, d_state1, d_state2, d_work};
+  for (void* p : ptrs)
+    if (reinterpret_cast<uintptr_t>(p) % ALIGN) return fail(SFH_EINVAL, "buffers must be 256-byte aligned");
+  int ndev = 0;
+  CU(cudaGetDeviceCount(&ndev), "cudaGetDeviceCount");
+  if (ndev == 0) return fail(SFH_ECUDA, "no CUDA device");
+  const HostMesh& hm = m->hm;
+  if (!m->dev_tables) {
+    // one allocation for all tables
+    struct Item { const void* src; size_t bytes; void** dst; };
+    const Item items[] = {
+        {hm.face_src.data(), hm.face_src.size() * 4, (void**)&m->d_face_src},
+        {hm.fslot.data(), hm.fslot.size() * 4, (void**)&m->d_fslot},
+        {hm.nbr27.data(), hm.nbr27.size() * 4, (void**)&m->d_nbr27},
+        {hm.parent.data(), hm.parent.size() * 4, (void**)&m->d_parent},
+        {hm.child0.data(), hm.child0.size() * 4, (void**)&m->d_child0},
+        {hm.coord.data(), hm.coord.size() * 4, (void**)&m->d_coord},
+        {hm.cf_block.data(), hm.cf_block.size() * 4, (void**)&m->d_cf_block},
+        {hm.cf_face.data(), hm.cf_face.size() * 4, (void**)&m->d_cf_face},
+        {hm.fh_src.data(), hm.fh_src.size() * 4, (void**)&m->d_fh_src},
+        {hm.restrict_list.data(), hm.restrict_list.size() * 4, (void**)&m->d_restrict_list},
+        {hm.reflux_list.data(), hm.reflux_list.size() * 4, (void**)&m->d_reflux_list},
+        {hm.perm.data(), hm.perm.size() * 8, (void**)&m->d_perm},
+    };
+    size_t total = 0;
+    for (const Item& it : items) total += up(it.bytes + 1);
+    cudaError_t e = cudaMalloc((void**)&m->dev_tables, total);
+    if (e != cudaSuccess) { m->dev_tables = nullptr; set_error("cudaMalloc of mesh tables failed"); return SFH_ENOMEM; }
+    size_t off = 0;
+    for (const Item& it : items) {
+      *it.dst = m->dev_tables + off;
+      if (it.bytes) CU(cudaMemcpy(m->dev_tables + off, it.src, it.bytes, cudaMemcpyHostToDevice), "upload tables");
+      off += up(it.bytes + 1);
+    }
+    CU(configure_kernels(), "cudaFuncSetAttribute");
+  }
+  m->state[0] = static_cast<double*>(d_state0);
+  m->state[1] = static_cast<double*>(d_state1);
+  m->state[2] = static_cast<double*>(d_state2);
+  const WorkLayout w = work_layout(hm);
+  char* wb = static_cast<char*>(d_work);
+  CU(cudaMemset(wb, 0, w.total), "zero work buffer");
+  m->ghost = reinterpret_cast<double*>(wb + w.ghost);
+  m->R = reinterpret_cast<double*>(wb + w.R);
+  m->FH = reinterpret_cast<double*>(wb + w.FH);
+  m->smax = reinterpret_cast<unsigned long long*>(wb + w.scalars);
+  m->dt_dev = reinterpret_cast<double*>(wb + w.scalars + 256);
+  m->t_dev = reinterpret_cast<double*>(wb + w.scalars + 512);
+  m->nbad = reinterpret_cast<unsigned long long*>(wb + w.scalars + 768);
+  for (int b = 0; b < 3; ++b) {
+    const int rc = make_tensor_maps(m->state[b], hm.nb, m->tm[b]);
+    if (rc) return rc;
+  }
+  for (int l = 0; l < MAX_LEVELS; ++l) for (int r = 0; r < 3; ++r) m->role[l][r] = r;
+  m->bound = true;
+  return SFH_OK;
+}
+
+int sfh_set_state(sfh_mesh* m, int which, const double* d_U, void* stream) {
+  int rc = check_bound(m);
+  if (rc) return rc;
+  if (which < 0 || which > 2 || !d_U) return fail(SFH_EINVAL, "bad argument");
+  for (int l = 0; l < m->hm.nlev; ++l) {
+    CU(launch_permute(d_U, role_buf(m, l, which), m->d_perm, int(m->hm.lev_first[l]), int(m->hm.lev_count[l]), 1,
+                      S(stream)), "permute_kernel");
+    m->launches += m->hm.lev_count[l] > 0;
+  }
+  return SFH_OK;
+}
+
+int sfh_get_state(sfh_mesh* m, int which, double* d_U, void* stream) {
+  int rc = check_bound(m);
+  if (rc) return rc;
+  if (which < 0 || which > 2 || !d_U) return fail(SFH_EINVAL, "bad argument");
+  for (int l = 0; l < m->hm.nlev; ++l) {
+    CU(launch_permute(role_buf(m, l, which), d_U, m->d_perm, int(m->hm.lev_first[l]), int(m->hm.lev_count[l]), 0,
+                      S(stream)), "permute_kernel");
+    m->launches += m->hm.lev_count[l] > 0;
+  }
+  return SFH_OK;
+}
+
+int sfh_fill_ghosts(sfh_mesh* m, int level, int which, int interp, double tau, void* stream) {
+  int rc = check_bound(m);
+  if (rc || (rc = check_level(m, level))) return rc;
+  if (which < 0 || which > 2) return fail(SFH_EINVAL, "which must be 0, 1 or 2");
+  for (int l = 0; l < m->hm.nlev; ++l)
+    if ((level < 0 || level == l) && (rc = fill_level(m, l, which, interp, tau, S(stream)))) return rc;
+  return SFH_OK;
+}
+
+int sfh_get_ghosted(sfh_mesh* m, int which, double* d_G, void* stream) {
+  int rc = check_bound(m);
+  if (rc) return rc;
+  if (which < 0 || which > 2 || !d_G) return fail(SFH_EINVAL, "bad argument");
+  for (int l = 0; l < m->hm.nlev; ++l) {
+    CU(launch_ghosted(role_buf(m, l, which), m->ghost, m->d_face_src, m->d_perm, int(m->hm.lev_first[l]),
+                      int(m->hm.lev_count[l]), d_G, S(stream)), "ghosted_kernel");
+    m->launches += m->hm.lev_count[l] > 0;
+  }
+  return SFH_OK;
+}
+
+int sfh_cfl_dt(sfh_mesh* m, int level, double* dt_host, void* stream) {
+  int rc = check_bound(m);
+  if (rc || (rc = check_level(m, level))) return rc;
+  if (!dt_host) return fail(SFH_EINVAL, "null dt_host");
+  return cfl_host(m, level, dt_host, S(stream));
+}
+
+int sfh_hydro_step(sfh_mesh* m, int level, double dt, int interp, double tau, double dtau, void* stream) {
+  int rc = check_bound(m);
+  if (rc || (rc = check_level(m, level))) return rc;
+  if (!(dt > 0.0)) return fail(SFH_EINVAL, "dt must be positive");
+  const Dt d{dt, nullptr};
+  cudaStream_t st = S(stream);
+  if (level >= 0) return hydro_level(m, level, d, interp, tau, dtau, st);
+  // all levels, stage by stage (synchronous mode)
+  for (int l = 0; l < m->hm.nlev; ++l) if ((rc = zero_fine_registers(m, l, st))) return rc;
+  for (int l = 0; l < m->hm.nlev; ++l) if ((rc = stage_level(m, l, 0, d, st))) return rc;
+  for (int l = 0; l < m->hm.nlev; ++l) if ((rc = fill_level(m, l, 1, interp, tau + 0.5 * dtau, st))) return rc;
+  for (int l = 0; l < m->hm.nlev; ++l) if ((rc = stage_level(m, l, 1, d, st))) return rc;
+  return SFH_OK;
+}
+
+int sfh_flux_correct(sfh_mesh* m, int coarse_level, double dt_coarse, void* stream) {
+  int rc = check_bound(m);
+  if (rc) return rc;
+  if (coarse_level < 0 || coarse_level >= m->hm.nlev) return fail(SFH_EINVAL, "level out of range");
+  return flux_correct_level(m, coarse_level, Dt{dt_coarse, nullptr}, S(stream));
+}
+
+int sfh_restrict(sfh_mesh* m, int coarse_level, int src_role, int dst_role, void* stream) {
+  int rc = check_bound(m);
+  if (rc) return rc;
+  const HostMesh& hm = m->hm;
+  if (coarse_level < 0 || coarse_level >= hm.nlev || src_role < 0 || src_role > 2 || dst_role < 0 || dst_role > 2)
+    return fail(SFH_EINVAL, "bad argument");
+  if (coarse_level + 1 >= hm.nlev || hm.restrict_count[coarse_level] == 0) return SFH_OK;
+  CU(launch_restrict(role_buf(m, coarse_level + 1, src_role), role_buf(m, coarse_level, dst_role),
+                     m->d_restrict_list + hm.restrict_first[coarse_level], m->d_child0,
+                     int(hm.restrict_count[coarse_level]), S(stream)), "restrict_kernel");
+  m->launches += 1;
+  return SFH_OK;
+}
+
+int sfh_end_step(sfh_mesh* m, int level) {
+  int rc = check_bound(m);
+  if (rc || (rc = check_level(m, level))) return rc;
+  for (int l = 0; l < m->hm.nlev; ++l) if (level < 0 || level == l) rotate(m, l);
+  return SFH_OK;
+}
+
+int sfh_advance(sfh_mesh* m, int ncoarse_steps, int mode, double dt_fixed, double* t_host, int64_t* nupd_host,
+                void* stream) {
+  int rc = check_bound(m);
+  if (rc) return rc;
+  if (ncoarse_steps < 0 || (mode != 0 && mode != 1)) return fail(SFH_EINVAL, "bad argument");
+  cudaStream_t st = S(stream);
+  const HostMesh& hm = m->hm;
+  double t = 0.0;
+  if (mode == 0) {
+    CU(cudaMemsetAsync(m->t_dev, 0, 8, st), "memset t");
+    for (int s = 0; s < ncoarse_steps; ++s) {
+      if ((rc = step_sync(m, dt_fixed, st))) return rc;
+      if (dt_fixed > 0.0) t += dt_fixed;
+      if (nupd_host) for (int l = 0; l < hm.nlev; ++l) nupd_host[l] += hm.lev_count[l] > 0;
+    }
+    double tdev = 0.0;
+    CU(cudaMemcpyAsync(&tdev, m->t_dev, 8, cudaMemcpyDeviceToHost, st), "memcpy t");
+    CU(cudaStreamSynchronize(st), "cudaStreamSynchronize");
+    t += tdev;
+  } else {
+    for (int s = 0; s < ncoarse_steps; ++s) {
+      double dt = dt_fixed;
+      if (!(dt > 0.0) && (rc = cfl_host(m, 0, &dt, st))) return rc;
+      if ((rc = advance_adaptive(m, 0, dt, 0.0, 0.0, nupd_host, st))) return rc;
+      t += dt;
+    }
+    CU(cudaStreamSynchronize(st), "cudaStreamSynchronize");
+  }
+  if (t_host) *t_host += t;
+  return SFH_OK;
+}
+
+int sfh_advance_host(sfh_mesh* m, const double* h_in, double* h_out, int ncoarse_steps, int mode, double dt_fixed,
+                     double* t_host, void* stream) {
+  int rc = check_bound(m);
+  if (rc) return rc;
+  if (!h_in || !h_out) return fail(SFH_EINVAL, "null host buffer");
+  cudaStream_t st = S(stream);
+  const size_t bytes = size_t(m->hm.nb) * BLK * 8;
+  // role 1 (U^{n+1/2}) of level 0 is scratch between steps: use its buffer for staging in caller order
+  double* stage = m->state[m->role[0][1]];
+  for (int l = 1; l < m->hm.nlev; ++l)
+    if (m->role[l][1] != m->role[0][1]) return fail(SFH_ESTATE, "internal: role 1 buffers differ between levels");
+  CU(cudaMemcpyAsync(stage, h_in, bytes, cudaMemcpyHostToDevice, st), "H2D");
+  if ((rc = sfh_set_state(m, 0, stage, stream))) return rc;
+  if ((rc = sfh_advance(m, ncoarse_steps, mode, dt_fixed, t_host, nullptr, stream))) return rc;
+  if ((rc = sfh_get_state(m, 0, stage, stream))) return rc;
+  CU(cudaMemcpyAsync(h_out, stage, bytes, cudaMemcpyDeviceToHost, st), "D2H");
+  CU(cudaStreamSynchronize(st), "cudaStreamSynchronize");
+  return SFH_OK;
+}
+
+int sfh_status(sfh_mesh* m, int which, int64_t* n_bad_cells, void* stream) {
+  int rc = check_bound(m);
+  if (rc) return rc;
+  if (which < 0 || which > 2 || !n_bad_cells) return fail(SFH_EINVAL, "bad argument");
+  cudaStream_t st = S(stream);
+  CU(cudaMemsetAsync(m->nbad, 0, 8, st), "memset");
+  for (int l = 0; l < m->hm.nlev; ++l) {
+    CU(launch_count_bad(role_buf(m, l, which), int(m->hm.lev_first[l]), int(m->hm.lev_count[l]), m->hm.cfg.gamma,
+                        m->nbad, st), "count_bad_kernel");
+    m->launches += m->hm.lev_count[l] > 0;
+  }
+  unsigned long long n = 0;
+  CU(cudaMemcpyAsync(&n, m->nbad, 8, cudaMemcpyDeviceToHost, st), "memcpy");
+  CU(cudaStreamSynchronize(st), "cudaStreamSynchronize");
+  *n_bad_cells = int64_t(n);
+  return SFH_OK;
+}
+
+}  // extern "C"

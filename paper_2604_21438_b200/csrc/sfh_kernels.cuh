@@ -1,0 +1,73 @@
+// sfh_kernels.cuh — launch wrappers of the CUDA kernels of libsfh (defined in sfh_kernels.cu).
+#pragma once
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include "sfh_internal.h"
+
+namespace sfh {
+
+struct StageParams {
+  const double* Usrc;   // state the stage differentiates: U^n (predictor) or U^{n+1/2} (corrector)
+  const double* Un;     // U^n, the state that is updated
+  double* Udst;         // U^{n+1/2} (predictor) or U^{n+1} (corrector)
+  const double* ghost;  // coarse-fine ghost slabs [ncf][5][2 layers x 64]
+  double* R;            // fine-side flux registers  [ncf][5][64]
+  double* FH;           // coarse-side flux registers [nfh][5][64]
+  const int32_t* face_src;
+  const int32_t* fslot;
+  const double* dt_dev;  // if non-null the step is read from device memory
+  double dt;
+  double h;
+  double gamma;
+  int first, count;      // slot range of the level
+  int use_regs;          // corrector: the level has flux-register faces
+};
+
+struct TensorMaps {      // tensor maps of ONE state buffer, one per face axis (box = 2-layer slab)
+  CUtensorMap ax[3];
+};
+
+struct ProlongParams {
+  const double* C0;      // coarse level: role `which` (interp = 0) or role 0 (interp = 1)
+  const double* C1;      // coarse role 1 (interp = 1)
+  const double* C2;      // coarse role 2 (interp = 1)
+  double* ghost;
+  const int32_t* cf_block;
+  const int32_t* cf_face;
+  const int32_t* parent;
+  const int32_t* coord;
+  const int32_t* nbr27;
+  int first, count;      // slab range of the fine level
+  int interp;
+  double tau;
+};
+
+cudaError_t launch_stage(int stage, const TensorMaps& tm, const StageParams& p, cudaStream_t st);
+cudaError_t launch_prolong(const ProlongParams& p, cudaStream_t st);
+cudaError_t launch_restrict(const double* Ufine, double* Ucoarse, const int32_t* list, const int32_t* child0,
+                            int count, cudaStream_t st);
+cudaError_t launch_reflux(double* U, const double* R, const double* FH, const int32_t* list, const int32_t* fslot,
+                          const int32_t* fh_src, int count, double h, double dt, const double* dt_dev,
+                          cudaStream_t st);
+cudaError_t launch_max_speed(const double* U, int first, int count, double gamma, unsigned long long* smax_bits,
+                             cudaStream_t st);
+struct LevelInfo {
+  double h[MAX_LEVELS];
+  int has[MAX_LEVELS];
+  int nlev;
+};
+// dt = min_l cfl*h_l/smax_l over levels with blocks; *dt_dev = dt; *t_dev += dt
+cudaError_t launch_dt_finalize(const unsigned long long* smax_bits, const LevelInfo& li, double cfl, double* dt_dev,
+                               double* t_dev, cudaStream_t st);
+cudaError_t launch_count_bad(const double* U, int first, int count, double gamma, unsigned long long* nbad,
+                             cudaStream_t st);
+// dst[slot][...] = src[perm[slot]][...] (to_internal) or the inverse, for slots [first, first+count)
+cudaError_t launch_permute(const double* src, double* dst, const int64_t* perm, int first, int count, int to_internal,
+                           cudaStream_t st);
+cudaError_t launch_ghosted(const double* U, const double* ghost, const int32_t* face_src, const int64_t* perm,
+                           int first, int count, double* G, cudaStream_t st);
+cudaError_t configure_kernels();
+
+}  // namespace sfh

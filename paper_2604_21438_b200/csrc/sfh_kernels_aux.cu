@@ -1,0 +1,321 @@
+// sfh_kernels_aux.cu — the smaller kernels of libsfh (sm_100a): coarse-fine ghost prolongation (a3),
+// restriction (a8), reflux (a9), CFL reduction (a10), status, layout permutation, ghosted export.
+#include <cmath>
+
+#include "sfh_device.cuh"
+#include "sfh_kernels.cuh"
+
+namespace sfh {
+
+// =====================================================================================================
+// a3: ghost slabs of coarse-fine faces.  One CTA of 128 threads per slab, one thread per ghost cell.
+// Fine ghost cell -> coarse cell (index >> 1) of the parent's neighbourhood; per variable the coarse
+// value and its 6 axis neighbours (each optionally interpolated in time, eq. 16) give minmod slopes
+// and the fine value Q + sum_d (+-1/4) slope_d (reading R3).
+// =====================================================================================================
+__global__ void __launch_bounds__(128) prolong_kernel(const ProlongParams p) {
+  const int slot = p.first + blockIdx.x;
+  const int F = p.cf_block[slot], f = p.cf_face[slot], axis = f >> 1, side = f & 1;
+  const int P = p.parent[F];
+  const int oct[3] = {p.coord[3 * F] & 1, p.coord[3 * F + 1] & 1, p.coord[3 * F + 2] & 1};
+  const int r = threadIdx.x;
+  int fc[3];   // fine local coordinates of this ghost cell, slab layouts as staged by the stage kernels
+  if (axis == 0) {
+    const int ll = r & 1;
+    fc[0] = side ? N + ll : ll - NG; fc[1] = (r >> 1) & 7; fc[2] = r >> 4;
+  } else if (axis == 1) {
+    const int ll = (r >> 3) & 1;
+    fc[0] = r & 7; fc[1] = side ? N + ll : ll - NG; fc[2] = r >> 4;
+  } else {
+    const int ll = r >> 6;
+    fc[0] = r & 7; fc[1] = (r >> 3) & 7; fc[2] = side ? N + ll : ll - NG;
+  }
+  int cc[3];
+  double sig[3];
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    cc[d] = oct[d] * 4 + (fc[d] >> 1);          // arithmetic shift: -2,-1 -> -1
+    sig[d] = (fc[d] & 1) ? 0.25 : -0.25;
+  }
+  const int32_t* nb = p.nbr27 + size_t(P) * 27;
+  // does the parent touch an outflow boundary?  (face-region codes)
+  bool out_lo[3], out_hi[3];
+  out_lo[0] = nb[12] == NBR_OUTSIDE; out_hi[0] = nb[14] == NBR_OUTSIDE;
+  out_lo[1] = nb[10] == NBR_OUTSIDE; out_hi[1] = nb[16] == NBR_OUTSIDE;
+  out_lo[2] = nb[4] == NBR_OUTSIDE;  out_hi[2] = nb[22] == NBR_OUTSIDE;
+
+  auto locate = [&](int c0, int c1, int c2) -> long long {   // offset of variable 0 of a coarse cell, or -1
+    int c[3] = {c0, c1, c2}, rg[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      rg[d] = 0;
+      if (c[d] < 0) { if (out_lo[d]) c[d] = 0; else { rg[d] = -1; c[d] += N; } }
+      else if (c[d] >= N) { if (out_hi[d]) c[d] = N - 1; else { rg[d] = 1; c[d] -= N; } }
+    }
+    const int Q = nb[(rg[2] + 1) * 9 + (rg[1] + 1) * 3 + (rg[0] + 1)];
+    if (Q < 0) return -1;
+    return (long long)Q * BLK + (c[2] * 8 + c[1]) * 8 + c[0];
+  };
+  long long o[7];
+  o[0] = locate(cc[0], cc[1], cc[2]);
+  o[1] = locate(cc[0] + 1, cc[1], cc[2]); o[2] = locate(cc[0] - 1, cc[1], cc[2]);
+  o[3] = locate(cc[0], cc[1] + 1, cc[2]); o[4] = locate(cc[0], cc[1] - 1, cc[2]);
+  o[5] = locate(cc[0], cc[1], cc[2] + 1); o[6] = locate(cc[0], cc[1], cc[2] - 1);
+  bool ok = true;
+#pragma unroll
+  for (int s = 0; s < 7; ++s) ok = ok && o[s] >= 0;
+  double* out = p.ghost + size_t(slot) * SLAB + r;
+#pragma unroll
+  for (int v = 0; v < NV; ++v) {
+    double q[7];
+#pragma unroll
+    for (int s = 0; s < 7; ++s) {
+      if (!ok) { q[s] = nan(""); continue; }
+      const long long a = o[s] + v * NC;
+      q[s] = p.interp ? time_interp(p.C0[a], p.C1[a], p.C2[a], p.tau) : p.C0[a];
+    }
+    double val = q[0];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) val = val + sig[d] * minmod(q[1 + 2 * d] - q[0], q[0] - q[2 + 2 * d]);
+    out[v * NG * FACE] = val;
+  }
+}
+
+cudaError_t launch_prolong(const ProlongParams& p, cudaStream_t st) {
+  if (p.count <= 0) return cudaSuccess;
+  prolong_kernel<<<p.count, 128, 0, st>>>(p);
+  return cudaGetLastError();
+}
+
+// =====================================================================================================
+// a8: restriction.  One CTA per covered block, one thread per coarse cell: mean of the 8 fine cells
+// in the fixed order cx fastest (reading R15).
+// =====================================================================================================
+__global__ void __launch_bounds__(NC) restrict_kernel(const double* __restrict__ Uf, double* __restrict__ Uc,
+                                                      const int32_t* __restrict__ list,
+                                                      const int32_t* __restrict__ child0) {
+  const int b = list[blockIdx.x];
+  const int t = threadIdx.x, i = t & 7, j = (t >> 3) & 7, k = t >> 6;
+  const int child = child0[b] + (i >> 2) + 2 * (j >> 2) + 4 * (k >> 2);
+  const int fi = 2 * (i & 3), fj = 2 * (j & 3), fk = 2 * (k & 3);
+  const double* src = Uf + size_t(child) * BLK;
+  double* dst = Uc + size_t(b) * BLK + t;
+#pragma unroll
+  for (int v = 0; v < NV; ++v) {
+    double sum = 0.0;
+#pragma unroll
+    for (int c = 0; c < 8; ++c)
+      sum += src[v * NC + ((fk + ((c >> 2) & 1)) * 8 + fj + ((c >> 1) & 1)) * 8 + fi + (c & 1)];
+    dst[v * NC] = 0.125 * sum;
+  }
+}
+
+cudaError_t launch_restrict(const double* Ufine, double* Ucoarse, const int32_t* list, const int32_t* child0, int count,
+                            cudaStream_t st) {
+  if (count <= 0) return cudaSuccess;
+  restrict_kernel<<<count, NC, 0, st>>>(Ufine, Ucoarse, list, child0);
+  return cudaGetLastError();
+}
+
+// =====================================================================================================
+// a9: reflux (Berger & Colella 1989 as cited).  One CTA of 64 threads per coarse
+// leaf block that owns corrected faces; faces in the fixed order x-, x+, y-, y+, z-, z+, one thread per
+// face cell, fine-face sum in fixed order: deterministic, no atomics.
+// =====================================================================================================
+__global__ void __launch_bounds__(FACE) reflux_kernel(double* __restrict__ U, const double* __restrict__ R,
+                                                      const double* __restrict__ FH,
+                                                      const int32_t* __restrict__ list,
+                                                      const int32_t* __restrict__ fslot,
+                                                      const int32_t* __restrict__ fh_src, double h, double dt_host,
+                                                      const double* __restrict__ dt_dev) {
+  const int b = list[blockIdx.x];
+  const int t = threadIdx.x, ta = t & 7, tb = t >> 3;
+  const double dt = dt_dev ? *dt_dev : dt_host;
+  double* Ub = U + size_t(b) * BLK;
+  for (int f = 0; f < 6; ++f) {
+    const int fs = fslot[b * 6 + f];
+    if (fs >= 0) {
+      const int d = f >> 1, side = f & 1, c = side ? N - 1 : 0;
+      const double s = side ? 1.0 : -1.0;
+      const int cell = d == 0 ? (tb * 8 + ta) * 8 + c : d == 1 ? (tb * 8 + c) * 8 + ta : (c * 8 + tb) * 8 + ta;
+      const int slot = fh_src[fs * 4 + (ta >> 2) + 2 * (tb >> 2)];
+      const int fa = 2 * (ta & 3), fb = 2 * (tb & 3);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) {
+        const double* r = R + size_t(slot) * REG + v * FACE;
+        double sumR = 0.0;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) sumR += r[(fb + (q >> 1)) * 8 + fa + (q & 1)];
+        const double FHv = FH[size_t(fs) * REG + v * FACE + t];
+        Ub[v * NC + cell] = Ub[v * NC + cell] - (s / h) * (0.25 * sumR - dt * FHv);
+      }
+    }
+    __syncthreads();
+  }
+}
+
+cudaError_t launch_reflux(double* U, const double* R, const double* FH, const int32_t* list, const int32_t* fslot,
+                          const int32_t* fh_src, int count, double h, double dt, const double* dt_dev,
+                          cudaStream_t st) {
+  if (count <= 0) return cudaSuccess;
+  reflux_kernel<<<count, FACE, 0, st>>>(U, R, FH, list, fslot, fh_src, h, dt, dt_dev);
+  return cudaGetLastError();
+}
+
+// =====================================================================================================
+// a10: CFL reduction ("grid-level reductions"; reading R16).  Per-thread running max,
+// warp-shuffle max, one atomicMax per CTA on the bit pattern (positive doubles order like integers).
+// =====================================================================================================
+__device__ __forceinline__ double warp_max(double x) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) x = fmax(x, __shfl_xor_sync(0xffffffffu, x, o));
+  return x;
+}
+
+__global__ void __launch_bounds__(256) max_speed_kernel(const double* __restrict__ U, int first, int count, double gamma,
+                                                        unsigned long long* smax_bits) {
+  const double gm1 = gamma - 1.0;
+  double smax = 0.0;
+  for (int b = blockIdx.x; b < count; b += gridDim.x) {
+    const double* Ub = U + size_t(first + b) * BLK;
+#pragma unroll
+    for (int c = threadIdx.x; c < NC; c += 256) {
+      double u[5], w[5];
+#pragma unroll
+      for (int v = 0; v < NV; ++v) u[v] = Ub[v * NC + c];
+      cons_to_prim(u, gm1, w);
+      const double cs = sound_speed(gamma, w[4], w[0]);
+      const double s = fmax(fmax(fabs(w[1]), fabs(w[2])), fabs(w[3])) + cs;
+      if (s > smax) smax = s;
+    }
+  }
+  smax = warp_max(smax);
+  __shared__ double wm[8];
+  if ((threadIdx.x & 31) == 0) wm[threadIdx.x >> 5] = smax;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    double x = threadIdx.x < 8 ? wm[threadIdx.x] : 0.0;
+    x = warp_max(x);
+    if (threadIdx.x == 0) atomicMax(smax_bits, (unsigned long long)__double_as_longlong(x));
+  }
+}
+
+cudaError_t launch_max_speed(const double* U, int first, int count, double gamma, unsigned long long* smax_bits,
+                             cudaStream_t st) {
+  cudaError_t e = cudaMemsetAsync(smax_bits, 0, sizeof(unsigned long long), st);
+  if (e != cudaSuccess || count <= 0) return e;
+  const int grid = count < 148 * 8 ? count : 148 * 8;
+  max_speed_kernel<<<grid, 256, 0, st>>>(U, first, count, gamma, smax_bits);
+  return cudaGetLastError();
+}
+
+__global__ void dt_finalize_kernel(const unsigned long long* smax_bits, LevelInfo li, double cfl, double* dt_dev,
+                                   double* t_dev) {
+  double dt = INFINITY;
+  for (int l = 0; l < li.nlev; ++l)
+    if (li.has[l]) dt = fmin(dt, cfl * li.h[l] / __longlong_as_double((long long)smax_bits[l]));
+  *dt_dev = dt;
+  *t_dev += dt;
+}
+
+cudaError_t launch_dt_finalize(const unsigned long long* smax_bits, const LevelInfo& li, double cfl, double* dt_dev,
+                               double* t_dev, cudaStream_t st) {
+  dt_finalize_kernel<<<1, 1, 0, st>>>(smax_bits, li, cfl, dt_dev, t_dev);
+  return cudaGetLastError();
+}
+
+// =====================================================================================================
+// status: cells with rho <= 0, P <= 0 or NaN (reading R28: reported, never floored)
+// =====================================================================================================
+__global__ void __launch_bounds__(256) count_bad_kernel(const double* __restrict__ U, int first, int count, double gamma,
+                                                        unsigned long long* nbad) {
+  const double gm1 = gamma - 1.0;
+  unsigned int bad = 0;
+  for (int b = blockIdx.x; b < count; b += gridDim.x) {
+    const double* Ub = U + size_t(first + b) * BLK;
+    for (int c = threadIdx.x; c < NC; c += 256) {
+      double u[5], w[5];
+#pragma unroll
+      for (int v = 0; v < NV; ++v) u[v] = Ub[v * NC + c];
+      cons_to_prim(u, gm1, w);
+      if (!(w[0] > 0.0) || !(w[4] > 0.0)) ++bad;
+    }
+  }
+  bad = __reduce_add_sync(0xffffffffu, bad);
+  if ((threadIdx.x & 31) == 0 && bad) atomicAdd(nbad, (unsigned long long)bad);
+}
+
+cudaError_t launch_count_bad(const double* U, int first, int count, double gamma, unsigned long long* nbad,
+                             cudaStream_t st) {
+  if (count <= 0) return cudaSuccess;
+  const int grid = count < 148 * 8 ? count : 148 * 8;
+  count_bad_kernel<<<grid, 256, 0, st>>>(U, first, count, gamma, nbad);
+  return cudaGetLastError();
+}
+
+// =====================================================================================================
+// caller layout <-> internal layout (block permutation only; both are interior-only [5][8][8][8])
+// =====================================================================================================
+__global__ void __launch_bounds__(256) permute_kernel(const double2* __restrict__ src, double2* __restrict__ dst,
+                                                      const int64_t* __restrict__ perm, int first, int to_internal) {
+  const int s = first + blockIdx.x;
+  const size_t a = size_t(s) * (BLK / 2), b = size_t(perm[s]) * (BLK / 2);
+  const double2* from = src + (to_internal ? b : a);
+  double2* to = dst + (to_internal ? a : b);
+  for (int t = threadIdx.x; t < BLK / 2; t += 256) to[t] = from[t];
+}
+
+cudaError_t launch_permute(const double* src, double* dst, const int64_t* perm, int first, int count, int to_internal,
+                           cudaStream_t st) {
+  if (count <= 0) return cudaSuccess;
+  permute_kernel<<<count, 256, 0, st>>>(reinterpret_cast<const double2*>(src), reinterpret_cast<double2*>(dst), perm,
+                                        first, to_internal);
+  return cudaGetLastError();
+}
+
+// =====================================================================================================
+// ghosted export (parity tests of the ghost fill): what the stage kernels stage, as 12^3 blocks
+// =====================================================================================================
+__global__ void __launch_bounds__(256) ghosted_kernel(const double* __restrict__ U, const double* __restrict__ ghost,
+                                                      const int32_t* __restrict__ face_src,
+                                                      const int64_t* __restrict__ perm, int first,
+                                                      double* __restrict__ G) {
+  constexpr int M = N + 2 * NG;
+  const int s = first + blockIdx.x;
+  double* out = G + size_t(perm[s]) * NV * M * M * M;
+  for (int t = threadIdx.x; t < NV * M * M * M; t += 256) {
+    const int v = t / (M * M * M), c = t % (M * M * M);
+    const int i = c % M - NG, j = (c / M) % M - NG, k = c / (M * M) - NG;
+    const int o[3] = {i < 0 ? -1 : i >= N ? 1 : 0, j < 0 ? -1 : j >= N ? 1 : 0, k < 0 ? -1 : k >= N ? 1 : 0};
+    const int nout = (o[0] != 0) + (o[1] != 0) + (o[2] != 0);
+    double val;
+    if (nout == 0) val = U[size_t(s) * BLK + v * NC + (k * 8 + j) * 8 + i];
+    else if (nout > 1) val = nan("");
+    else {
+      const int axis = o[0] ? 0 : o[1] ? 1 : 2, side = o[axis] > 0;
+      const int src = face_src[s * 6 + 2 * axis + side];
+      int q[3] = {i, j, k};
+      if (src == SRC_OUTFLOW) {
+        q[axis] = side ? N - 1 : 0;
+        val = U[size_t(s) * BLK + v * NC + (q[2] * 8 + q[1]) * 8 + q[0]];
+      } else if (src >= 0) {
+        q[axis] += side ? -N : N;
+        val = U[size_t(src) * BLK + v * NC + (q[2] * 8 + q[1]) * 8 + q[0]];
+      } else {
+        const int ll = side ? q[axis] - N : q[axis] + NG;
+        const int r = axis == 0 ? (k * 8 + j) * 2 + ll : axis == 1 ? (k * 2 + ll) * 8 + i : (ll * 8 + j) * 8 + i;
+        val = ghost[size_t(-2 - src) * SLAB + v * NG * FACE + r];
+      }
+    }
+    out[t] = val;
+  }
+}
+
+cudaError_t launch_ghosted(const double* U, const double* ghost, const int32_t* face_src, const int64_t* perm, int first,
+                           int count, double* G, cudaStream_t st) {
+  if (count <= 0) return cudaSuccess;
+  ghosted_kernel<<<count, 256, 0, st>>>(U, ghost, face_src, perm, first, G);
+  return cudaGetLastError();
+}
+
+}  // namespace sfh
