@@ -1,0 +1,292 @@
+#!/usr/bin/env python
+"""bench.py — hydro cell-updates/s of the B200 AMR hydro step (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C2] [--impl ours|reference]
+
+A "step" is one coarse step of the whole hot path (CFL reduction, ghost fill incl. prolongation,
+predictor, corrector, flux registers, restriction, reflux; all sub-steps of the finer levels in
+adaptive mode) over one synthetic problem; one cell-update = one predictor+corrector update of one
+cell of one block of any level (the paper's unit).  Default workload: C2 =
+BASELINE.json configs[1], uniform periodic 256^3 in 8^3 blocks (the paper's Table 5 shape).
+Prints ONE JSON line (rank 0).  N > 1 runs N independent replicas, one per GPU (DESIGN.md:
+"replicas only"; the path has no multi-GPU exchange in scope).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "hydro cell-updates/sec (fp64, 1xB200)"
+UNIT = "cell-updates/s"
+CORRECTOR_BYTES_PER_CELL = 120.0   # read U^n, U^{n+1/2}, write U^{n+1}, 5 fp64 each
+PREDICTOR_BYTES_PER_CELL = 80.0    # read U^n, write U^{n+1/2}
+# dram__bytes_read.sum + dram__bytes_write.sum of one corrector launch on C2, from the ncu --set full
+# capture summarised in profiles/ (None until captured)
+CORRECTOR_TRAFFIC_BYTES_C2 = None
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="C2", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--scale", type=int, default=1, help="shrink the base grid (debugging only; invalid as a bench value)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json, copy bandwidth)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.lines = []
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return None
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        rows = [l.split(", ") for t, l in self.lines if t0 - 0.05 <= t <= t1 + 0.15]
+        if not rows:
+            rows = [l.split(", ") for _, l in self.lines]
+        if not rows:
+            return None
+        try:
+            sm = sorted(float(r[0]) for r in rows)
+            names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+            reasons = [n for i, n in enumerate(names) if any(r[3 + i].strip().lower() == "active" for r in rows)]
+            return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(rows[0][1]), "reasons": reasons,
+                    "samples": len(rows), "power_w_max": max(float(r[2]) for r in rows)}
+        except Exception:
+            return None
+
+
+def cell_updates(census, nupd):
+    return float(sum(512 * c * int(n) for c, n in zip(census, nupd)))
+
+
+def oracle_sample(config, scale_hint):
+    """The oracle on a bounded sample of the same workload: the same recipe on a smaller base grid."""
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from helpers import oracle_for
+    from sfh_inputs import make_config
+    sample_scale = {"C1": 1, "C2": 1, "C3": 2, "C4": 2, "C5": 4}[config] * max(1, scale_hint)
+    p = make_config(config, sample_scale)
+    o = oracle_for(p)
+    o.restrict_all(0)
+    n = p.nb0[0] * 8
+    what = "%s recipe at base %d^3 (1/%d of the base cells), blocks/level %s" % (config, n, sample_scale ** 3, p.census())
+    return p, o, what
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle as it stands, on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    p, o, what = oracle_sample(args.config, args.scale)
+    cores = len(os.sched_getaffinity(0))
+    for _ in range(args.warmup):
+        o.advance(1, p.mode)
+    o.nupd[:] = 0
+    t0 = time.perf_counter()
+    o.advance(args.steps, p.mode)
+    dt = time.perf_counter() - t0
+    cu = cell_updates(p.census(), o.nupd)
+    val = cu / dt
+    sample = what + ", %d coarse step(s) per run" % args.steps
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": p.notes.get("workload", p.name), "config": args.config, "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    import paper_2604_21438_b200 as sfh
+    from sfh_inputs import make_config
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (libsfh has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = "cuda:%d" % local
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+
+    p = make_config(args.config, args.scale)
+    census = p.census()
+    g = sfh.Mesh.from_problem(p, device=dev)
+    U0 = torch.from_numpy(p.U).pin_memory()
+    Ud = U0.to(dev)
+
+    def reset():
+        g.set_state(Ud)
+        g.restrict_all(0)
+        g.nupd[:] = 0
+        torch.cuda.synchronize()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- warm-up
+    reset()
+    for _ in range(max(args.warmup, 0)):
+        g.advance(1, p.mode)
+    bad_warm = g.status()
+
+    # ---- timed region: K coarse steps, state resident in HBM
+    reset()
+    g.profile(True)
+    g.kernel_times()
+    l0 = g.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    t0 = time.time()
+    e0.record()
+    g.advance(args.steps, p.mode)
+    e1.record()
+    barrier()
+    t1 = time.time()
+    clocks = sampler.stop(t0, t1) if sampler else None
+    ms = e0.elapsed_time(e1)
+    launches = g.launch_count() - l0
+    kt = g.kernel_times()
+    g.profile(False)
+    nupd = g.nupd.copy()
+    cu = cell_updates(census, nupd)
+    bad = g.status()
+    if world > 1:
+        t = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * cu / (ms * 1e-3)
+
+    # ---- end to end through sfh_advance_host: pinned host buffers, H2D and D2H every step
+    reset()
+    hin = g.get_state().cpu().pin_memory()    # restriction-consistent initial hierarchy, caller layout
+    hout = torch.empty_like(hin).pin_memory()
+    g.advance_host(hin, hout, 1, p.mode)      # warm
+    g.nupd[:] = 0
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        g.advance_host(hin, hout, 1, p.mode)
+        hin, hout = hout, hin
+    e1.record()
+    barrier()
+    ms_e2e = e0.elapsed_time(e1)
+    cu_e2e = cell_updates(census, g.nupd)
+    if world > 1:
+        t = torch.tensor([ms_e2e], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_e2e = float(t.item())
+    state_bytes = int(U0.numel() * 8)
+
+    # ---- roofline of the dominant kernel (the corrector stage), CUDA events around each launch
+    peak, peak_src = peaks()
+    c_ms, c_n = kt["corrector"]
+    corr_bytes = CORRECTOR_BYTES_PER_CELL * cu            # every cell-update passes the corrector once
+    achieved = corr_bytes / (c_ms * 1e-3) / 1e9 if c_ms > 0 else 0.0
+    roofline = {"bound": "hbm", "kernel": "stage_kernel<1> (corrector)", "achieved": achieved, "peak": peak,
+                "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
+                "traffic": CORRECTOR_TRAFFIC_BYTES_C2 if (args.config == "C2" and args.scale == 1) else None,
+                "algorithmic_bytes_per_launch": corr_bytes / max(c_n, 1), "launches": c_n,
+                "avg_launch_ms": c_ms / max(c_n, 1),
+                "kernel_ms": {k: round(v[0], 4) for k, v in kt.items()},
+                "kernel_launches": {k: v[1] for k, v in kt.items()},
+                "step_hbm_GBps_at_200B_per_update": 200.0 * cu / (ms * 1e-3) / 1e9}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        # the oracle as it stands on this box's host cores, on a bounded sample: whole coarse steps of
+        # the same recipe (at a smaller base grid for the large configs) until ~12 s have passed
+        ps, o, what = oracle_sample(args.config, args.scale)
+        tt, nst = time.perf_counter(), 0
+        while nst < max(args.steps, 1) and (nst == 0 or time.perf_counter() - tt < 12.0):
+            o.advance(1, ps.mode)
+            nst += 1
+        tt = time.perf_counter() - tt
+        cpu = {"value": cell_updates(ps.census(), o.nupd) / tt, "unit": UNIT, "cores": len(os.sched_getaffinity(0)),
+               "kind": "oracle", "sample": what + ", %d coarse step(s), %.1f s" % (nst, tt)}
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": p.notes.get("workload", p.name), "config": args.config, "scale": args.scale,
+                   "blocks_per_level": census, "updates_per_level": [int(x) for x in nupd],
+                   "mode": "adaptive" if p.mode else "synchronous",
+                   "l2": "inputs larger than L2 (one state copy %.0f MB vs 126 MB L2)" % (state_bytes / 1e6),
+                   "parallelism": "replicas x%d" % world, "bad_cells": int(bad), "bad_cells_after_warmup": int(bad_warm)},
+        "clocks": clocks,
+        "e2e": {"value": world * cu_e2e / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": state_bytes,
+                "d2h_bytes_per_step": state_bytes, "ms_per_step": ms_e2e / args.steps},
+        "gpu_launches": int(launches),
+        "roofline": roofline,
+        "cpu_baseline": cpu,
+    }
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -159,15 +159,26 @@ int sfh_advance(sfh_mesh* m, int ncoarse_steps, int mode, double dt_fixed, doubl
                 int64_t* nupd_host, void* stream);
 
 /* End-to-end convenience: h_in (HOST, caller layout) -> device role 0, sfh_advance, role 0 -> h_out
- * (HOST).  Host buffers should be pinned for full PCIe speed.  Synchronous. */
+ * (HOST).  Host buffers should be pinned for full PCIe speed.  t_host, nupd_host as in sfh_advance.
+ * Synchronous. */
 int sfh_advance_host(sfh_mesh* m, const double* h_in, double* h_out, int ncoarse_steps, int mode,
-                     double dt_fixed, double* t_host, void* stream);
+                     double dt_fixed, double* t_host, int64_t* nupd_host, void* stream);
 
 /* Number of interior cells of role `which` with rho <= 0, P <= 0 or NaN (all blocks).  Synchronises. */
 int sfh_status(sfh_mesh* m, int which, int64_t* n_bad_cells, void* stream);
 
 /* Kernels launched by this library since the mesh was created (for bench.py's gpu_launches). */
 int64_t sfh_launch_count(const sfh_mesh* m);
+
+/* Per-kernel device timing for roofline reports.  While enabled, every launch of a hot-path kernel
+ * is bracketed by two CUDA events on the caller's stream.  Kernel classes: 0 predictor stage (a4),
+ * 1 corrector stage (a6+a7), 2 coarse-fine ghost prolongation (a3), 3 restriction (a8), 4 reflux
+ * (a9), 5 CFL reduction (a10).  sfh_kernel_times synchronises on the recorded events, ADDS the
+ * elapsed milliseconds and launch counts since the last call to ms[6] / count[6] (host arrays)
+ * and forgets them. */
+#define SFH_NUM_KERNEL_CLASSES 6
+int sfh_profile(sfh_mesh* m, int enable);
+int sfh_kernel_times(sfh_mesh* m, double* ms, int64_t* count);
 
 const char* sfh_last_error(void);
 

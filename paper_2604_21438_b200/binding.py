@@ -71,9 +71,11 @@ def load_library(path=None):
         "sfh_restrict": (i32, [vp, i32, i32, i32, vp]),
         "sfh_end_step": (i32, [vp, i32]),
         "sfh_advance": (i32, [vp, i32, i32, dbl, C.POINTER(dbl), vp, vp]),
-        "sfh_advance_host": (i32, [vp, vp, vp, i32, i32, dbl, C.POINTER(dbl), vp]),
+        "sfh_advance_host": (i32, [vp, vp, vp, i32, i32, dbl, C.POINTER(dbl), vp, vp]),
         "sfh_status": (i32, [vp, i32, C.POINTER(i64), vp]),
         "sfh_launch_count": (i64, [vp]),
+        "sfh_profile": (i32, [vp, i32]),
+        "sfh_kernel_times": (i32, [vp, vp, vp]),
         "sfh_last_error": (C.c_char_p, []),
     }
     for name, (res, args) in sig.items():
@@ -236,8 +238,21 @@ class Mesh:
         """h_in, h_out: host tensors/arrays in caller layout (pinned for full PCIe speed)."""
         pin = h_in.data_ptr() if hasattr(h_in, "data_ptr") else h_in.ctypes.data
         pout = h_out.data_ptr() if hasattr(h_out, "data_ptr") else h_out.ctypes.data
-        self._chk(self.L.sfh_advance_host(self.h, pin, pout, nsteps, mode, dt_fixed, C.byref(self.t), _stream()))
+        self._chk(self.L.sfh_advance_host(self.h, pin, pout, nsteps, mode, dt_fixed, C.byref(self.t),
+                                          self.nupd.ctypes.data, _stream()))
         return self.t.value
+
+    KERNEL_CLASSES = ("predictor", "corrector", "prolong", "restrict", "reflux", "max_speed")
+
+    def profile(self, enable=True):
+        self._chk(self.L.sfh_profile(self.h, int(enable)))
+
+    def kernel_times(self):
+        """{class: (total ms, launches)} since the last call (synchronises)."""
+        ms = np.zeros(6, dtype=np.float64)
+        cnt = np.zeros(6, dtype=np.int64)
+        self._chk(self.L.sfh_kernel_times(self.h, ms.ctypes.data, cnt.ctypes.data))
+        return {k: (float(ms[i]), int(cnt[i])) for i, k in enumerate(self.KERNEL_CLASSES)}
 
     def status(self, which=0):
         n = C.c_int64()

@@ -5,6 +5,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <vector>
 
 #include "sfh_kernels.cuh"
 
@@ -31,6 +32,11 @@ struct sfh_mesh {
   int role[MAX_LEVELS][3];              // role -> physical state buffer, per level
   TensorMaps tm[3];                     // per physical state buffer
   int64_t launches = 0;
+  // optional per-kernel-class timing (sfh_profile / sfh_kernel_times)
+  bool profiling = false;
+  struct Span { int cls; cudaEvent_t a, b; };
+  std::vector<Span> spans;
+  std::vector<cudaEvent_t> event_pool;
 };
 
 namespace {
@@ -97,6 +103,31 @@ int make_tensor_maps(void* base, int64_t nb, TensorMaps& out) {
 }
 
 inline cudaStream_t S(void* s) { return reinterpret_cast<cudaStream_t>(s); }
+
+// Brackets one kernel launch with two events when profiling is on.
+struct Timed {
+  sfh_mesh* m;
+  cudaStream_t st;
+  cudaEvent_t a = nullptr, b = nullptr;
+  int cls;
+  static cudaEvent_t take(sfh_mesh* m) {
+    cudaEvent_t e = nullptr;
+    if (!m->event_pool.empty()) { e = m->event_pool.back(); m->event_pool.pop_back(); }
+    else if (cudaEventCreate(&e) != cudaSuccess) e = nullptr;
+    return e;
+  }
+  Timed(sfh_mesh* m_, int cls_, cudaStream_t st_) : m(m_), st(st_), cls(cls_) {
+    if (!m->profiling) return;
+    a = take(m);
+    b = take(m);
+    if (a) cudaEventRecord(a, st);
+  }
+  ~Timed() {
+    if (!a || !b) return;
+    cudaEventRecord(b, st);
+    m->spans.push_back({cls, a, b});
+  }
+};
 inline double* role_buf(const sfh_mesh* m, int l, int r) { return m->state[m->role[l][r]]; }
 
 int check_bound(const sfh_mesh* m) {
@@ -125,7 +156,10 @@ int fill_level(sfh_mesh* m, int l, int which, int interp, double tau, cudaStream
   p.nbr27 = m->d_nbr27;
   p.first = int(hm.cf_first[l]); p.count = int(hm.cf_count[l]);
   p.interp = interp; p.tau = tau;
-  CU(launch_prolong(p, st), "prolong_kernel");
+  {
+    Timed tmr(m, 2, st);
+    CU(launch_prolong(p, st), "prolong_kernel");
+  }
   m->launches += 1;
   return SFH_OK;
 }
@@ -143,7 +177,10 @@ int stage_level(sfh_mesh* m, int l, int stage, Dt dt, cudaStream_t st) {
   p.dt_dev = dt.dev; p.dt = dt.host; p.h = hm.h[l]; p.gamma = hm.cfg.gamma;
   p.first = int(hm.lev_first[l]); p.count = int(hm.lev_count[l]);
   p.use_regs = stage == 1 && (hm.cf_count[l] > 0 || hm.reflux_count[l] > 0);
-  CU(launch_stage(stage, m->tm[m->role[l][src_role]], p, st), "stage_kernel");
+  {
+    Timed tmr(m, stage, st);
+    CU(launch_stage(stage, m->tm[m->role[l][src_role]], p, st), "stage_kernel");
+  }
   m->launches += 1;
   return SFH_OK;
 }
@@ -167,11 +204,17 @@ int hydro_level(sfh_mesh* m, int l, Dt dt, int interp, double tau, double dtau, 
 int flux_correct_level(sfh_mesh* m, int lc, Dt dt, cudaStream_t st) {
   const HostMesh& hm = m->hm;
   if (lc + 1 >= hm.nlev || hm.lev_count[lc + 1] == 0) return SFH_OK;
-  CU(launch_restrict(role_buf(m, lc + 1, 0), role_buf(m, lc, 2), m->d_restrict_list + hm.restrict_first[lc],
-                     m->d_child0, int(hm.restrict_count[lc]), st), "restrict_kernel");
+  {
+    Timed tmr(m, 3, st);
+    CU(launch_restrict(role_buf(m, lc + 1, 0), role_buf(m, lc, 2), m->d_restrict_list + hm.restrict_first[lc],
+                       m->d_child0, int(hm.restrict_count[lc]), st), "restrict_kernel");
+  }
   m->launches += hm.restrict_count[lc] > 0;
-  CU(launch_reflux(role_buf(m, lc, 2), m->R, m->FH, m->d_reflux_list + hm.reflux_first[lc], m->d_fslot, m->d_fh_src,
-                   int(hm.reflux_count[lc]), hm.h[lc], dt.host, dt.dev, st), "reflux_kernel");
+  {
+    Timed tmr(m, 4, st);
+    CU(launch_reflux(role_buf(m, lc, 2), m->R, m->FH, m->d_reflux_list + hm.reflux_first[lc], m->d_fslot,
+                     m->d_fh_src, int(hm.reflux_count[lc]), hm.h[lc], dt.host, dt.dev, st), "reflux_kernel");
+  }
   m->launches += hm.reflux_count[lc] > 0;
   return SFH_OK;
 }
@@ -180,6 +223,7 @@ void rotate(sfh_mesh* m, int l) { std::swap(m->role[l][0], m->role[l][2]); }
 
 int max_speed_level(sfh_mesh* m, int l, cudaStream_t st) {
   const HostMesh& hm = m->hm;
+  Timed tmr(m, 5, st);
   CU(launch_max_speed(role_buf(m, l, 0), int(hm.lev_first[l]), int(hm.lev_count[l]), hm.cfg.gamma, m->smax + l, st),
      "max_speed_kernel");
   m->launches += hm.lev_count[l] > 0;
@@ -293,6 +337,8 @@ int sfh_create_mesh(const sfh_config* cfg, int64_t nblocks, const int32_t* level
 
 int sfh_destroy_mesh(sfh_mesh* m) {
   if (!m) return SFH_OK;
+  for (auto& sp : m->spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
+  for (cudaEvent_t e : m->event_pool) cudaEventDestroy(e);
   if (m->dev_tables) cudaFree(m->dev_tables);
   delete m;
   return SFH_OK;
@@ -517,7 +563,7 @@ int sfh_advance(sfh_mesh* m, int ncoarse_steps, int mode, double dt_fixed, doubl
 }
 
 int sfh_advance_host(sfh_mesh* m, const double* h_in, double* h_out, int ncoarse_steps, int mode, double dt_fixed,
-                     double* t_host, void* stream) {
+                     double* t_host, int64_t* nupd_host, void* stream) {
   int rc = check_bound(m);
   if (rc) return rc;
   if (!h_in || !h_out) return fail(SFH_EINVAL, "null host buffer");
@@ -529,10 +575,31 @@ int sfh_advance_host(sfh_mesh* m, const double* h_in, double* h_out, int ncoarse
     if (m->role[l][1] != m->role[0][1]) return fail(SFH_ESTATE, "internal: role 1 buffers differ between levels");
   CU(cudaMemcpyAsync(stage, h_in, bytes, cudaMemcpyHostToDevice, st), "H2D");
   if ((rc = sfh_set_state(m, 0, stage, stream))) return rc;
-  if ((rc = sfh_advance(m, ncoarse_steps, mode, dt_fixed, t_host, nullptr, stream))) return rc;
+  if ((rc = sfh_advance(m, ncoarse_steps, mode, dt_fixed, t_host, nupd_host, stream))) return rc;
   if ((rc = sfh_get_state(m, 0, stage, stream))) return rc;
   CU(cudaMemcpyAsync(h_out, stage, bytes, cudaMemcpyDeviceToHost, st), "D2H");
   CU(cudaStreamSynchronize(st), "cudaStreamSynchronize");
+  return SFH_OK;
+}
+
+int sfh_profile(sfh_mesh* m, int enable) {
+  if (!m) return fail(SFH_EINVAL, "null mesh");
+  m->profiling = enable != 0;
+  return SFH_OK;
+}
+
+int sfh_kernel_times(sfh_mesh* m, double* ms, int64_t* count) {
+  if (!m || !ms || !count) return fail(SFH_EINVAL, "null argument");
+  for (auto& sp : m->spans) {
+    CU(cudaEventSynchronize(sp.b), "cudaEventSynchronize");
+    float t = 0.f;
+    CU(cudaEventElapsedTime(&t, sp.a, sp.b), "cudaEventElapsedTime");
+    ms[sp.cls] += double(t);
+    count[sp.cls] += 1;
+    m->event_pool.push_back(sp.a);
+    m->event_pool.push_back(sp.b);
+  }
+  m->spans.clear();
   return SFH_OK;
 }
 

@@ -1,0 +1,257 @@
+"""Parity of the CUDA path (through the C ABI of include/sfh.h) with the CPU oracle, element by
+element on the same seeded inputs.  Tolerances are BASELINE.json's north_star: fp64 cell values
+within 1e-12 (one step) / 1e-10 (ten steps) in the normalised max norm of DESIGN.md "Parity norm",
+CFL dt within 1e-14 relative; copies (same-level ghosts, permutation) bit-exact."""
+import numpy as np
+import pytest
+
+import paper_2604_21438_b200 as sfh
+from helpers import oracle_for, parity_errors, problem_from_tree, small_amr_tree, smooth_fields
+from sfh_inputs import make_config, uniform_tree, Tree
+from sfh_inputs.configs import sod
+
+pytestmark = pytest.mark.gpu
+
+TOL1, TOL10, TOLDT = 1e-12, 1e-10, 1e-14
+
+
+def gpu_for(p, U=None):
+    m = sfh.Mesh.from_problem(p)
+    m.set_state(p.U if U is None else U)
+    return m
+
+
+def both(p):
+    """Oracle and GPU meshes holding the same restriction-consistent initial hierarchy (each side
+    restricts with its own code; the result is compared bit for bit)."""
+    o = oracle_for(p)
+    o.restrict_all(0)
+    g = gpu_for(p)
+    g.restrict_all(0)
+    Ug = g.get_state().cpu().numpy()
+    assert np.array_equal(Ug, o.get_state()), "restriction of the initial data differs"
+    return o, g
+
+
+def compare(o, g, gamma, tol):
+    Uo = o.get_state()
+    Ug = g.get_state().cpu().numpy()
+    assert np.isfinite(Ug).all()
+    err = parity_errors(Ug, Uo, gamma)
+    assert (err <= tol).all(), err
+    return err
+
+
+PROBLEMS = {
+    "C1": lambda: make_config("C1"),
+    "C2/4": lambda: make_config("C2", 4),
+    "C3/8": lambda: make_config("C3", 8),
+    "C4/4": lambda: make_config("C4", 4),
+    "C5/8": lambda: make_config("C5", 8),
+    "amr-small": lambda: problem_from_tree(small_amr_tree(), mode=1),
+    "amr-outflow": lambda: problem_from_tree(small_amr_tree(periodic=(False, True, False), offset=(-1, 0, 1)), mode=1),
+    "ragged": lambda: problem_from_tree(uniform_tree((3, 1, 5)), gamma=1.4),
+    "one-block": lambda: problem_from_tree(uniform_tree((1, 1, 1))),
+}
+
+
+@pytest.mark.parametrize("name", list(PROBLEMS))
+def test_cfl_dt_parity(name):
+    p = PROBLEMS[name]()
+    o, g = both(p)
+    for l in [-1] + list(range(p.max_level + 1)):
+        if l >= 0 and p.census()[l] == 0:
+            continue
+        a, b = g.cfl_dt(l), o.cfl_dt(l)
+        assert abs(a - b) <= TOLDT * b, (l, a, b)
+
+
+@pytest.mark.parametrize("name", list(PROBLEMS))
+def test_one_sync_step_parity(name):
+    p = PROBLEMS[name]()
+    o, g = both(p)
+    dt = 0.8 * o.cfl_dt()
+    o.advance(1, 0, dt)
+    g.advance(1, 0, dt)
+    compare(o, g, p.gamma, TOL1)
+
+
+@pytest.mark.parametrize("name", list(PROBLEMS))
+def test_config_run_parity(name):
+    """The configured number of steps in the configured mode (sync for uniform grids, adaptive
+    level-by-level stepping for AMR), CFL steps computed by each side."""
+    p = PROBLEMS[name]()
+    o, g = both(p)
+    o.advance(1, p.mode)
+    g.advance(1, p.mode)
+    assert abs(g.t.value - o.t.value) <= TOLDT * o.t.value
+    compare(o, g, p.gamma, TOL1)
+    n = max(p.nsteps, 10) - 1
+    o.advance(n, p.mode)
+    g.advance(n, p.mode)
+    assert np.array_equal(o.nupd, g.nupd), (o.nupd, g.nupd)
+    assert abs(g.t.value - o.t.value) <= 1e-13 * o.t.value
+    assert o.status() == 0 and g.status() == 0
+    compare(o, g, p.gamma, TOL10)
+
+
+@pytest.mark.slow
+def test_c5_quarter_scale_adaptive_parity():
+    p = make_config("C5", 4)
+    o, g = both(p)
+    o.advance(p.nsteps, 1)
+    g.advance(p.nsteps, 1)
+    assert np.array_equal(o.nupd, g.nupd)
+    compare(o, g, p.gamma, TOL10)
+
+
+# ------------------------------------------------------------------ ghost fill (a2, a3, a5)
+def ghost_count():
+    """[12,12,12] int: number of indices of a cell outside the interior [2,10)."""
+    o = np.r_[1, 1, np.zeros(8, int), 1, 1]
+    return o[:, None, None] + o[None, :, None] + o[None, None, :]
+
+
+def face_mask():
+    return ghost_count() == 1
+
+
+@pytest.mark.parametrize("name", ["amr-small", "amr-outflow", "C1", "ragged", "one-block", "C4/4"])
+@pytest.mark.parametrize("interp", [0, 1])
+def test_ghost_fill_parity(name, interp):
+    p = PROBLEMS[name]()
+    if interp and p.max_level == 0:
+        pytest.skip("temporal interpolation needs a coarse level")
+    o, g = both(p)
+    rng = np.random.default_rng(7)
+    # three different time copies so that eq. (16) is exercised with distinct U^n, U^{n+1/2}, U^{n+1}
+    U0 = o.get_state()
+    for which, f in ((1, 1.03), (2, 1.08)):
+        Uw = U0 * (f + 0.01 * rng.random(U0.shape[:1])[:, None, None, None, None])
+        o.set_state(Uw, which)
+        g.set_state(Uw, which)
+    tau = 0.375
+    for which in (0, 1):
+        o.fill_ghosts(-1, which, interp, tau)
+        g.fill_ghosts(-1, which, interp, tau)
+        Go = o.U[which]
+        Gg = g.get_ghosted(which).cpu().numpy()
+        fm = face_mask()
+        assert np.isnan(Gg[:, :, ghost_count() >= 2]).all()      # edge/corner ghosts: no stage reads them
+        assert np.array_equal(Gg[:, :, 2:10, 2:10, 2:10], Go[:, :, 2:10, 2:10, 2:10])
+        a, b = Gg[:, :, fm], Go[:, :, fm]
+        assert np.isfinite(a).all()
+        scale = np.abs(b).max(axis=(0, 2))[None, :, None]
+        # prolongation (and eq. 16) is ~10-20 roundings; FMA contraction may move each by an ulp
+        assert (np.abs(a - b) <= 4e-15 * scale).all(), np.abs((a - b) / scale).max()
+        if p.max_level == 0:
+            assert np.array_equal(a, b)          # pure copies
+
+
+# ------------------------------------------------------------------ the five calls, driven step by step
+def test_stepwise_calls_match_oracle_adaptive():
+    """One adaptive coarse step of a 3-level mesh written out with the individual ABI calls
+    (fill_ghosts / hydro_step / cfl_dt / flux_correct / end_step) against the same sequence of
+    oracle calls."""
+    p = PROBLEMS["amr-small"]()
+    o, g = both(p)
+
+    def adv_o(l, dt, tau, dt_parent):
+        if l < p.max_level:
+            o.zero_registers(l)
+        o.fill_ghosts(l, 0, 1, tau)
+        o.predictor(l, dt)
+        o.fill_ghosts(l, 1, 1, 0.0 if l == 0 else tau + 0.5 * dt / dt_parent)
+        o.corrector(l, dt)
+        if l < p.max_level:
+            n = 0
+            while dt / 2 ** n > o.cfl_dt(l + 1):
+                n += 1
+            for s in range(2 ** n):
+                adv_o(l + 1, dt / 2 ** n, s / 2 ** n, dt)
+            o.restrict(l, 0, 2)
+            o.reflux(l, 2, dt)
+        o.copy_level(l, 2, 0)
+
+    def adv_g(l, dt, tau, dt_parent):
+        interp = int(l > 0)
+        g.fill_ghosts(l, 0, interp, tau)
+        g.hydro_step(l, dt, interp, tau, dt / dt_parent if l else 0.0)
+        if l < p.max_level:
+            n = 0
+            while dt / 2 ** n > g.cfl_dt(l + 1):
+                n += 1
+            for s in range(2 ** n):
+                adv_g(l + 1, dt / 2 ** n, s / 2 ** n, dt)
+            g.flux_correct(l, dt)
+        g.end_step(l)
+
+    dt0 = o.cfl_dt(0)
+    assert abs(g.cfl_dt(0) - dt0) <= TOLDT * dt0
+    for _ in range(2):
+        adv_o(0, dt0, 0.0, dt0)
+        adv_g(0, dt0, 0.0, dt0)
+    compare(o, g, p.gamma, TOL1 * 4)
+    # and the library's own driver gives the same as its calls one by one
+    g2 = gpu_for(p)
+    g2.restrict_all(0)
+    g2.advance(2, 1, dt0)
+    assert np.array_equal(g2.get_state().cpu().numpy(), g.get_state().cpu().numpy())
+
+
+# ------------------------------------------------------------------ properties on the CUDA path itself
+def test_gpu_uniform_equals_fully_refined_bitwise():
+    nb = 2
+    tu = uniform_tree((2 * nb,) * 3)
+    tr = uniform_tree((nb,) * 3, 1, fully_refined_to=1)
+    pu = problem_from_tree(tu)
+    pr = problem_from_tree(tr)
+    gu, gr = gpu_for(pu), gpu_for(pr)
+    gr.restrict_all(0)
+    dt = 0.5 * gu.cfl_dt()
+    gu.advance(3, 0, dt)
+    gr.advance(3, 0, dt)
+    Uu = gu.get_state().cpu().numpy()
+    Ur = gr.get_state().cpu().numpy()[pr.level == 1]
+    key = lambda ijk: (ijk[:, 0] * 64 + ijk[:, 1]) * 64 + ijk[:, 2]
+    assert np.array_equal(Uu[np.argsort(key(pu.ijk))], Ur[np.argsort(key(pr.ijk[pr.level == 1]))])
+
+
+def test_gpu_free_stream_and_conservation():
+    from helpers import leaf_totals
+    p = PROBLEMS["amr-small"]()
+    o, g = both(p)
+    leaf = o.is_leaf()
+    h0 = o.cell_width(0)
+    tot0 = leaf_totals(leaf, g.get_state().cpu().numpy(), p.level, h0)
+    g.advance(3, 1)
+    tot1 = leaf_totals(leaf, g.get_state().cpu().numpy(), p.level, h0)
+    scale = np.abs(tot0).max()
+    assert (np.abs(tot1 - tot0) <= 2e-14 * max(scale, 1.0)).all(), tot1 - tot0
+    # free stream
+    U = np.empty_like(p.U)
+    U[:] = np.array([1.3, 0.4, -0.2, 0.7, 2.9])[None, :, None, None, None]
+    g.set_state(U)
+    g.advance(2, 1)
+    assert np.abs(g.get_state().cpu().numpy() - U).max() < 1e-14
+
+
+def test_status_counts_bad_cells_and_e2e_host_path():
+    import torch
+    p = PROBLEMS["C2/4"]()
+    g = gpu_for(p)
+    assert g.status() == 0
+    U = p.U.copy()
+    U[3, 0, 1, 2, 3] = -1.0          # negative density
+    U[5, 4, 0, 0, 0] = 0.0           # negative pressure
+    g.set_state(U)
+    assert g.status() == 2
+    # end-to-end call with host buffers == device-resident call
+    g.set_state(p.U)
+    g.advance(2, 0)
+    ref = g.get_state().cpu()
+    hin = torch.from_numpy(p.U).pin_memory()
+    hout = torch.empty_like(hin).pin_memory()
+    g.advance_host(hin, hout, 2, 0)
+    assert torch.equal(hout, ref.reshape(hout.shape))
+    assert g.launch_count() > 0
