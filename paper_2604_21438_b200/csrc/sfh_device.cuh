@@ -45,6 +45,10 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
                "l"(src), "r"(bytes), "r"(bar)
                : "memory");
 }
+// asynchronous prefetch of a contiguous global range into L2 (bytes multiple of 16)
+__device__ __forceinline__ void prefetch_l2(const void* src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+}
 // 4-D tiled tensor copy global -> shared; coordinates innermost first
 __device__ __forceinline__ void tensor4_g2s(uint32_t dst, const CUtensorMap* tm, int c0, int c1, int c2, int c3,
                                             uint32_t bar) {
@@ -70,48 +74,78 @@ __device__ __forceinline__ double time_interp(double U0, double Uh, double U1, d
   return (U1 - U1st) * (tau * tau) + ((1.0 - tau) * U0 + tau * U1st);  // eq. (16)
 }
 
-// conserved -> primitive (rho, vx, vy, vz, P), eq. (8)
-__device__ __forceinline__ void cons_to_prim(const double u[5], double gm1, double w[5]) {
-  const double rho = u[0];
-  w[0] = rho;
-  w[1] = u[1] / rho;
-  w[2] = u[2] / rho;
-  w[3] = u[3] / rho;
-  const double ke = 0.5 * (u[1] * u[1] + u[2] * u[2] + u[3] * u[3]) / rho;
+// Arithmetic conventions of the CUDA path: the
+// formulas are the oracle's, rearranged so that every fp64 division becomes ONE correctly rounded
+// reciprocal (__drcp_rn, ~7 DFMA issue slots against ~12 for a division) shared by all quotients
+// with that denominator, and sqrt(g P / rho) becomes (g P) rsqrt(g P rho) (~12 slots against ~25).
+// Each rearrangement moves a result by a few ulp; nothing is approximated beyond rounding.
+
+// conserved -> primitive (rho, vx, vy, vz, P), eq. (8); returns 1/rho
+__device__ __forceinline__ double cons_to_prim(const double u[5], double gm1, double w[5]) {
+  const double ir = __drcp_rn(u[0]);
+  w[0] = u[0];
+  w[1] = u[1] * ir;
+  w[2] = u[2] * ir;
+  w[3] = u[3] * ir;
+  const double ke = (0.5 * (u[1] * u[1] + u[2] * u[2] + u[3] * u[3])) * ir;
   w[4] = gm1 * (u[4] - ke);
+  return ir;
+}
+
+// primitive -> conserved (used where a stored half-step state W^{n+1/2} feeds eq. (16))
+__device__ __forceinline__ void prim_to_cons(const double w[5], double igm1, double u[5]) {
+  u[0] = w[0];
+  u[1] = w[0] * w[1];
+  u[2] = w[0] * w[2];
+  u[3] = w[0] * w[3];
+  u[4] = w[4] * igm1 + 0.5 * w[0] * (w[1] * w[1] + w[2] * w[2] + w[3] * w[3]);
+}
+
+// c_s = sqrt(gamma P / rho) as (gamma P) rsqrt(gamma P rho)
+__device__ __forceinline__ double sound_speed(double gamma, double P, double rho) {
+  const double gP = gamma * P;
+  return gP * rsqrt(gP * rho);
 }
 
 // HLLC flux (Toro et al. 1994 as cited; Davis wave speeds, reading R6) in the face
 // frame: u = normal velocity, v, w = the two tangential ones; Fn = (mass, normal momentum, tangential
-// momenta, energy).  cL, cR = sound speeds of the two states.
-__device__ __forceinline__ void hllc_flux(double rL, double uL, double vL, double wL, double PL, double cL, double rR,
-                                          double uR, double vR, double wR, double PR, double cR, double gm1,
-                                          double Fn[5]) {
+// momenta, energy).  cL, cR = sound speeds of the two states; igm1 = 1/(gamma-1).
+// Star state as in the oracle, U*_K = q_K (rho, rho S*, rho v, rho w, E + rho (S*-u)(S* + P/(rho (S_K-u))))_K
+// with q_K = (S_K-u_K)/(S_K-S*); here 1/(S_K-S*) is formed once and the pressure term is carried as
+// q rho (S*-u) P / (rho (S_K-u)) = P (S*-u)/(S_K-S*), which removes the third division.
+// HAVE_E: the total energies of the two states are known (cell-centred states: the conserved E).
+template <bool HAVE_E>
+__device__ __forceinline__ void hllc_flux(double rL, double uL, double vL, double wL, double PL, double cL, double EL,
+                                          double rR, double uR, double vR, double wR, double PR, double cR, double ER,
+                                          double igm1, double Fn[5]) {
   const double SL = fmin(uL - cL, uR - cR);
   const double SR = fmax(uL + cL, uR + cR);
-  const double EL = PL / gm1 + 0.5 * rL * (uL * uL + vL * vL + wL * wL);
-  const double ER = PR / gm1 + 0.5 * rR * (uR * uR + vR * vR + wR * wR);
-  if (SL >= 0.0) {
-    Fn[0] = rL * uL; Fn[1] = rL * uL * uL + PL; Fn[2] = rL * uL * vL; Fn[3] = rL * uL * wL; Fn[4] = uL * (EL + PL);
-  } else if (SR <= 0.0) {
-    Fn[0] = rR * uR; Fn[1] = rR * uR * uR + PR; Fn[2] = rR * uR * vR; Fn[3] = rR * uR * wR; Fn[4] = uR * (ER + PR);
-  } else {
+  double Ss = 0.0;
+  const bool star = SL < 0.0 && SR > 0.0;
+  if (star) {
     const double mL = rL * (SL - uL), mR = rR * (SR - uR);
-    const double Ss = (PR - PL + mL * uL - mR * uR) / (mL - mR);
-    const bool left = Ss >= 0.0;
-    const double r = left ? rL : rR, u = left ? uL : uR, v = left ? vL : vR, w = left ? wL : wR;
-    const double P = left ? PL : PR, E = left ? EL : ER, S = left ? SL : SR, mk = left ? mL : mR;
-    // U*_K = (S_K - u_K)/(S_K - S*) (rho, rho S*, rho v, rho w, E + rho (S* - u)(S* + P/(rho (S_K - u))))
-    const double q = (S - u) / (S - Ss);
-    const double ru = r * u;
-    Fn[0] = ru + S * (q * r - r);
-    Fn[1] = (ru * u + P) + S * (q * (r * Ss) - ru);
-    Fn[2] = ru * v + S * (q * (r * v) - r * v);
-    Fn[3] = ru * w + S * (q * (r * w) - r * w);
-    Fn[4] = u * (E + P) + S * (q * (E + r * (Ss - u) * (Ss + P / mk)) - E);
+    Ss = (PR - PL + mL * uL - mR * uR) * __drcp_rn(mL - mR);
+  }
+  const bool left = star ? (Ss >= 0.0) : (SL >= 0.0);
+  const double r = left ? rL : rR, u = left ? uL : uR, v = left ? vL : vR, w = left ? wL : wR;
+  const double P = left ? PL : PR, S = left ? SL : SR;
+  const double E = HAVE_E ? (left ? EL : ER) : P * igm1 + 0.5 * r * (u * u + v * v + w * w);
+  const double ru = r * u;
+  Fn[0] = ru;
+  Fn[1] = ru * u + P;
+  Fn[2] = ru * v;
+  Fn[3] = ru * w;
+  Fn[4] = u * (E + P);
+  if (star) {
+    const double inv = __drcp_rn(S - Ss);
+    const double q = (S - u) * inv;
+    const double rv = r * v, rw = r * w, d = Ss - u;
+    Fn[0] += S * (q * r - r);
+    Fn[1] += S * (q * (r * Ss) - ru);
+    Fn[2] += S * (q * rv - rv);
+    Fn[3] += S * (q * rw - rw);
+    Fn[4] += S * ((q * (E + (r * d) * Ss) + (P * d) * inv) - E);
   }
 }
-
-__device__ __forceinline__ double sound_speed(double gamma, double P, double rho) { return sqrt(gamma * P / rho); }
 
 }  // namespace sfh

@@ -60,21 +60,12 @@ struct WLayout {
   }
 };
 
-// index of cell (position c along D, pencil (a,b)) in a flux-difference array; x rows are XOR
-// swizzled so that the x walkers' stores spread over the banks
-template <int D>
-__device__ __forceinline__ int df_index(int c, int a, int b) {
-  if (D == 0) return (b * 8 + a) * 8 + (c ^ a);
-  if (D == 1) return b * 64 + c * 8 + a;
-  return c * 64 + b * 8 + a;
-}
-
 // ---- conversion of the staged conserved cells to primitives --------------------------------------
 template <int STAGE>
 __device__ __forceinline__ void convert_block(const double* __restrict__ L, double* __restrict__ W,
                                               const int* __restrict__ fsrc, double gamma, double gm1, int tid) {
   constexpr int H = STAGE == 0 ? 1 : 2;
-  constexpr int NVW = STAGE == 0 ? 6 : 5;
+  constexpr int NVW = STAGE == 0 ? 7 : 5;
   using WL = WLayout<H, NVW>;
   for (int idx = tid; idx < NC + 6 * NG * FACE; idx += STAGE_THREADS) {
     int src, svs, dst, dvs;
@@ -116,113 +107,143 @@ __device__ __forceinline__ void convert_block(const double* __restrict__ L, doub
     double u[5], w[5];
 #pragma unroll
     for (int v = 0; v < 5; ++v) u[v] = L[src + v * svs];
-    cons_to_prim(u, gm1, w);
+    const double ir = cons_to_prim(u, gm1, w);
 #pragma unroll
     for (int v = 0; v < 5; ++v) W[dst + v * dvs] = w[v];
-    if (STAGE == 0) W[dst + 5 * dvs] = sound_speed(gamma, w[4], w[0]);
+    if (STAGE == 0) {
+      const double c2 = (gamma * w[4]) * ir;         // c_s^2 = gamma P / rho
+      W[dst + 5 * dvs] = c2 * rsqrt(c2);
+      W[dst + 6 * dvs] = u[4];                       // total energy of the cell (eq. 8)
+    }
   }
 }
 
 // ---- pencil walks ----------------------------------------------------------------------------------
-// Face f = 0..8 of a pencil lies between cells f-1 and f.  Flux components are returned in the
-// global variable order; n, t1, t2 = normal and tangential momentum slots as in F[1+D], ...
-template <int D>
-__device__ __forceinline__ void store_regs(const StageParams& p, int blk, int side, int a, int b, const double F[5],
-                                           double dt) {
+// One thread per pencil; 64 pencils per axis; the three axes run side by side in different warps but
+// through the SAME rolled loop (runtime strides), so the instruction footprint is one flux body per
+// stage.  Face f = 0..8 of a pencil lies between cells f-1 and f; each flux is computed once and used
+// by both adjacent cells (the paper's mapping).
+template <int H, int NVW>
+struct Pencil {
+  using WL = WLayout<H, NVW>;
+  int lo0, lo_cs, lo_vs;   // cells c < 0:   offset lo0 + (c + H) * lo_cs, variable stride lo_vs
+  int mid0, mid_cs;        // cells 0..7:    offset mid0 + c * mid_cs,     variable stride XV
+  int hi0, hi_cs, hi_vs;   // cells c >= 8:  offset hi0 + (c - 8) * hi_cs
+  int vn, vt1, vt2;        // variable slots of the normal / tangential velocities (momenta)
+  int df0, df_cs, df_swz;  // flux-difference index of cell c: df0 + ((c ^ df_swz) * df_cs)
+  __device__ __forceinline__ Pencil(int D, int a, int b) {
+    vn = 1 + D; vt1 = 1 + (D + 1) % 3; vt2 = 1 + (D + 2) % 3;
+    if (D == 0) {
+      lo0 = (b * 8 + a) * WL::RS; lo_cs = 1; lo_vs = WL::XV;
+      mid0 = lo0 + H; mid_cs = 1;
+      hi0 = mid0 + N; hi_cs = 1; hi_vs = WL::XV;
+      df0 = (b * 8 + a) * 8; df_cs = 1; df_swz = a;      // x rows are XOR swizzled (bank spread)
+    } else if (D == 1) {
+      lo0 = WL::Y0 + b * H * 8 + a; lo_cs = 8; lo_vs = WL::YV;
+      mid0 = b * 8 * WL::RS + a + H; mid_cs = WL::RS;
+      hi0 = lo0 + NVW * WL::YV; hi_cs = 8; hi_vs = WL::YV;
+      df0 = D * BLK + b * 64 + a; df_cs = 8; df_swz = 0;
+    } else {
+      lo0 = WL::Z0 + b * 8 + a; lo_cs = 64; lo_vs = WL::ZV;
+      mid0 = b * WL::RS + a + H; mid_cs = 8 * WL::RS;
+      hi0 = lo0 + NVW * WL::ZV; hi_cs = 64; hi_vs = WL::ZV;
+      df0 = D * BLK + b * 8 + a; df_cs = 64; df_swz = 0;
+    }
+  }
+  // loads cell c >= 0 in the face frame (rho, normal v, tangential v's, P[, c_s])
+  __device__ __forceinline__ void load(const double* __restrict__ W, int c, double w[NVW]) const {
+    const bool hi = c >= N;
+    const int o = hi ? hi0 + (c - N) * hi_cs : mid0 + c * mid_cs;
+    const int s = hi ? hi_vs : WL::XV;
+    w[0] = W[o]; w[1] = W[o + vn * s]; w[2] = W[o + vt1 * s]; w[3] = W[o + vt2 * s]; w[4] = W[o + 4 * s];
+    if (NVW == 7) { w[5] = W[o + 5 * s]; w[NVW - 1] = W[o + 6 * s]; }
+  }
+  __device__ __forceinline__ void load_lo(const double* __restrict__ W, int c, double w[NVW]) const {
+    const int o = lo0 + (c + H) * lo_cs, s = lo_vs;
+    w[0] = W[o]; w[1] = W[o + vn * s]; w[2] = W[o + vt1 * s]; w[3] = W[o + vt2 * s]; w[4] = W[o + 4 * s];
+    if (NVW == 7) { w[5] = W[o + 5 * s]; w[NVW - 1] = W[o + 6 * s]; }
+  }
+  // dF of cell c = F(face c+1) - F(face c), stored in the global variable order
+  __device__ __forceinline__ void store_df(double* __restrict__ dF, int c, const double Fa[5], const double Fb[5]) const {
+    const int ci = df0 + ((c ^ df_swz) * df_cs);
+    dF[ci] = Fa[0] - Fb[0];
+    dF[ci + vn * NC] = Fa[1] - Fb[1];
+    dF[ci + vt1 * NC] = Fa[2] - Fb[2];
+    dF[ci + vt2 * NC] = Fa[3] - Fb[3];
+    dF[ci + 4 * NC] = Fa[4] - Fb[4];
+  }
+};
+
+// flux registers at coarse-fine faces (a7; reading R14); Fn in the face frame
+__device__ __forceinline__ void store_regs(const StageParams& p, int blk, int D, int side, int t, int vn, int vt1,
+                                           int vt2, const double Fn[5], double dt) {
   const int f = 2 * D + side;
   const int src = p.face_src[blk * 6 + f];
   const int fs = p.fslot[blk * 6 + f];
-  const int t = b * 8 + a;
-  if (src <= -2) {   // fine side of a coarse-fine face: accumulate dt * F (reading R14)
+  if (src <= -2) {   // fine side of a coarse-fine face: accumulate dt * F
     double* r = p.R + size_t(-2 - src) * REG + t;
-#pragma unroll
-    for (int v = 0; v < 5; ++v) r[v * FACE] += dt * F[v];
+    r[0] += dt * Fn[0]; r[vn * FACE] += dt * Fn[1]; r[vt1 * FACE] += dt * Fn[2]; r[vt2 * FACE] += dt * Fn[3];
+    r[4 * FACE] += dt * Fn[4];
   }
   if (fs >= 0) {     // coarse leaf next to a covered block: keep its own flux
     double* r = p.FH + size_t(fs) * REG + t;
-#pragma unroll
-    for (int v = 0; v < 5; ++v) r[v * FACE] = F[v];
+    r[0] = Fn[0]; r[vn * FACE] = Fn[1]; r[vt1 * FACE] = Fn[2]; r[vt2 * FACE] = Fn[3]; r[4 * FACE] = Fn[4];
   }
 }
 
-template <int D>
-__device__ __forceinline__ void walk_predictor(const double* __restrict__ W, double* __restrict__ dF, int a, int b,
-                                               double gm1) {
-  using WL = WLayout<1, 6>;
-  constexpr int n = 1 + D, t1 = 1 + (D + 1) % 3, t2 = 1 + (D + 2) % 3;
-  double wl[6], Fp[5];
-  {
-    const int o = WL::template off<D>(-1, a, b), s = WL::template vs<D>(-1);
-#pragma unroll
-    for (int v = 0; v < 6; ++v) wl[v] = W[o + v * s];
-  }
-#pragma unroll
+__device__ __forceinline__ void walk_predictor(const double* __restrict__ W, double* __restrict__ dF, int D, int a, int b,
+                                               double igm1) {
+  const Pencil<1, 7> pc(D, a, b);
+  double wl[7], Fp[5];
+  pc.load_lo(W, -1, wl);
+#pragma unroll 1
   for (int f = 0; f <= N; ++f) {
-    double wr[6], Fn[5], F[5];
-    const int o = WL::template off<D>(f, a, b), s = WL::template vs<D>(f);
+    double wr[7], Fn[5];
+    pc.load(W, f, wr);
+    hllc_flux<true>(wl[0], wl[1], wl[2], wl[3], wl[4], wl[5], wl[6], wr[0], wr[1], wr[2], wr[3], wr[4], wr[5], wr[6],
+                    igm1, Fn);
+    if (f > 0) pc.store_df(dF, f - 1, Fn, Fp);
 #pragma unroll
-    for (int v = 0; v < 6; ++v) wr[v] = W[o + v * s];
-    hllc_flux(wl[0], wl[n], wl[t1], wl[t2], wl[4], wl[5], wr[0], wr[n], wr[t1], wr[t2], wr[4], wr[5], gm1, Fn);
-    F[0] = Fn[0]; F[n] = Fn[1]; F[t1] = Fn[2]; F[t2] = Fn[3]; F[4] = Fn[4];
-    if (f > 0) {
-      const int ci = df_index<D>(f - 1, a, b);
+    for (int v = 0; v < 5; ++v) Fp[v] = Fn[v];
 #pragma unroll
-      for (int v = 0; v < 5; ++v) dF[D * BLK + v * NC + ci] = F[v] - Fp[v];
-    }
-#pragma unroll
-    for (int v = 0; v < 5; ++v) Fp[v] = F[v];
-#pragma unroll
-    for (int v = 0; v < 6; ++v) wl[v] = wr[v];
+    for (int v = 0; v < 7; ++v) wl[v] = wr[v];
   }
 }
 
-template <int D>
-__device__ __forceinline__ void walk_corrector(const double* __restrict__ W, double* __restrict__ dF, int a, int b,
-                                               double gamma, double gm1, const StageParams& p, int blk, double dt) {
-  using WL = WLayout<2, 5>;
-  constexpr int n = 1 + D, t1 = 1 + (D + 1) % 3, t2 = 1 + (D + 2) % 3;
-  // cells -2, -1: difference and the left face state of face 0 need the slope of cell -1
+__device__ __forceinline__ void walk_corrector(const double* __restrict__ W, double* __restrict__ dF, int D, int a, int b,
+                                               double gamma, double igm1, const StageParams& p, int blk, double dt) {
+  const Pencil<2, 5> pc(D, a, b);
+  // cells -2, -1: the left face state of face 0 needs the slope of cell -1
   double wm[5], wc[5], dm[5], WLs[5], Fp[5];
-  {
-    const int o0 = WL::template off<D>(-2, a, b), s0 = WL::template vs<D>(-2);
-    const int o1 = WL::template off<D>(-1, a, b), s1 = WL::template vs<D>(-1);
+  pc.load_lo(W, -2, wm);
+  pc.load_lo(W, -1, wc);
 #pragma unroll
-    for (int v = 0; v < 5; ++v) {
-      wm[v] = W[o0 + v * s0];
-      wc[v] = W[o1 + v * s1];
-      dm[v] = wc[v] - wm[v];
-    }
-  }
+  for (int v = 0; v < 5; ++v) { dm[v] = wc[v] - wm[v]; WLs[v] = 0.0; Fp[v] = 0.0; }
   // invariant at the top of iteration c (c = 0..9): wc = W_{c-1}, dm = W_{c-1} - W_{c-2};
   // for c >= 1, WLs = left state of face c-1 (= W_{c-2} + slope_{c-2}/2)
-#pragma unroll
+#pragma unroll 1
   for (int c = 0; c <= N + 1; ++c) {
     double wn[5], dn[5], sl[5];
-    const int o = WL::template off<D>(c, a, b), s = WL::template vs<D>(c);
+    pc.load(W, c, wn);
 #pragma unroll
     for (int v = 0; v < 5; ++v) {
-      wn[v] = W[o + v * s];
       dn[v] = wn[v] - wc[v];
       sl[v] = minmod(dn[v], dm[v]);      // slope of cell c-1 (reading R12), primitives (R11)
     }
     if (c >= 1) {
       // face f = c-1 between cells c-2 and c-1: right state from cell c-1
-      double WRs[5], Fn[5], F[5];
+      double WRs[5], Fn[5];
 #pragma unroll
       for (int v = 0; v < 5; ++v) WRs[v] = wc[v] - 0.5 * sl[v];
       const double cL = sound_speed(gamma, WLs[4], WLs[0]);
       const double cR = sound_speed(gamma, WRs[4], WRs[0]);
-      hllc_flux(WLs[0], WLs[n], WLs[t1], WLs[t2], WLs[4], cL, WRs[0], WRs[n], WRs[t1], WRs[t2], WRs[4], cR, gm1, Fn);
-      F[0] = Fn[0]; F[n] = Fn[1]; F[t1] = Fn[2]; F[t2] = Fn[3]; F[4] = Fn[4];
+      hllc_flux<false>(WLs[0], WLs[1], WLs[2], WLs[3], WLs[4], cL, 0.0, WRs[0], WRs[1], WRs[2], WRs[3], WRs[4], cR, 0.0,
+                       igm1, Fn);
       const int f = c - 1;
-      if (f > 0) {
-        const int ci = df_index<D>(f - 1, a, b);
+      if (f > 0) pc.store_df(dF, f - 1, Fn, Fp);
+      if (p.use_regs && (f == 0 || f == N)) store_regs(p, blk, D, f == N, b * 8 + a, pc.vn, pc.vt1, pc.vt2, Fn, dt);
 #pragma unroll
-        for (int v = 0; v < 5; ++v) dF[D * BLK + v * NC + ci] = F[v] - Fp[v];
-      }
-      if (p.use_regs && (f == 0 || f == N)) store_regs<D>(p, blk, f == N, a, b, F, dt);
-#pragma unroll
-      for (int v = 0; v < 5; ++v) Fp[v] = F[v];
+      for (int v = 0; v < 5; ++v) Fp[v] = Fn[v];
     }
 #pragma unroll
     for (int v = 0; v < 5; ++v) {
@@ -270,8 +291,10 @@ stage_kernel(const __grid_constant__ TensorMaps tm, const StageParams p) {
         bulk_g2s(dst, p.ghost + size_t(-2 - s) * SLAB, SLAB * 8, bar_a);
       }
     }
+    // U^n of this block is read again in the update at the end: pull it towards L2 now
+    if (STAGE == 1) prefetch_l2(p.Un + size_t(blk) * BLK, BLK * 8);
   }
-  const double gamma = p.gamma, gm1 = p.gamma - 1.0;
+  const double gamma = p.gamma, gm1 = p.gamma - 1.0, igm1 = __drcp_rn(gm1);
   const double dt = p.dt_dev ? *p.dt_dev : p.dt;
   mbar_wait(bar_a, 0);
 
@@ -280,15 +303,8 @@ stage_kernel(const __grid_constant__ TensorMaps tm, const StageParams p) {
 
   {
     const int pen = tid & 63, a = pen & 7, b = pen >> 3, D = tid >> 6;
-    if (STAGE == 0) {
-      if (D == 0) walk_predictor<0>(W, L, a, b, gm1);
-      else if (D == 1) walk_predictor<1>(W, L, a, b, gm1);
-      else walk_predictor<2>(W, L, a, b, gm1);
-    } else {
-      if (D == 0) walk_corrector<0>(W, L, a, b, gamma, gm1, p, blk, dt);
-      else if (D == 1) walk_corrector<1>(W, L, a, b, gamma, gm1, p, blk, dt);
-      else walk_corrector<2>(W, L, a, b, gamma, gm1, p, blk, dt);
-    }
+    if (STAGE == 0) walk_predictor(W, L, D, a, b, igm1);
+    else walk_corrector(W, L, D, a, b, gamma, igm1, p, blk, dt);
   }
   __syncthreads();
 
@@ -296,15 +312,26 @@ stage_kernel(const __grid_constant__ TensorMaps tm, const StageParams p) {
   const double lam = (STAGE == 0 ? 0.5 * dt : dt) / p.h;
   const double* __restrict__ Un = p.Un + size_t(blk) * BLK;
   double* __restrict__ Uo = p.Udst + size_t(blk) * BLK;
-  for (int idx = tid; idx < BLK; idx += STAGE_THREADS) {
-    const int cell = idx & (NC - 1), v = idx >> 9, row = cell >> 3, i = cell & 7;
-    const double dfx = L[v * NC + row * 8 + (i ^ (row & 7))];
-    const double sum = (dfx + L[BLK + idx]) + L[2 * BLK + idx];
-    Uo[idx] = Un[idx] - lam * sum;
+  constexpr int ROUNDS = (BLK + STAGE_THREADS - 1) / STAGE_THREADS;
+  double un[ROUNDS];
+#pragma unroll
+  for (int r = 0; r < ROUNDS; ++r) {          // all loads in flight before the first use
+    const int idx = tid + r * STAGE_THREADS;
+    un[r] = idx < BLK ? Un[idx] : 0.0;
+  }
+#pragma unroll
+  for (int r = 0; r < ROUNDS; ++r) {
+    const int idx = tid + r * STAGE_THREADS;
+    if (idx < BLK) {
+      const int cell = idx & (NC - 1), v = idx >> 9, row = cell >> 3, i = cell & 7;
+      const double dfx = L[v * NC + row * 8 + (i ^ (row & 7))];
+      const double sum = (dfx + L[BLK + idx]) + L[2 * BLK + idx];
+      Uo[idx] = un[r] - lam * sum;
+    }
   }
 }
 
-static_assert(WLayout<2, 5>::TOTAL <= W_DOUBLES && WLayout<1, 6>::TOTAL <= W_DOUBLES, "primitive array too small");
+static_assert(WLayout<2, 5>::TOTAL <= W_DOUBLES && WLayout<1, 7>::TOTAL <= W_DOUBLES, "primitive array too small");
 static_assert(LAND_DOUBLES <= DF_DOUBLES, "landing area must fit in the flux-difference area");
 static_assert((W_DOUBLES * 8) % 128 == 0 && (SLAB * 8) % 128 == 0 && (BLK * 8) % 128 == 0, "TMA destinations: 128 B");
 
