@@ -74,20 +74,44 @@ __device__ __forceinline__ double time_interp(double U0, double Uh, double U1, d
   return (U1 - U1st) * (tau * tau) + ((1.0 - tau) * U0 + tau * U1st);  // eq. (16)
 }
 
-// Arithmetic conventions of the CUDA path: the
-// formulas are the oracle's, rearranged so that every fp64 division becomes ONE correctly rounded
-// reciprocal (__drcp_rn, ~7 DFMA issue slots against ~12 for a division) shared by all quotients
-// with that denominator, and sqrt(g P / rho) becomes (g P) rsqrt(g P rho) (~12 slots against ~25).
+// Arithmetic conventions of the stage kernels.
+// The stage kernels are bound by the fp64 pipe and by instruction issue, so every formula of the
+// oracle is evaluated in the form that needs the fewest fp64 instructions and no branches:
+//  * 1/x and 1/sqrt(x) start from the hardware seed (MUFU.RCP64H / MUFU.RSQ64H, which read only the
+//    upper 32 bits of x: relative error < 2^-19) followed by ONE third-order step (error ~ e^3 < 2^-57,
+//    i.e. the result is within 1 ulp); no range checks: the arguments are ratios of positive, normal
+//    densities, pressures and wave-speed differences (a non-positive rho or P is reported by sfh_status
+//    and has no defined result on either side);
+//  * min/max/minmod are compare+select (no NaN fix-ups);
+//  * the HLLC star flux is written as F_K + S_K (U*_K - U_K) with U*_K - U_K expanded analytically.
 // Each rearrangement moves a result by a few ulp; nothing is approximated beyond rounding.
+
+__device__ __forceinline__ double rcp_fast(double x) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double e = fma(-x, y, 1.0);
+  const double t = fma(e, e, e);
+  return fma(y, t, y);                       // y (1 + e + e^2)
+}
+__device__ __forceinline__ double rsqrt_fast(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double e = fma(-x, y * y, 1.0);      // 1 - x y^2
+  const double p = fma(e, 0.375, 0.5);
+  return fma(p, y * e, y);                   // y (1 + e/2 + 3 e^2/8)
+}
+__device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }
+__device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
 
 // conserved -> primitive (rho, vx, vy, vz, P), eq. (8); returns 1/rho
 __device__ __forceinline__ double cons_to_prim(const double u[5], double gm1, double w[5]) {
-  const double ir = __drcp_rn(u[0]);
+  const double ir = rcp_fast(u[0]);
   w[0] = u[0];
   w[1] = u[1] * ir;
   w[2] = u[2] * ir;
   w[3] = u[3] * ir;
-  const double ke = (0.5 * (u[1] * u[1] + u[2] * u[2] + u[3] * u[3])) * ir;
+  const double m2 = fma(u[3], u[3], fma(u[2], u[2], u[1] * u[1]));
+  const double ke = (0.5 * ir) * m2;
   w[4] = gm1 * (u[4] - ke);
   return ir;
 }
@@ -104,48 +128,42 @@ __device__ __forceinline__ void prim_to_cons(const double w[5], double igm1, dou
 // c_s = sqrt(gamma P / rho) as (gamma P) rsqrt(gamma P rho)
 __device__ __forceinline__ double sound_speed(double gamma, double P, double rho) {
   const double gP = gamma * P;
-  return gP * rsqrt(gP * rho);
+  return gP * rsqrt_fast(gP * rho);
 }
 
 // HLLC flux (Toro et al. 1994 as cited; Davis wave speeds, reading R6) in the face
 // frame: u = normal velocity, v, w = the two tangential ones; Fn = (mass, normal momentum, tangential
 // momenta, energy).  cL, cR = sound speeds of the two states; igm1 = 1/(gamma-1).
-// Star state as in the oracle, U*_K = q_K (rho, rho S*, rho v, rho w, E + rho (S*-u)(S* + P/(rho (S_K-u))))_K
-// with q_K = (S_K-u_K)/(S_K-S*); here 1/(S_K-S*) is formed once and the pressure term is carried as
-// q rho (S*-u) P / (rho (S_K-u)) = P (S*-u)/(S_K-S*), which removes the third division.
+// Branch-free.  With K the upwind side (L if S_L >= 0, or if S_L < 0 < S_R and S* >= 0; else R),
+//   F = F_K + s (U*_K - U_K),  s = S_K inside the star region (S_L < 0 < S_R), else 0,
+// and with d = S* - u_K, g = d/(S_K - S*), A = rho_K g the oracle's star state
+//   U*_K = q (rho, rho S*, rho v, rho w, E + rho d (S* + P/(rho (S_K-u))))_K,  q = (S_K-u_K)/(S_K-S*) = 1 + g
+// gives  U*_K - U_K = (A, rho d + A S*, A v, A w, g (E + P + rho d S*) + rho d S*).
+// The denominator m_L - m_R of S* is strictly negative for positive rho (m_L < 0 < m_R), whatever
+// the wave pattern, so S* is always finite; S_K - S* is replaced by 1 outside the star region.
 // HAVE_E: the total energies of the two states are known (cell-centred states: the conserved E).
 template <bool HAVE_E>
 __device__ __forceinline__ void hllc_flux(double rL, double uL, double vL, double wL, double PL, double cL, double EL,
                                           double rR, double uR, double vR, double wR, double PR, double cR, double ER,
                                           double igm1, double Fn[5]) {
-  const double SL = fmin(uL - cL, uR - cR);
-  const double SR = fmax(uL + cL, uR + cR);
-  double Ss = 0.0;
+  const double SL = dmin(uL - cL, uR - cR);
+  const double SR = dmax(uL + cL, uR + cR);
+  const double mL = rL * (SL - uL), mR = rR * (SR - uR);
+  const double Ss = (((PR - PL) + mL * uL) - mR * uR) * rcp_fast(mL - mR);
   const bool star = SL < 0.0 && SR > 0.0;
-  if (star) {
-    const double mL = rL * (SL - uL), mR = rR * (SR - uR);
-    Ss = (PR - PL + mL * uL - mR * uR) * __drcp_rn(mL - mR);
-  }
-  const bool left = star ? (Ss >= 0.0) : (SL >= 0.0);
+  const bool left = !(SL < 0.0) || (SR > 0.0 && Ss >= 0.0);
   const double r = left ? rL : rR, u = left ? uL : uR, v = left ? vL : vR, w = left ? wL : wR;
   const double P = left ? PL : PR, S = left ? SL : SR;
-  const double E = HAVE_E ? (left ? EL : ER) : P * igm1 + 0.5 * r * (u * u + v * v + w * w);
-  const double ru = r * u;
-  Fn[0] = ru;
-  Fn[1] = ru * u + P;
-  Fn[2] = ru * v;
-  Fn[3] = ru * w;
-  Fn[4] = u * (E + P);
-  if (star) {
-    const double inv = __drcp_rn(S - Ss);
-    const double q = (S - u) * inv;
-    const double rv = r * v, rw = r * w, d = Ss - u;
-    Fn[0] += S * (q * r - r);
-    Fn[1] += S * (q * (r * Ss) - ru);
-    Fn[2] += S * (q * rv - rv);
-    Fn[3] += S * (q * rw - rw);
-    Fn[4] += S * ((q * (E + (r * d) * Ss) + (P * d) * inv) - E);
-  }
+  const double E = HAVE_E ? (left ? EL : ER) : fma(P, igm1, (0.5 * r) * fma(w, w, fma(v, v, u * u)));
+  const double ru = r * u, EP = E + P;
+  const double inv = rcp_fast(star ? S - Ss : 1.0);
+  const double s = star ? S : 0.0;
+  const double d = Ss - u, g = d * inv, rd = r * d, A = rd * inv, rdS = rd * Ss;
+  Fn[0] = fma(s, A, ru);
+  Fn[1] = fma(s, fma(A, Ss, rd), fma(ru, u, P));
+  Fn[2] = fma(s, A * v, ru * v);
+  Fn[3] = fma(s, A * w, ru * w);
+  Fn[4] = fma(s, fma(g, EP + rdS, rdS), u * EP);
 }
 
 }  // namespace sfh

@@ -24,40 +24,22 @@ constexpr int LAND_INT = 0;                 // landing area (doubles): interior 
 constexpr int LAND_HALO = BLK;              // then 6 slabs of SLAB doubles, face f = 2*axis + side
 constexpr int LAND_DOUBLES = BLK + 6 * SLAB;  // 6400
 constexpr int DF_DOUBLES = 3 * BLK;           // 7680, aliases the landing area
-constexpr int W_DOUBLES = 6720;               // max over stages of the primitive array
+constexpr int W_DOUBLES = 6720;               // the primitive array (both stages)
 constexpr int STAGE_SMEM = (W_DOUBLES + DF_DOUBLES) * 8 + 16 + 32;   // 115248 B (+1 KB reserved) -> 2 CTAs per SM
 
-// Primitive-array layout for a stage with H halo layers and NVW stored variables.
+// Primitive-array layout for a stage with H halo layers and NVW stored variables: W[var][pos], every
+// variable with the same stride VS, so that a cell's variables sit at compile-time offsets from the
+// cell's position.  Positions: 64 x rows of 8+2H cells (+1 pad: odd stride, conflict-free x pencils),
+// then the two y slabs [side][k][h][i], then the two z slabs [side][h][j][i].
 template <int H, int NVW>
 struct WLayout {
-  static constexpr int RS = N + 2 * H + 1;          // x-row stride (odd: conflict-free x pencils)
-  static constexpr int XV = 64 * RS;                // variable stride of the x-row array
-  static constexpr int X0 = 0;
-  static constexpr int YV = N * H * N;              // variable stride of a y slab [k][h][i]
-  static constexpr int Y0 = NVW * XV;               // two y slabs (low, high)
-  static constexpr int ZV = H * N * N;              // z slab [h][j][i]
-  static constexpr int Z0 = Y0 + 2 * NVW * YV;
-  static constexpr int TOTAL = Z0 + 2 * NVW * ZV;
-  // offset of variable 0 and variable stride of the cell at position c in [-H, 8+H) along axis D
-  // of the pencil (a, b) = the two other axes in increasing order
-  template <int D>
-  __device__ static __forceinline__ int off(int c, int a, int b) {
-    if (D == 0) return X0 + (b * 8 + a) * RS + c + H;
-    if (D == 1) {
-      if (c < 0) return Y0 + (b * H + (c + H)) * 8 + a;
-      if (c >= N) return Y0 + NVW * YV + (b * H + (c - N)) * 8 + a;
-      return X0 + (b * 8 + c) * RS + a + H;
-    }
-    if (c < 0) return Z0 + ((c + H) * 8 + b) * 8 + a;
-    if (c >= N) return Z0 + NVW * ZV + ((c - N) * 8 + b) * 8 + a;
-    return X0 + (c * 8 + b) * RS + a + H;
-  }
-  template <int D>
-  __device__ static __forceinline__ int vs(int c) {
-    if (D == 0) return XV;
-    if (D == 1) return (c < 0 || c >= N) ? YV : XV;
-    return (c < 0 || c >= N) ? ZV : XV;
-  }
+  static constexpr int RS = N + 2 * H + 1;          // x-row stride
+  static constexpr int YS = N * H * N;              // one y slab
+  static constexpr int ZS = H * N * N;              // one z slab
+  static constexpr int Y0 = 64 * RS;
+  static constexpr int Z0 = Y0 + 2 * YS;
+  static constexpr int VS = Z0 + 2 * ZS;            // variable stride
+  static constexpr int TOTAL = NVW * VS;
 };
 
 // ---- conversion of the staged conserved cells to primitives --------------------------------------
@@ -68,11 +50,11 @@ __device__ __forceinline__ void convert_block(const double* __restrict__ L, doub
   constexpr int NVW = STAGE == 0 ? 7 : 5;
   using WL = WLayout<H, NVW>;
   for (int idx = tid; idx < NC + 6 * NG * FACE; idx += STAGE_THREADS) {
-    int src, svs, dst, dvs;
+    int src, svs, dst;
     if (idx < NC) {
       const int i = idx & 7, j = (idx >> 3) & 7, k = idx >> 6;
       src = LAND_INT + idx; svs = NC;
-      dst = WL::X0 + (k * 8 + j) * WL::RS + i + H; dvs = WL::XV;
+      dst = (k * 8 + j) * WL::RS + i + H;
     } else {
       const int q = idx - NC, f = q >> 7, r = q & 127, axis = f >> 1, side = f & 1;
       const bool outflow = fsrc[f] == SRC_OUTFLOW;
@@ -84,7 +66,7 @@ __device__ __forceinline__ void convert_block(const double* __restrict__ L, doub
         const int c = side ? N + ll : ll - NG;
         if (c < -H || c >= N + H) continue;
         src = outflow ? LAND_INT + k * 64 + j * 8 + edge : LAND_HALO + f * SLAB + r;
-        dst = WL::X0 + (k * 8 + j) * WL::RS + c + H; dvs = WL::XV;
+        dst = (k * 8 + j) * WL::RS + c + H;
       } else if (axis == 1) {
         const int i = r & 7, k = r >> 4;
         ll = (r >> 3) & 1;
@@ -92,7 +74,7 @@ __device__ __forceinline__ void convert_block(const double* __restrict__ L, doub
         if (c < -H || c >= N + H) continue;
         const int hh = side ? c - N : c + H;
         src = outflow ? LAND_INT + k * 64 + edge * 8 + i : LAND_HALO + f * SLAB + r;
-        dst = WL::Y0 + side * NVW * WL::YV + (k * H + hh) * 8 + i; dvs = WL::YV;
+        dst = WL::Y0 + side * WL::YS + (k * H + hh) * 8 + i;
       } else {
         const int i = r & 7, j = (r >> 3) & 7;
         ll = r >> 6;
@@ -100,7 +82,7 @@ __device__ __forceinline__ void convert_block(const double* __restrict__ L, doub
         if (c < -H || c >= N + H) continue;
         const int hh = side ? c - N : c + H;
         src = outflow ? LAND_INT + edge * 64 + j * 8 + i : LAND_HALO + f * SLAB + r;
-        dst = WL::Z0 + side * NVW * WL::ZV + (hh * 8 + j) * 8 + i; dvs = WL::ZV;
+        dst = WL::Z0 + side * WL::ZS + (hh * 8 + j) * 8 + i;
       }
       svs = outflow ? NC : NG * FACE;
     }
@@ -109,149 +91,174 @@ __device__ __forceinline__ void convert_block(const double* __restrict__ L, doub
     for (int v = 0; v < 5; ++v) u[v] = L[src + v * svs];
     const double ir = cons_to_prim(u, gm1, w);
 #pragma unroll
-    for (int v = 0; v < 5; ++v) W[dst + v * dvs] = w[v];
+    for (int v = 0; v < 5; ++v) W[dst + v * WL::VS] = w[v];
     if (STAGE == 0) {
       const double c2 = (gamma * w[4]) * ir;         // c_s^2 = gamma P / rho
-      W[dst + 5 * dvs] = c2 * rsqrt(c2);
-      W[dst + 6 * dvs] = u[4];                       // total energy of the cell (eq. 8)
+      W[dst + 5 * WL::VS] = c2 * rsqrt_fast(c2);
+      W[dst + 6 * WL::VS] = u[4];                    // total energy of the cell (eq. 8)
     }
   }
 }
 
 // ---- pencil walks ----------------------------------------------------------------------------------
 // One thread per pencil; 64 pencils per axis; the three axes run side by side in different warps but
-// through the SAME rolled loop (runtime strides), so the instruction footprint is one flux body per
-// stage.  Face f = 0..8 of a pencil lies between cells f-1 and f; each flux is computed once and used
-// by both adjacent cells (the paper's mapping).
+// through the SAME loop body (run-time positions and strides), so the instruction footprint is one
+// flux body per stage.  Face f = 0..8 of a pencil lies between cells f-1 and f; each flux is computed
+// once and used by both adjacent cells (the paper's mapping).  A pencil is three runs of
+// positions in W: cells -H..-1 (low halo), 0..7 (interior x row), 8..7+H (high halo); the walk keeps
+// one running position that is re-seated when it enters the next run.  Loops are unrolled by two so
+// that the carried cell/face state ping-pongs between registers instead of being moved.
 template <int H, int NVW>
 struct Pencil {
   using WL = WLayout<H, NVW>;
-  int lo0, lo_cs, lo_vs;   // cells c < 0:   offset lo0 + (c + H) * lo_cs, variable stride lo_vs
-  int mid0, mid_cs;        // cells 0..7:    offset mid0 + c * mid_cs,     variable stride XV
-  int hi0, hi_cs, hi_vs;   // cells c >= 8:  offset hi0 + (c - 8) * hi_cs
-  int vn, vt1, vt2;        // variable slots of the normal / tangential velocities (momenta)
+  int lo0, lo_cs;          // cell c < 0 at lo0 + (c + H) * lo_cs
+  int mid0, mid_cs;        // cell 0..7 at mid0 + c * mid_cs
+  int hi0, hi_cs;          // cell c >= 8 at hi0 + (c - 8) * hi_cs
+  int on, ot1, ot2;        // offsets of the normal / tangential velocity variables
   int df0, df_cs, df_swz;  // flux-difference index of cell c: df0 + ((c ^ df_swz) * df_cs)
   __device__ __forceinline__ Pencil(int D, int a, int b) {
-    vn = 1 + D; vt1 = 1 + (D + 1) % 3; vt2 = 1 + (D + 2) % 3;
+    on = (1 + D) * WL::VS; ot1 = (1 + (D + 1) % 3) * WL::VS; ot2 = (1 + (D + 2) % 3) * WL::VS;
     if (D == 0) {
-      lo0 = (b * 8 + a) * WL::RS; lo_cs = 1; lo_vs = WL::XV;
+      lo0 = (b * 8 + a) * WL::RS; lo_cs = 1;
       mid0 = lo0 + H; mid_cs = 1;
-      hi0 = mid0 + N; hi_cs = 1; hi_vs = WL::XV;
+      hi0 = mid0 + N; hi_cs = 1;
       df0 = (b * 8 + a) * 8; df_cs = 1; df_swz = a;      // x rows are XOR swizzled (bank spread)
     } else if (D == 1) {
-      lo0 = WL::Y0 + b * H * 8 + a; lo_cs = 8; lo_vs = WL::YV;
+      lo0 = WL::Y0 + b * H * 8 + a; lo_cs = 8;
       mid0 = b * 8 * WL::RS + a + H; mid_cs = WL::RS;
-      hi0 = lo0 + NVW * WL::YV; hi_cs = 8; hi_vs = WL::YV;
+      hi0 = lo0 + WL::YS; hi_cs = 8;
       df0 = D * BLK + b * 64 + a; df_cs = 8; df_swz = 0;
     } else {
-      lo0 = WL::Z0 + b * 8 + a; lo_cs = 64; lo_vs = WL::ZV;
+      lo0 = WL::Z0 + b * 8 + a; lo_cs = 64;
       mid0 = b * WL::RS + a + H; mid_cs = 8 * WL::RS;
-      hi0 = lo0 + NVW * WL::ZV; hi_cs = 64; hi_vs = WL::ZV;
+      hi0 = lo0 + WL::ZS; hi_cs = 64;
       df0 = D * BLK + b * 8 + a; df_cs = 64; df_swz = 0;
     }
   }
-  // loads cell c >= 0 in the face frame (rho, normal v, tangential v's, P[, c_s])
-  __device__ __forceinline__ void load(const double* __restrict__ W, int c, double w[NVW]) const {
-    const bool hi = c >= N;
-    const int o = hi ? hi0 + (c - N) * hi_cs : mid0 + c * mid_cs;
-    const int s = hi ? hi_vs : WL::XV;
-    w[0] = W[o]; w[1] = W[o + vn * s]; w[2] = W[o + vt1 * s]; w[3] = W[o + vt2 * s]; w[4] = W[o + 4 * s];
-    if (NVW == 7) { w[5] = W[o + 5 * s]; w[NVW - 1] = W[o + 6 * s]; }
+  // the cell at position o, in the face frame (rho, normal v, tangential v's, P[, c_s, E])
+  __device__ __forceinline__ void load(const double* __restrict__ W, int o, double w[NVW]) const {
+    w[0] = W[o]; w[1] = W[o + on]; w[2] = W[o + ot1]; w[3] = W[o + ot2]; w[4] = W[o + 4 * WL::VS];
+    if (NVW == 7) { w[5] = W[o + 5 * WL::VS]; w[6] = W[o + 6 * WL::VS]; }
   }
-  __device__ __forceinline__ void load_lo(const double* __restrict__ W, int c, double w[NVW]) const {
-    const int o = lo0 + (c + H) * lo_cs, s = lo_vs;
-    w[0] = W[o]; w[1] = W[o + vn * s]; w[2] = W[o + vt1 * s]; w[3] = W[o + vt2 * s]; w[4] = W[o + 4 * s];
-    if (NVW == 7) { w[5] = W[o + 5 * s]; w[NVW - 1] = W[o + 6 * s]; }
-  }
-  // dF of cell c = F(face c+1) - F(face c), stored in the global variable order
+  // dF of cell c = F(face c+1) - F(face c), stored in the FACE frame (the update un-permutes)
   __device__ __forceinline__ void store_df(double* __restrict__ dF, int c, const double Fa[5], const double Fb[5]) const {
     const int ci = df0 + ((c ^ df_swz) * df_cs);
-    dF[ci] = Fa[0] - Fb[0];
-    dF[ci + vn * NC] = Fa[1] - Fb[1];
-    dF[ci + vt1 * NC] = Fa[2] - Fb[2];
-    dF[ci + vt2 * NC] = Fa[3] - Fb[3];
-    dF[ci + 4 * NC] = Fa[4] - Fb[4];
+#pragma unroll
+    for (int q = 0; q < 5; ++q) dF[ci + q * NC] = Fa[q] - Fb[q];
   }
 };
 
 // flux registers at coarse-fine faces (a7; reading R14); Fn in the face frame
-__device__ __forceinline__ void store_regs(const StageParams& p, int blk, int D, int side, int t, int vn, int vt1,
-                                           int vt2, const double Fn[5], double dt) {
+__device__ __noinline__ void store_regs(const int32_t* face_src, const int32_t* fslot, double* R, double* FH, int blk,
+                                        int D, int side, int t, double F0, double F1, double F2, double F3, double F4,
+                                        double dt) {
+  const double Fn[5] = {F0, F1, F2, F3, F4};
   const int f = 2 * D + side;
-  const int src = p.face_src[blk * 6 + f];
-  const int fs = p.fslot[blk * 6 + f];
+  const int src = face_src[blk * 6 + f];
+  const int fs = fslot[blk * 6 + f];
+  const int vn = 1 + D, vt1 = 1 + (D + 1) % 3, vt2 = 1 + (D + 2) % 3;
   if (src <= -2) {   // fine side of a coarse-fine face: accumulate dt * F
-    double* r = p.R + size_t(-2 - src) * REG + t;
+    double* r = R + size_t(-2 - src) * REG + t;
     r[0] += dt * Fn[0]; r[vn * FACE] += dt * Fn[1]; r[vt1 * FACE] += dt * Fn[2]; r[vt2 * FACE] += dt * Fn[3];
     r[4 * FACE] += dt * Fn[4];
   }
   if (fs >= 0) {     // coarse leaf next to a covered block: keep its own flux
-    double* r = p.FH + size_t(fs) * REG + t;
+    double* r = FH + size_t(fs) * REG + t;
     r[0] = Fn[0]; r[vn * FACE] = Fn[1]; r[vt1 * FACE] = Fn[2]; r[vt2 * FACE] = Fn[3]; r[4 * FACE] = Fn[4];
   }
 }
 
+// predictor: first-order HLLC on the cell-centred states (reading R8)
 __device__ __forceinline__ void walk_predictor(const double* __restrict__ W, double* __restrict__ dF, int D, int a, int b,
                                                double igm1) {
   const Pencil<1, 7> pc(D, a, b);
-  double wl[7], Fp[5];
-  pc.load_lo(W, -1, wl);
+  double w0[7], w1[7], F0[5], F1[5];
+  pc.load(W, pc.lo0, w0);                     // cell -1
+  pc.load(W, pc.mid0, w1);                    // cell 0
+  hllc_flux<true>(w0[0], w0[1], w0[2], w0[3], w0[4], w0[5], w0[6], w1[0], w1[1], w1[2], w1[3], w1[4], w1[5], w1[6],
+                  igm1, F0);                  // face 0
+  int o = pc.mid0;
 #pragma unroll 1
-  for (int f = 0; f <= N; ++f) {
-    double wr[7], Fn[5];
-    pc.load(W, f, wr);
-    hllc_flux<true>(wl[0], wl[1], wl[2], wl[3], wl[4], wl[5], wl[6], wr[0], wr[1], wr[2], wr[3], wr[4], wr[5], wr[6],
-                    igm1, Fn);
-    if (f > 0) pc.store_df(dF, f - 1, Fn, Fp);
-#pragma unroll
-    for (int v = 0; v < 5; ++v) Fp[v] = Fn[v];
-#pragma unroll
-    for (int v = 0; v < 7; ++v) wl[v] = wr[v];
+  for (int f = 1; f < N; f += 2) {            // faces f (cells f-1 | f) and f+1 (cells f | f+1)
+    o += pc.mid_cs;
+    pc.load(W, o, w0);                        // cell f
+    hllc_flux<true>(w1[0], w1[1], w1[2], w1[3], w1[4], w1[5], w1[6], w0[0], w0[1], w0[2], w0[3], w0[4], w0[5], w0[6],
+                    igm1, F1);
+    pc.store_df(dF, f - 1, F1, F0);
+    o = (f + 1 == N) ? pc.hi0 : o + pc.mid_cs;
+    pc.load(W, o, w1);                        // cell f+1
+    hllc_flux<true>(w0[0], w0[1], w0[2], w0[3], w0[4], w0[5], w0[6], w1[0], w1[1], w1[2], w1[3], w1[4], w1[5], w1[6],
+                    igm1, F0);
+    pc.store_df(dF, f, F0, F1);
   }
+}
+
+// corrector: minmod-limited linear reconstruction of the primitives (readings R11, R12) + HLLC
+struct FaceState { double v[5]; };
+// slope of the cell with value wc from its two one-sided differences; returns the right state of the
+// cell's lower face in R and the left state of its upper face in Lnext:  W -/+ minmod/2
+__device__ __forceinline__ void limited_states(const double wc[5], const double dn[5], const double dm[5], double R[5],
+                                               double Lnext[5]) {
+#pragma unroll
+  for (int v = 0; v < 5; ++v) {
+    // minmod(dn, dm)/2 = k m with m the difference of smaller magnitude, k = 1/2 if the signs agree
+    const double m = fabs(dn[v]) < fabs(dm[v]) ? dn[v] : dm[v];
+    const bool same = (__double2hiint(dn[v]) ^ __double2hiint(dm[v])) >= 0;
+    const double k = __hiloint2double(same ? 0x3fe00000 : 0, 0);
+    R[v] = fma(-k, m, wc[v]);
+    Lnext[v] = fma(k, m, wc[v]);
+  }
+}
+__device__ __forceinline__ void corrector_flux(const double WLs[5], const double WRs[5], double gamma, double igm1,
+                                               double Fn[5]) {
+  const double cL = sound_speed(gamma, WLs[4], WLs[0]);
+  const double cR = sound_speed(gamma, WRs[4], WRs[0]);
+  hllc_flux<false>(WLs[0], WLs[1], WLs[2], WLs[3], WLs[4], cL, 0.0, WRs[0], WRs[1], WRs[2], WRs[3], WRs[4], cR, 0.0,
+                   igm1, Fn);
 }
 
 __device__ __forceinline__ void walk_corrector(const double* __restrict__ W, double* __restrict__ dF, int D, int a, int b,
                                                double gamma, double igm1, const StageParams& p, int blk, double dt) {
   const Pencil<2, 5> pc(D, a, b);
-  // cells -2, -1: the left face state of face 0 needs the slope of cell -1
-  double wm[5], wc[5], dm[5], WLs[5], Fp[5];
-  pc.load_lo(W, -2, wm);
-  pc.load_lo(W, -1, wc);
+  double wa[5], wb[5], da[5], db[5], La[5], Lb[5], R[5], F0[5], F1[5];
+  // cells -2, -1, 0: slope of cell -1 -> left state of face 0
+  pc.load(W, pc.lo0, wa);
+  pc.load(W, pc.lo0 + pc.lo_cs, wb);
 #pragma unroll
-  for (int v = 0; v < 5; ++v) { dm[v] = wc[v] - wm[v]; WLs[v] = 0.0; Fp[v] = 0.0; }
-  // invariant at the top of iteration c (c = 0..9): wc = W_{c-1}, dm = W_{c-1} - W_{c-2};
-  // for c >= 1, WLs = left state of face c-1 (= W_{c-2} + slope_{c-2}/2)
+  for (int v = 0; v < 5; ++v) da[v] = wb[v] - wa[v];          // W_-1 - W_-2
+  pc.load(W, pc.mid0, wa);
+#pragma unroll
+  for (int v = 0; v < 5; ++v) db[v] = wa[v] - wb[v];          // W_0 - W_-1
+  limited_states(wb, db, da, R, La);                          // La = left state of face 0
+  // face 0: cell 1 gives the slope of cell 0
+  int o = pc.mid0 + pc.mid_cs;
+  pc.load(W, o, wb);
+#pragma unroll
+  for (int v = 0; v < 5; ++v) da[v] = wb[v] - wa[v];          // W_1 - W_0
+  limited_states(wa, da, db, R, Lb);                          // R = right state of face 0, Lb = left of face 1
+  corrector_flux(La, R, gamma, igm1, F0);
+  if (p.use_regs) store_regs(p.face_src, p.fslot, p.R, p.FH, blk, D, 0, b * 8 + a, F0[0], F0[1], F0[2], F0[3], F0[4], dt);
+  // invariant at the top of a trip (f odd): wb = W_f, da = W_f - W_{f-1}, Lb = left state of face f,
+  // F0 = flux of face f-1, o = position of cell f
 #pragma unroll 1
-  for (int c = 0; c <= N + 1; ++c) {
-    double wn[5], dn[5], sl[5];
-    pc.load(W, c, wn);
+  for (int f = 1; f < N; f += 2) {
+    o = (f + 1 == N) ? pc.hi0 : o + pc.mid_cs;
+    const int cs = (f + 1 == N) ? pc.hi_cs : pc.mid_cs;
+    pc.load(W, o, wa);                                        // cell f+1
 #pragma unroll
-    for (int v = 0; v < 5; ++v) {
-      dn[v] = wn[v] - wc[v];
-      sl[v] = minmod(dn[v], dm[v]);      // slope of cell c-1 (reading R12), primitives (R11)
-    }
-    if (c >= 1) {
-      // face f = c-1 between cells c-2 and c-1: right state from cell c-1
-      double WRs[5], Fn[5];
+    for (int v = 0; v < 5; ++v) db[v] = wa[v] - wb[v];
+    limited_states(wb, db, da, R, La);                        // right state of face f, left of face f+1
+    corrector_flux(Lb, R, gamma, igm1, F1);                   // face f
+    pc.store_df(dF, f - 1, F1, F0);
+    o += cs;
+    pc.load(W, o, wb);                                        // cell f+2
 #pragma unroll
-      for (int v = 0; v < 5; ++v) WRs[v] = wc[v] - 0.5 * sl[v];
-      const double cL = sound_speed(gamma, WLs[4], WLs[0]);
-      const double cR = sound_speed(gamma, WRs[4], WRs[0]);
-      hllc_flux<false>(WLs[0], WLs[1], WLs[2], WLs[3], WLs[4], cL, 0.0, WRs[0], WRs[1], WRs[2], WRs[3], WRs[4], cR, 0.0,
-                       igm1, Fn);
-      const int f = c - 1;
-      if (f > 0) pc.store_df(dF, f - 1, Fn, Fp);
-      if (p.use_regs && (f == 0 || f == N)) store_regs(p, blk, D, f == N, b * 8 + a, pc.vn, pc.vt1, pc.vt2, Fn, dt);
-#pragma unroll
-      for (int v = 0; v < 5; ++v) Fp[v] = Fn[v];
-    }
-#pragma unroll
-    for (int v = 0; v < 5; ++v) {
-      WLs[v] = wc[v] + 0.5 * sl[v];      // left state of face c
-      wc[v] = wn[v];
-      dm[v] = dn[v];
-    }
+    for (int v = 0; v < 5; ++v) da[v] = wb[v] - wa[v];
+    limited_states(wa, da, db, R, Lb);                        // right state of face f+1, left of face f+2
+    corrector_flux(La, R, gamma, igm1, F0);                   // face f+1
+    pc.store_df(dF, f, F0, F1);
   }
+  if (p.use_regs) store_regs(p.face_src, p.fslot, p.R, p.FH, blk, D, 1, b * 8 + a, F0[0], F0[1], F0[2], F0[3], F0[4], dt);
 }
 
 // ---- the stage kernel --------------------------------------------------------------------------------
@@ -308,25 +315,32 @@ stage_kernel(const __grid_constant__ TensorMaps tm, const StageParams p) {
   }
   __syncthreads();
 
-  // U_out = U^n - lambda ((dFx + dFy) + dFz), lambda = dt/(2h) (predictor) or dt/h (corrector)
+  // U_out = U^n - lambda ((dFx + dFy) + dFz), lambda = dt/(2h) (predictor) or dt/h (corrector).
+  // The flux differences are stored in the face frame (mass, normal, tangential 1, tangential 2,
+  // energy): variable v of axis D is entry q with 1 + (D + q - 1) % 3 == v, q = 1..3.
   const double lam = (STAGE == 0 ? 0.5 * dt : dt) / p.h;
   const double* __restrict__ Un = p.Un + size_t(blk) * BLK;
   double* __restrict__ Uo = p.Udst + size_t(blk) * BLK;
-  constexpr int ROUNDS = (BLK + STAGE_THREADS - 1) / STAGE_THREADS;
-  double un[ROUNDS];
+  constexpr int CR = (NC + STAGE_THREADS - 1) / STAGE_THREADS;   // 3 rounds of cells, all 5 variables each
+  double un[CR][NV];
 #pragma unroll
-  for (int r = 0; r < ROUNDS; ++r) {          // all loads in flight before the first use
-    const int idx = tid + r * STAGE_THREADS;
-    un[r] = idx < BLK ? Un[idx] : 0.0;
+  for (int r = 0; r < CR; ++r) {              // all loads in flight before the first use
+    const int cell = tid + r * STAGE_THREADS;
+#pragma unroll
+    for (int v = 0; v < NV; ++v) un[r][v] = cell < NC ? Un[v * NC + cell] : 0.0;
   }
 #pragma unroll
-  for (int r = 0; r < ROUNDS; ++r) {
-    const int idx = tid + r * STAGE_THREADS;
-    if (idx < BLK) {
-      const int cell = idx & (NC - 1), v = idx >> 9, row = cell >> 3, i = cell & 7;
-      const double dfx = L[v * NC + row * 8 + (i ^ (row & 7))];
-      const double sum = (dfx + L[BLK + idx]) + L[2 * BLK + idx];
-      Uo[idx] = un[r] - lam * sum;
+  for (int r = 0; r < CR; ++r) {
+    const int cell = tid + r * STAGE_THREADS;
+    if (cell < NC) {
+      const int row = cell >> 3, i = cell & 7;
+      const int cx = row * 8 + (i ^ (row & 7));
+#pragma unroll
+      for (int v = 0; v < NV; ++v) {
+        const int qx = v, qy = (v == 0 || v == 4) ? v : 1 + (v + 1) % 3, qz = (v == 0 || v == 4) ? v : 1 + v % 3;
+        const double sum = (L[qx * NC + cx] + L[BLK + qy * NC + cell]) + L[2 * BLK + qz * NC + cell];
+        Uo[v * NC + cell] = un[r][v] - lam * sum;
+      }
     }
   }
 }
