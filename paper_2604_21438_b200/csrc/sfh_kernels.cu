@@ -44,59 +44,60 @@ struct WLayout {
 
 // ---- conversion of the staged conserved cells to primitives --------------------------------------
 template <int STAGE>
+__device__ __forceinline__ void convert_cell(const double* __restrict__ L, double* __restrict__ W, int src, int svs,
+                                             int dst, double gamma, double gm1) {
+  constexpr int H = STAGE == 0 ? 1 : 2;
+  constexpr int NVW = STAGE == 0 ? 7 : 5;
+  using WL = WLayout<H, NVW>;
+  double u[5], w[5];
+#pragma unroll
+  for (int v = 0; v < 5; ++v) u[v] = L[src + v * svs];
+  const double ir = cons_to_prim(u, gm1, w);
+#pragma unroll
+  for (int v = 0; v < 5; ++v) W[dst + v * WL::VS] = w[v];
+  if (STAGE == 0) {
+    const double c2 = (gamma * w[4]) * ir;         // c_s^2 = gamma P / rho
+    W[dst + 5 * WL::VS] = c2 * rsqrt_fast(c2);
+    W[dst + 6 * WL::VS] = u[4];                    // total energy of the cell (eq. 8)
+  }
+}
+
+// Interior: 512 cells in 3 rounds.  Halo: the H layers next to each of the 6 faces, 64 H cells per
+// face; a warp covers 32 consecutive cells of ONE face, so the per-axis branches are warp-uniform.
+// An outflow face (reading R1) has no staged slab: its halo cells copy the block's own edge layer.
+template <int STAGE>
 __device__ __forceinline__ void convert_block(const double* __restrict__ L, double* __restrict__ W,
                                               const int* __restrict__ fsrc, double gamma, double gm1, int tid) {
   constexpr int H = STAGE == 0 ? 1 : 2;
   constexpr int NVW = STAGE == 0 ? 7 : 5;
   using WL = WLayout<H, NVW>;
-  for (int idx = tid; idx < NC + 6 * NG * FACE; idx += STAGE_THREADS) {
-    int src, svs, dst;
-    if (idx < NC) {
-      const int i = idx & 7, j = (idx >> 3) & 7, k = idx >> 6;
-      src = LAND_INT + idx; svs = NC;
-      dst = (k * 8 + j) * WL::RS + i + H;
-    } else {
-      const int q = idx - NC, f = q >> 7, r = q & 127, axis = f >> 1, side = f & 1;
-      const bool outflow = fsrc[f] == SRC_OUTFLOW;
-      const int edge = side ? 7 : 0;
-      int ll;
-      if (axis == 0) {
-        ll = r & 1;
-        const int j = (r >> 1) & 7, k = r >> 4;
-        const int c = side ? N + ll : ll - NG;
-        if (c < -H || c >= N + H) continue;
-        src = outflow ? LAND_INT + k * 64 + j * 8 + edge : LAND_HALO + f * SLAB + r;
-        dst = (k * 8 + j) * WL::RS + c + H;
-      } else if (axis == 1) {
-        const int i = r & 7, k = r >> 4;
-        ll = (r >> 3) & 1;
-        const int c = side ? N + ll : ll - NG;
-        if (c < -H || c >= N + H) continue;
-        const int hh = side ? c - N : c + H;
-        src = outflow ? LAND_INT + k * 64 + edge * 8 + i : LAND_HALO + f * SLAB + r;
-        dst = WL::Y0 + side * WL::YS + (k * H + hh) * 8 + i;
-      } else {
-        const int i = r & 7, j = (r >> 3) & 7;
-        ll = r >> 6;
-        const int c = side ? N + ll : ll - NG;
-        if (c < -H || c >= N + H) continue;
-        const int hh = side ? c - N : c + H;
-        src = outflow ? LAND_INT + edge * 64 + j * 8 + i : LAND_HALO + f * SLAB + r;
-        dst = WL::Z0 + side * WL::ZS + (hh * 8 + j) * 8 + i;
-      }
-      svs = outflow ? NC : NG * FACE;
-    }
-    double u[5], w[5];
 #pragma unroll
-    for (int v = 0; v < 5; ++v) u[v] = L[src + v * svs];
-    const double ir = cons_to_prim(u, gm1, w);
+  for (int r = 0; r < 3; ++r) {
+    const int cell = tid + r * STAGE_THREADS;
+    if (cell < NC) convert_cell<STAGE>(L, W, LAND_INT + cell, NC, (cell >> 3) * WL::RS + (cell & 7) + H, gamma, gm1);
+  }
+  constexpr int PER_FACE = H * FACE;               // 64 or 128
 #pragma unroll
-    for (int v = 0; v < 5; ++v) W[dst + v * WL::VS] = w[v];
-    if (STAGE == 0) {
-      const double c2 = (gamma * w[4]) * ir;         // c_s^2 = gamma P / rho
-      W[dst + 5 * WL::VS] = c2 * rsqrt_fast(c2);
-      W[dst + 6 * WL::VS] = u[4];                    // total energy of the cell (eq. 8)
+  for (int r = 0; r < 6 * PER_FACE / STAGE_THREADS; ++r) {
+    const int q = tid + r * STAGE_THREADS;
+    const int f = q / PER_FACE, rr = q % PER_FACE, axis = f >> 1, side = f & 1;
+    const int t = rr & 63, ta = t & 7, tb = t >> 3;
+    const int hh = rr >> 6;                        // layer within the H halo layers, outwards-increasing index c
+    const int ll = side ? hh : hh + NG - H;        // layer within the staged 2-layer slab
+    const bool outflow = fsrc[f] == SRC_OUTFLOW;
+    const int edge = side ? N - 1 : 0;
+    int src, dst;
+    if (axis == 0) {          // ta = j, tb = k; slab [v][k][j][ll]
+      src = outflow ? LAND_INT + t * 8 + edge : LAND_HALO + f * SLAB + t * 2 + ll;
+      dst = t * WL::RS + (side ? N + H + hh : hh);
+    } else if (axis == 1) {   // ta = i, tb = k; slab [v][k][ll][i]
+      src = outflow ? LAND_INT + tb * 64 + edge * 8 + ta : LAND_HALO + f * SLAB + tb * 16 + ll * 8 + ta;
+      dst = WL::Y0 + side * WL::YS + (tb * H + hh) * 8 + ta;
+    } else {                  // ta = i, tb = j; slab [v][ll][j][i]
+      src = outflow ? LAND_INT + edge * 64 + t : LAND_HALO + f * SLAB + ll * 64 + t;
+      dst = WL::Z0 + side * WL::ZS + hh * 64 + t;
     }
+    convert_cell<STAGE>(L, W, src, outflow ? NC : NG * FACE, dst, gamma, gm1);
   }
 }
 
@@ -262,6 +263,38 @@ __device__ __forceinline__ void walk_corrector(const double* __restrict__ W, dou
 }
 
 // ---- the stage kernel --------------------------------------------------------------------------------
+// Persistent: CTA c of the grid handles blocks c, c + gridDim.x, ... of the level.  Per block:
+//   thread 0 stages the block (TMA) -> all wait on the mbarrier -> convert -> walks -> update.
+// The staging of the NEXT block is issued as soon as the update has read the flux differences (which
+// share the landing area), and the block after that is pulled into L2 at the same time, so that the
+// TMA copies hit L2 instead of paying the DRAM latency on the critical path.
+__device__ __forceinline__ void issue_stage_loads(const TensorMaps& tm, const StageParams& p, int blk, double* L,
+                                                  int* fsrc, uint32_t bar_a) {
+  int s[6];
+#pragma unroll
+  for (int f = 0; f < 6; ++f) s[f] = p.face_src[blk * 6 + f];
+  uint32_t bytes = BLK * 8;
+#pragma unroll
+  for (int f = 0; f < 6; ++f) {
+    fsrc[f] = s[f];
+    bytes += (s[f] != SRC_OUTFLOW) ? SLAB * 8 : 0;
+  }
+  fence_proxy_async();                    // the landing area was last written through the generic proxy
+  mbar_expect_tx(bar_a, bytes);           // (release: publishes fsrc to the threads that see the phase complete)
+  bulk_g2s(smem_u32(L + LAND_INT), p.Usrc + size_t(blk) * BLK, BLK * 8, bar_a);
+#pragma unroll
+  for (int f = 0; f < 6; ++f) {
+    const uint32_t dst = smem_u32(L + LAND_HALO + f * SLAB);
+    if (s[f] >= 0) {
+      // my low-side ghost layers are the neighbour's two highest layers, and vice versa
+      const int axis = f >> 1, lo = (f & 1) ? 0 : N - NG;
+      tensor4_g2s(dst, &tm.ax[axis], axis == 0 ? lo : 0, axis == 1 ? lo : 0, axis == 2 ? lo : 0, s[f] * NV, bar_a);
+    } else if (s[f] <= -2) {
+      bulk_g2s(dst, p.ghost + size_t(-2 - s[f]) * SLAB, SLAB * 8, bar_a);
+    }
+  }
+}
+
 template <int STAGE>
 __global__ void __launch_bounds__(STAGE_THREADS, 2)
 stage_kernel(const __grid_constant__ TensorMaps tm, const StageParams p) {
@@ -272,74 +305,71 @@ stage_kernel(const __grid_constant__ TensorMaps tm, const StageParams p) {
   int* fsrc = reinterpret_cast<int*>(bar + 2);     // halo source of the 6 faces
 
   const int tid = threadIdx.x;
-  const int blk = p.first + blockIdx.x;
+  const int last = p.first + p.count;
+  const int stride = gridDim.x;
+  int blk = p.first + blockIdx.x;
   const uint32_t bar_a = smem_u32(bar);
-  if (tid < 6) fsrc[tid] = p.face_src[blk * 6 + tid];
   if (tid == 0) {
     mbar_init(bar_a, 1);
     fence_mbar_init();
+    issue_stage_loads(tm, p, blk, L, fsrc, bar_a);
+    if (blk + stride < last) {
+      prefetch_l2(p.Usrc + size_t(blk + stride) * BLK, BLK * 8);
+      if (STAGE == 1) prefetch_l2(p.Un + size_t(blk + stride) * BLK, BLK * 8);
+    }
   }
   __syncthreads();
-  if (tid == 0) {
-    uint32_t bytes = BLK * 8;
+  const double gamma = p.gamma, gm1 = p.gamma - 1.0, igm1 = 1.0 / gm1;
+  const double dt = p.dt_dev ? *p.dt_dev : p.dt;
+  const double lam = (STAGE == 0 ? 0.5 * dt : dt) / p.h;
+  const int pen = tid & 63, pa = pen & 7, pb = pen >> 3, D = tid >> 6;
+  uint32_t parity = 0;
+
+  for (; blk < last; blk += stride) {
+    mbar_wait(bar_a, parity);
+    parity ^= 1;
+    convert_block<STAGE>(L, W, fsrc, gamma, gm1, tid);
+    __syncthreads();
+
+    if (STAGE == 0) walk_predictor(W, L, D, pa, pb, igm1);
+    else walk_corrector(W, L, D, pa, pb, gamma, igm1, p, blk, dt);
+
+    // U_out = U^n - lambda ((dFx + dFy) + dFz), lambda = dt/(2h) (predictor) or dt/h (corrector).
+    // The flux differences are stored in the face frame (mass, normal, tangential 1, tangential 2,
+    // energy): variable v of axis D is entry q with 1 + (D + q - 1) % 3 == v, q = 1..3.
+    const double* __restrict__ Un = p.Un + size_t(blk) * BLK;
+    double* __restrict__ Uo = p.Udst + size_t(blk) * BLK;
+    constexpr int CR = (NC + STAGE_THREADS - 1) / STAGE_THREADS;   // 3 rounds of cells, all 5 variables each
+    double un[CR][NV];
 #pragma unroll
-    for (int f = 0; f < 6; ++f) bytes += (fsrc[f] != SRC_OUTFLOW) ? SLAB * 8 : 0;
-    mbar_expect_tx(bar_a, bytes);
-    bulk_g2s(smem_u32(L + LAND_INT), p.Usrc + size_t(blk) * BLK, BLK * 8, bar_a);
+    for (int r = 0; r < CR; ++r) {              // in flight while the other walkers finish
+      const int cell = tid + r * STAGE_THREADS;
 #pragma unroll
-    for (int f = 0; f < 6; ++f) {
-      const int s = fsrc[f];
-      const uint32_t dst = smem_u32(L + LAND_HALO + f * SLAB);
-      if (s >= 0) {
-        // my low-side ghost layers are the neighbour's two highest layers, and vice versa
-        const int axis = f >> 1, lo = (f & 1) ? 0 : N - NG;
-        tensor4_g2s(dst, &tm.ax[axis], axis == 0 ? lo : 0, axis == 1 ? lo : 0, axis == 2 ? lo : 0, s * NV, bar_a);
-      } else if (s <= -2) {
-        bulk_g2s(dst, p.ghost + size_t(-2 - s) * SLAB, SLAB * 8, bar_a);
+      for (int v = 0; v < NV; ++v) un[r][v] = cell < NC ? Un[v * NC + cell] : 0.0;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < CR; ++r) {
+      const int cell = tid + r * STAGE_THREADS;
+      if (cell < NC) {
+        const int row = cell >> 3, i = cell & 7;
+        const int cx = row * 8 + (i ^ (row & 7));
+        double sum[NV];
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+          const int qx = v, qy = (v == 0 || v == 4) ? v : 1 + (v + 1) % 3, qz = (v == 0 || v == 4) ? v : 1 + v % 3;
+          sum[v] = (L[qx * NC + cx] + L[BLK + qy * NC + cell]) + L[2 * BLK + qz * NC + cell];
+        }
+#pragma unroll
+        for (int v = 0; v < NV; ++v) Uo[v * NC + cell] = un[r][v] - lam * sum[v];
       }
     }
-    // U^n of this block is read again in the update at the end: pull it towards L2 now
-    if (STAGE == 1) prefetch_l2(p.Un + size_t(blk) * BLK, BLK * 8);
-  }
-  const double gamma = p.gamma, gm1 = p.gamma - 1.0, igm1 = __drcp_rn(gm1);
-  const double dt = p.dt_dev ? *p.dt_dev : p.dt;
-  mbar_wait(bar_a, 0);
-
-  convert_block<STAGE>(L, W, fsrc, gamma, gm1, tid);
-  __syncthreads();
-
-  {
-    const int pen = tid & 63, a = pen & 7, b = pen >> 3, D = tid >> 6;
-    if (STAGE == 0) walk_predictor(W, L, D, a, b, igm1);
-    else walk_corrector(W, L, D, a, b, gamma, igm1, p, blk, dt);
-  }
-  __syncthreads();
-
-  // U_out = U^n - lambda ((dFx + dFy) + dFz), lambda = dt/(2h) (predictor) or dt/h (corrector).
-  // The flux differences are stored in the face frame (mass, normal, tangential 1, tangential 2,
-  // energy): variable v of axis D is entry q with 1 + (D + q - 1) % 3 == v, q = 1..3.
-  const double lam = (STAGE == 0 ? 0.5 * dt : dt) / p.h;
-  const double* __restrict__ Un = p.Un + size_t(blk) * BLK;
-  double* __restrict__ Uo = p.Udst + size_t(blk) * BLK;
-  constexpr int CR = (NC + STAGE_THREADS - 1) / STAGE_THREADS;   // 3 rounds of cells, all 5 variables each
-  double un[CR][NV];
-#pragma unroll
-  for (int r = 0; r < CR; ++r) {              // all loads in flight before the first use
-    const int cell = tid + r * STAGE_THREADS;
-#pragma unroll
-    for (int v = 0; v < NV; ++v) un[r][v] = cell < NC ? Un[v * NC + cell] : 0.0;
-  }
-#pragma unroll
-  for (int r = 0; r < CR; ++r) {
-    const int cell = tid + r * STAGE_THREADS;
-    if (cell < NC) {
-      const int row = cell >> 3, i = cell & 7;
-      const int cx = row * 8 + (i ^ (row & 7));
-#pragma unroll
-      for (int v = 0; v < NV; ++v) {
-        const int qx = v, qy = (v == 0 || v == 4) ? v : 1 + (v + 1) % 3, qz = (v == 0 || v == 4) ? v : 1 + v % 3;
-        const double sum = (L[qx * NC + cx] + L[BLK + qy * NC + cell]) + L[2 * BLK + qz * NC + cell];
-        Uo[v * NC + cell] = un[r][v] - lam * sum;
+    __syncthreads();                            // the landing area is free again
+    if (tid == 0 && blk + stride < last) {
+      issue_stage_loads(tm, p, blk + stride, L, fsrc, bar_a);
+      if (blk + 2 * stride < last) {
+        prefetch_l2(p.Usrc + size_t(blk + 2 * stride) * BLK, BLK * 8);
+        if (STAGE == 1) prefetch_l2(p.Un + size_t(blk + 2 * stride) * BLK, BLK * 8);
       }
     }
   }
@@ -349,7 +379,18 @@ static_assert(WLayout<2, 5>::TOTAL <= W_DOUBLES && WLayout<1, 7>::TOTAL <= W_DOU
 static_assert(LAND_DOUBLES <= DF_DOUBLES, "landing area must fit in the flux-difference area");
 static_assert((W_DOUBLES * 8) % 128 == 0 && (SLAB * 8) % 128 == 0 && (BLK * 8) % 128 == 0, "TMA destinations: 128 B");
 
+static int g_stage_ctas = 2 * 148;   // persistent grid: resident CTAs per SM x SMs (set by configure_kernels)
+
 cudaError_t configure_kernels() {
+  int dev = 0, sms = 0, per_sm = 0;
+  if (cudaGetDevice(&dev) == cudaSuccess &&
+      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0) {
+    cudaFuncSetAttribute(stage_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGE_SMEM);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, stage_kernel<1>, STAGE_THREADS, STAGE_SMEM) != cudaSuccess ||
+        per_sm < 1)
+      per_sm = 1;
+    g_stage_ctas = sms * per_sm;
+  }
   cudaError_t e = cudaFuncSetAttribute(stage_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGE_SMEM);
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(stage_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGE_SMEM);
@@ -361,8 +402,9 @@ cudaError_t configure_kernels() {
 
 cudaError_t launch_stage(int stage, const TensorMaps& tm, const StageParams& p, cudaStream_t st) {
   if (p.count <= 0) return cudaSuccess;
-  if (stage == 0) stage_kernel<0><<<p.count, STAGE_THREADS, STAGE_SMEM, st>>>(tm, p);
-  else stage_kernel<1><<<p.count, STAGE_THREADS, STAGE_SMEM, st>>>(tm, p);
+  const int grid = p.count < g_stage_ctas ? p.count : g_stage_ctas;
+  if (stage == 0) stage_kernel<0><<<grid, STAGE_THREADS, STAGE_SMEM, st>>>(tm, p);
+  else stage_kernel<1><<<grid, STAGE_THREADS, STAGE_SMEM, st>>>(tm, p);
   return cudaGetLastError();
 }
 
