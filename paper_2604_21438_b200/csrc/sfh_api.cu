@@ -87,12 +87,24 @@ int make_tensor_maps(void* base, int64_t nb, TensorMaps& out) {
   const cuuint64_t dims[4] = {N, N, N, cuuint64_t(NV) * cuuint64_t(nb)};
   const cuuint64_t strides[3] = {N * 8, N * N * 8, N * N * N * 8};
   const cuuint32_t estr[4] = {1, 1, 1, 1};
-  for (int axis = 0; axis < 3; ++axis) {
-    cuuint32_t box[4] = {N, N, N, NV};
-    box[axis] = NG;
-    const CUresult r = encode(&out.ax[axis], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, estr,
-                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                              CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  for (int axis = 0; axis < 4; ++axis) {      // 3 = the swizzled z-plane-pair map
+    CUresult r;
+    if (axis < 3) {
+      cuuint32_t box[4] = {N, N, N, NV};
+      box[axis] = NG;
+      r = encode(&out.ax[axis], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, estr,
+                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    } else {
+      // 128-byte swizzle wants 128-byte rows (a 64-byte inner box would be padded to 128-byte lines,
+      // measured): view two consecutive x rows (j, j+1) as one row of 16 doubles -> [5 nb][8][4][16]
+      const cuuint64_t dims2[4] = {2 * N, N / 2, N, cuuint64_t(NV) * cuuint64_t(nb)};
+      const cuuint64_t strides2[3] = {2 * N * 8, N * N * 8, N * N * N * 8};
+      const cuuint32_t box2[4] = {2 * N, N / 2, NG, NV};
+      r = encode(&out.zs, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims2, strides2, box2, estr,
+                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    }
     if (r != CUDA_SUCCESS) {
       char buf[96];
       snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled failed (CUresult %d)", int(r));
@@ -156,6 +168,11 @@ int fill_level(sfh_mesh* m, int l, int which, int interp, double tau, cudaStream
   p.nbr27 = m->d_nbr27;
   p.first = int(hm.cf_first[l]); p.count = int(hm.cf_count[l]);
   p.interp = interp; p.tau = tau;
+  // role 1 (the half-step state) is stored as primitives
+  p.c0_prim = !interp && which == 1;
+  p.c1_prim = 1;
+  p.out_prim = which == 1;
+  p.gamma = hm.cfg.gamma;
   {
     Timed tmr(m, 2, st);
     CU(launch_prolong(p, st), "prolong_kernel");
@@ -441,7 +458,7 @@ int sfh_set_state(sfh_mesh* m, int which, const double* d_U, void* stream) {
   if (which < 0 || which > 2 || !d_U) return fail(SFH_EINVAL, "bad argument");
   for (int l = 0; l < m->hm.nlev; ++l) {
     CU(launch_permute(d_U, role_buf(m, l, which), m->d_perm, int(m->hm.lev_first[l]), int(m->hm.lev_count[l]), 1,
-                      S(stream)), "permute_kernel");
+                      which == 1, m->hm.cfg.gamma, S(stream)), "permute_kernel");
     m->launches += m->hm.lev_count[l] > 0;
   }
   return SFH_OK;
@@ -453,7 +470,7 @@ int sfh_get_state(sfh_mesh* m, int which, double* d_U, void* stream) {
   if (which < 0 || which > 2 || !d_U) return fail(SFH_EINVAL, "bad argument");
   for (int l = 0; l < m->hm.nlev; ++l) {
     CU(launch_permute(role_buf(m, l, which), d_U, m->d_perm, int(m->hm.lev_first[l]), int(m->hm.lev_count[l]), 0,
-                      S(stream)), "permute_kernel");
+                      which == 1, m->hm.cfg.gamma, S(stream)), "permute_kernel");
     m->launches += m->hm.lev_count[l] > 0;
   }
   return SFH_OK;
@@ -474,7 +491,7 @@ int sfh_get_ghosted(sfh_mesh* m, int which, double* d_G, void* stream) {
   if (which < 0 || which > 2 || !d_G) return fail(SFH_EINVAL, "bad argument");
   for (int l = 0; l < m->hm.nlev; ++l) {
     CU(launch_ghosted(role_buf(m, l, which), m->ghost, m->d_face_src, m->d_perm, int(m->hm.lev_first[l]),
-                      int(m->hm.lev_count[l]), d_G, S(stream)), "ghosted_kernel");
+                      int(m->hm.lev_count[l]), which == 1, m->hm.cfg.gamma, d_G, S(stream)), "ghosted_kernel");
     m->launches += m->hm.lev_count[l] > 0;
   }
   return SFH_OK;
@@ -515,6 +532,8 @@ int sfh_restrict(sfh_mesh* m, int coarse_level, int src_role, int dst_role, void
   const HostMesh& hm = m->hm;
   if (coarse_level < 0 || coarse_level >= hm.nlev || src_role < 0 || src_role > 2 || dst_role < 0 || dst_role > 2)
     return fail(SFH_EINVAL, "bad argument");
+  if (src_role == 1 || dst_role == 1)
+    return fail(SFH_EINVAL, "the half-step state (role 1) is never restricted (DESIGN.md reading R10)");
   if (coarse_level + 1 >= hm.nlev || hm.restrict_count[coarse_level] == 0) return SFH_OK;
   CU(launch_restrict(role_buf(m, coarse_level + 1, src_role), role_buf(m, coarse_level, dst_role),
                      m->d_restrict_list + hm.restrict_first[coarse_level], m->d_child0,
@@ -611,7 +630,7 @@ int sfh_status(sfh_mesh* m, int which, int64_t* n_bad_cells, void* stream) {
   CU(cudaMemsetAsync(m->nbad, 0, 8, st), "memset");
   for (int l = 0; l < m->hm.nlev; ++l) {
     CU(launch_count_bad(role_buf(m, l, which), int(m->hm.lev_first[l]), int(m->hm.lev_count[l]), m->hm.cfg.gamma,
-                        m->nbad, st), "count_bad_kernel");
+                        which == 1, m->nbad, st), "count_bad_kernel");
     m->launches += m->hm.lev_count[l] > 0;
   }
   unsigned long long n = 0;

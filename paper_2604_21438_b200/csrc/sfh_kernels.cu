@@ -195,7 +195,6 @@ __device__ __forceinline__ void walk_predictor(const double* __restrict__ W, dou
 }
 
 // corrector: minmod-limited linear reconstruction of the primitives (readings R11, R12) + HLLC
-struct FaceState { double v[5]; };
 // slope of the cell with value wc from its two one-sided differences; returns the right state of the
 // cell's lower face in R and the left state of its upper face in Lnext:  W -/+ minmod/2
 __device__ __forceinline__ void limited_states(const double wc[5], const double dn[5], const double dm[5], double R[5],
@@ -218,58 +217,141 @@ __device__ __forceinline__ void corrector_flux(const double WLs[5], const double
                    igm1, Fn);
 }
 
-__device__ __forceinline__ void walk_corrector(const double* __restrict__ W, double* __restrict__ dF, int D, int a, int b,
+// ---- corrector: landing layout and walk -------------------------------------------------------------
+// The half-step state is stored as primitives, so the corrector needs no
+// conversion: the pencils walk the staged tiles where TMA put them.  Landing area (doubles), every
+// tile [v][128 cells] (variable stride 128):
+//   z column: 6 z-plane pairs of 640 doubles: the low z halo, the 4 interior pairs, the high z halo,
+//             each 128-byte swizzled (zs_pos), so a cell (i, j, k), k in [-2, 10), sits at
+//             ((k + 2) >> 1) * 640 + zs_pos(k & 1, j, i);
+//   then the x-low, x-high, y-low, y-high slabs, dense: x [v][k][j][ll], y [v][k][ll][i].
+constexpr int C_ZCOL = 0, C_XLO = 6 * SLAB, C_XHI = 7 * SLAB, C_YLO = 8 * SLAB, C_YHI = 9 * SLAB;
+constexpr int C_LAND = 10 * SLAB;                    // 6400 doubles
+constexpr int CORR_SMEM = (C_LAND + DF_DOUBLES) * 8 + 16 + 32 + 1024;   // 113712 B (1 KB alignment slack) -> 2 CTAs per SM
+constexpr int CVS = NG * FACE;                       // variable stride of every tile (128)
+
+__device__ __forceinline__ int c_pos_zcol(int i, int j, int k) { return ((k + 2) >> 1) * SLAB + zs_pos(k & 1, j, i); }
+
+// position of cell c in [-2, 10) of the pencil (a, b) along axis D
+template <int D>
+__device__ __forceinline__ int c_pos(int c, int a, int b) {
+  if (D == 2) return c_pos_zcol(a, b, c);
+  if (D == 0) {
+    if (c < 0) return C_XLO + (b * 8 + a) * 2 + c + 2;
+    if (c >= N) return C_XHI + (b * 8 + a) * 2 + c - N;
+    return c_pos_zcol(c, a, b);
+  }
+  if (c < 0) return C_YLO + b * 16 + (c + 2) * 8 + a;
+  if (c >= N) return C_YHI + b * 16 + (c - N) * 8 + a;
+  return c_pos_zcol(a, c, b);
+}
+
+template <int D>
+__device__ __forceinline__ void c_load(const double* __restrict__ Wl, int o, double w[5]) {
+  constexpr int vn = 1 + D, vt1 = 1 + (D + 1) % 3, vt2 = 1 + (D + 2) % 3;
+  w[0] = Wl[o]; w[1] = Wl[o + vn * CVS]; w[2] = Wl[o + vt1 * CVS]; w[3] = Wl[o + vt2 * CVS]; w[4] = Wl[o + 4 * CVS];
+}
+
+// dF of cell c of the pencil = F(face c+1) - F(face c), in the FACE frame (the update un-permutes)
+template <int D>
+__device__ __forceinline__ void c_store_df(double* __restrict__ dF, int c, int a, int b, const double Fa[5],
+                                           const double Fb[5]) {
+  const int ci = D == 0 ? (b * 8 + a) * 8 + (c ^ a) : D == 1 ? BLK + b * 64 + c * 8 + a : 2 * BLK + c * 64 + b * 8 + a;
+#pragma unroll
+  for (int q = 0; q < 5; ++q) dF[ci + q * NC] = Fa[q] - Fb[q];
+}
+
+template <int D>
+__device__ __forceinline__ void walk_corrector(const double* __restrict__ Wl, double* __restrict__ dF, int a, int b,
                                                double gamma, double igm1, const StageParams& p, int blk, double dt) {
-  const Pencil<2, 5> pc(D, a, b);
   double wa[5], wb[5], da[5], db[5], La[5], Lb[5], R[5], F0[5], F1[5];
   // cells -2, -1, 0: slope of cell -1 -> left state of face 0
-  pc.load(W, pc.lo0, wa);
-  pc.load(W, pc.lo0 + pc.lo_cs, wb);
+  c_load<D>(Wl, c_pos<D>(-2, a, b), wa);
+  c_load<D>(Wl, c_pos<D>(-1, a, b), wb);
 #pragma unroll
   for (int v = 0; v < 5; ++v) da[v] = wb[v] - wa[v];          // W_-1 - W_-2
-  pc.load(W, pc.mid0, wa);
+  c_load<D>(Wl, c_pos<D>(0, a, b), wa);
 #pragma unroll
   for (int v = 0; v < 5; ++v) db[v] = wa[v] - wb[v];          // W_0 - W_-1
   limited_states(wb, db, da, R, La);                          // La = left state of face 0
   // face 0: cell 1 gives the slope of cell 0
-  int o = pc.mid0 + pc.mid_cs;
-  pc.load(W, o, wb);
+  c_load<D>(Wl, c_pos<D>(1, a, b), wb);
 #pragma unroll
   for (int v = 0; v < 5; ++v) da[v] = wb[v] - wa[v];          // W_1 - W_0
   limited_states(wa, da, db, R, Lb);                          // R = right state of face 0, Lb = left of face 1
   corrector_flux(La, R, gamma, igm1, F0);
   if (p.use_regs) store_regs(p.face_src, p.fslot, p.R, p.FH, blk, D, 0, b * 8 + a, F0[0], F0[1], F0[2], F0[3], F0[4], dt);
   // invariant at the top of a trip (f odd): wb = W_f, da = W_f - W_{f-1}, Lb = left state of face f,
-  // F0 = flux of face f-1, o = position of cell f
+  // F0 = flux of face f-1
 #pragma unroll 1
   for (int f = 1; f < N; f += 2) {
-    o = (f + 1 == N) ? pc.hi0 : o + pc.mid_cs;
-    const int cs = (f + 1 == N) ? pc.hi_cs : pc.mid_cs;
-    pc.load(W, o, wa);                                        // cell f+1
+    c_load<D>(Wl, c_pos<D>(f + 1, a, b), wa);                 // cell f+1
 #pragma unroll
     for (int v = 0; v < 5; ++v) db[v] = wa[v] - wb[v];
     limited_states(wb, db, da, R, La);                        // right state of face f, left of face f+1
     corrector_flux(Lb, R, gamma, igm1, F1);                   // face f
-    pc.store_df(dF, f - 1, F1, F0);
-    o += cs;
-    pc.load(W, o, wb);                                        // cell f+2
+    c_store_df<D>(dF, f - 1, a, b, F1, F0);
+    c_load<D>(Wl, c_pos<D>(f + 2, a, b), wb);                 // cell f+2
 #pragma unroll
     for (int v = 0; v < 5; ++v) da[v] = wb[v] - wa[v];
     limited_states(wa, da, db, R, Lb);                        // right state of face f+1, left of face f+2
     corrector_flux(La, R, gamma, igm1, F0);                   // face f+1
-    pc.store_df(dF, f, F0, F1);
+    c_store_df<D>(dF, f, a, b, F0, F1);
   }
   if (p.use_regs) store_regs(p.face_src, p.fslot, p.R, p.FH, blk, D, 1, b * 8 + a, F0[0], F0[1], F0[2], F0[3], F0[4], dt);
 }
 
-// ---- the stage kernel --------------------------------------------------------------------------------
-// Persistent: CTA c of the grid handles blocks c, c + gridDim.x, ... of the level.  Per block:
-//   thread 0 stages the block (TMA) -> all wait on the mbarrier -> convert -> walks -> update.
-// The staging of the NEXT block is issued as soon as the update has read the flux differences (which
-// share the landing area), and the block after that is pulled into L2 at the same time, so that the
-// TMA copies hit L2 instead of paying the DRAM latency on the critical path.
-__device__ __forceinline__ void issue_stage_loads(const TensorMaps& tm, const StageParams& p, int blk, double* L,
-                                                  int* fsrc, uint32_t bar_a) {
+// ---- the stage kernels -------------------------------------------------------------------------------
+// Both are persistent: CTA c of the grid handles blocks c, c + gridDim.x, ... of the level, thread 0
+// stages each block with TMA and everybody waits on ONE mbarrier whose phase alternates per block.
+// The block after the one being staged is pulled into L2 at the same time, so the TMA copies hit L2
+// instead of paying the DRAM latency on the critical path.
+
+// U_out = U^n - lambda ((dFx + dFy) + dFz), lambda = dt/(2h) (predictor) or dt/h (corrector).
+// The flux differences are stored in the face frame (mass, normal, tangential 1, tangential 2,
+// energy): variable v of axis D is entry q with 1 + (D + q - 1) % 3 == v, q = 1..3.
+// 3 rounds of cells, all 5 variables each.  PRIM_OUT: store primitives (the half-step state).
+constexpr int CR = (NC + STAGE_THREADS - 1) / STAGE_THREADS;
+__device__ __forceinline__ void load_un(const double* __restrict__ Un, int tid, double un[CR][NV]) {
+#pragma unroll
+  for (int r = 0; r < CR; ++r) {
+    const int cell = tid + r * STAGE_THREADS;
+#pragma unroll
+    for (int v = 0; v < NV; ++v) un[r][v] = cell < NC ? Un[v * NC + cell] : 0.0;
+  }
+}
+template <bool PRIM_OUT>
+__device__ __forceinline__ void update_block(const double* __restrict__ dF, const double un[CR][NV], double lam,
+                                             double gm1, double* __restrict__ Uo, int tid) {
+#pragma unroll
+  for (int r = 0; r < CR; ++r) {
+    const int cell = tid + r * STAGE_THREADS;
+    if (cell < NC) {
+      const int row = cell >> 3, i = cell & 7;
+      const int cx = row * 8 + (i ^ (row & 7));
+      double u[NV];
+#pragma unroll
+      for (int v = 0; v < NV; ++v) {
+        const int qx = v, qy = (v == 0 || v == 4) ? v : 1 + (v + 1) % 3, qz = (v == 0 || v == 4) ? v : 1 + v % 3;
+        const double sum = (dF[qx * NC + cx] + dF[BLK + qy * NC + cell]) + dF[2 * BLK + qz * NC + cell];
+        u[v] = un[r][v] - lam * sum;
+      }
+      if (PRIM_OUT) {
+        double w[NV];
+        cons_to_prim(u, gm1, w);
+#pragma unroll
+        for (int v = 0; v < NV; ++v) Uo[v * NC + cell] = w[v];
+      } else {
+#pragma unroll
+        for (int v = 0; v < NV; ++v) Uo[v * NC + cell] = u[v];
+      }
+    }
+  }
+}
+
+// ---- predictor: stage conserved U^n -> convert -> walks -> update, stores W^{n+1/2} (primitives) ----
+__device__ __forceinline__ void issue_predictor_loads(const TensorMaps& tm, const StageParams& p, int blk, double* L,
+                                                      int* fsrc, uint32_t bar_a) {
   int s[6];
 #pragma unroll
   for (int f = 0; f < 6; ++f) s[f] = p.face_src[blk * 6 + f];
@@ -295,10 +377,9 @@ __device__ __forceinline__ void issue_stage_loads(const TensorMaps& tm, const St
   }
 }
 
-template <int STAGE>
 __global__ void __launch_bounds__(STAGE_THREADS, 2)
-stage_kernel(const __grid_constant__ TensorMaps tm, const StageParams p) {
-  extern __shared__ __align__(128) unsigned char smem_raw[];
+predictor_kernel(const __grid_constant__ TensorMaps tm, const StageParams p) {
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
   double* W = reinterpret_cast<double*>(smem_raw);
   double* L = W + W_DOUBLES;                       // landing area, later the flux differences
   uint64_t* bar = reinterpret_cast<uint64_t*>(L + DF_DOUBLES);
@@ -312,99 +393,172 @@ stage_kernel(const __grid_constant__ TensorMaps tm, const StageParams p) {
   if (tid == 0) {
     mbar_init(bar_a, 1);
     fence_mbar_init();
-    issue_stage_loads(tm, p, blk, L, fsrc, bar_a);
-    if (blk + stride < last) {
-      prefetch_l2(p.Usrc + size_t(blk + stride) * BLK, BLK * 8);
-      if (STAGE == 1) prefetch_l2(p.Un + size_t(blk + stride) * BLK, BLK * 8);
-    }
+    issue_predictor_loads(tm, p, blk, L, fsrc, bar_a);
+    if (blk + stride < last) prefetch_l2(p.Usrc + size_t(blk + stride) * BLK, BLK * 8);
   }
   __syncthreads();
   const double gamma = p.gamma, gm1 = p.gamma - 1.0, igm1 = 1.0 / gm1;
   const double dt = p.dt_dev ? *p.dt_dev : p.dt;
-  const double lam = (STAGE == 0 ? 0.5 * dt : dt) / p.h;
+  const double lam = 0.5 * dt / p.h;
   const int pen = tid & 63, pa = pen & 7, pb = pen >> 3, D = tid >> 6;
   uint32_t parity = 0;
 
   for (; blk < last; blk += stride) {
     mbar_wait(bar_a, parity);
     parity ^= 1;
-    convert_block<STAGE>(L, W, fsrc, gamma, gm1, tid);
+    convert_block<0>(L, W, fsrc, gamma, gm1, tid);
     __syncthreads();
-
-    if (STAGE == 0) walk_predictor(W, L, D, pa, pb, igm1);
-    else walk_corrector(W, L, D, pa, pb, gamma, igm1, p, blk, dt);
-
-    // U_out = U^n - lambda ((dFx + dFy) + dFz), lambda = dt/(2h) (predictor) or dt/h (corrector).
-    // The flux differences are stored in the face frame (mass, normal, tangential 1, tangential 2,
-    // energy): variable v of axis D is entry q with 1 + (D + q - 1) % 3 == v, q = 1..3.
-    const double* __restrict__ Un = p.Un + size_t(blk) * BLK;
-    double* __restrict__ Uo = p.Udst + size_t(blk) * BLK;
-    constexpr int CR = (NC + STAGE_THREADS - 1) / STAGE_THREADS;   // 3 rounds of cells, all 5 variables each
+    walk_predictor(W, L, D, pa, pb, igm1);
     double un[CR][NV];
-#pragma unroll
-    for (int r = 0; r < CR; ++r) {              // in flight while the other walkers finish
-      const int cell = tid + r * STAGE_THREADS;
-#pragma unroll
-      for (int v = 0; v < NV; ++v) un[r][v] = cell < NC ? Un[v * NC + cell] : 0.0;
-    }
+    load_un(p.Un + size_t(blk) * BLK, tid, un);   // in flight while the other walkers finish
     __syncthreads();
-#pragma unroll
-    for (int r = 0; r < CR; ++r) {
-      const int cell = tid + r * STAGE_THREADS;
-      if (cell < NC) {
-        const int row = cell >> 3, i = cell & 7;
-        const int cx = row * 8 + (i ^ (row & 7));
-        double sum[NV];
-#pragma unroll
-        for (int v = 0; v < NV; ++v) {
-          const int qx = v, qy = (v == 0 || v == 4) ? v : 1 + (v + 1) % 3, qz = (v == 0 || v == 4) ? v : 1 + v % 3;
-          sum[v] = (L[qx * NC + cx] + L[BLK + qy * NC + cell]) + L[2 * BLK + qz * NC + cell];
-        }
-#pragma unroll
-        for (int v = 0; v < NV; ++v) Uo[v * NC + cell] = un[r][v] - lam * sum[v];
-      }
-    }
-    __syncthreads();                            // the landing area is free again
+    update_block<true>(L, un, lam, gm1, p.Udst + size_t(blk) * BLK, tid);
+    __syncthreads();                              // the landing area is free again
     if (tid == 0 && blk + stride < last) {
-      issue_stage_loads(tm, p, blk + stride, L, fsrc, bar_a);
-      if (blk + 2 * stride < last) {
-        prefetch_l2(p.Usrc + size_t(blk + 2 * stride) * BLK, BLK * 8);
-        if (STAGE == 1) prefetch_l2(p.Un + size_t(blk + 2 * stride) * BLK, BLK * 8);
-      }
+      issue_predictor_loads(tm, p, blk + stride, L, fsrc, bar_a);
+      if (blk + 2 * stride < last) prefetch_l2(p.Usrc + size_t(blk + 2 * stride) * BLK, BLK * 8);
     }
   }
 }
 
-static_assert(WLayout<2, 5>::TOTAL <= W_DOUBLES && WLayout<1, 7>::TOTAL <= W_DOUBLES, "primitive array too small");
+// ---- corrector: stage W^{n+1/2} (primitives) -> walks -> update with U^n, stores U^{n+1} ------------
+// fsrc[6] = 1 if any face of the block is an outflow face
+__device__ __forceinline__ void issue_corrector_loads(const TensorMaps& tm, const StageParams& p, int blk, double* Wl,
+                                                      int* fsrc, uint32_t bar_a) {
+  int s[6];
+#pragma unroll
+  for (int f = 0; f < 6; ++f) s[f] = p.face_src[blk * 6 + f];
+  uint32_t bytes = BLK * 8;
+  int any_out = 0;
+#pragma unroll
+  for (int f = 0; f < 6; ++f) {
+    fsrc[f] = s[f];
+    bytes += (s[f] != SRC_OUTFLOW) ? SLAB * 8 : 0;
+    any_out |= s[f] == SRC_OUTFLOW;
+  }
+  fsrc[6] = any_out;
+  mbar_expect_tx(bar_a, bytes);           // (release: publishes fsrc to the threads that see the phase complete)
+#pragma unroll
+  for (int kk = 0; kk < 4; ++kk)          // interior: 4 z-plane pairs
+    tensor4_g2s(smem_u32(Wl + C_ZCOL + (1 + kk) * SLAB), &tm.zs, 0, 0, 2 * kk, blk * NV, bar_a);
+#pragma unroll
+  for (int f = 0; f < 6; ++f) {
+    const int axis = f >> 1, side = f & 1;
+    const uint32_t dst = smem_u32(Wl + (axis == 2 ? C_ZCOL + side * 5 * SLAB : axis == 0 ? C_XLO + side * SLAB
+                                                                                           : C_YLO + side * SLAB));
+    if (s[f] >= 0) {
+      const int lo = side ? 0 : N - NG;
+      if (axis == 2) tensor4_g2s(dst, &tm.zs, 0, 0, lo, s[f] * NV, bar_a);
+      else tensor4_g2s(dst, &tm.ax[axis], axis == 0 ? lo : 0, axis == 1 ? lo : 0, 0, s[f] * NV, bar_a);
+    } else if (s[f] <= -2) {
+      bulk_g2s(dst, p.ghost + size_t(-2 - s[f]) * SLAB, SLAB * 8, bar_a);   // z slabs come pre-swizzled
+    }
+  }
+}
+
+// halo of an outflow face (reading R1): copies of the block's own edge layer
+__device__ __forceinline__ void fill_outflow_slabs(double* __restrict__ Wl, const int* __restrict__ fsrc, int tid) {
+#pragma unroll 1
+  for (int q = tid; q < 6 * CVS; q += STAGE_THREADS) {
+    const int f = q >> 7, r = q & 127, axis = f >> 1, side = f & 1;
+    if (fsrc[f] != SRC_OUTFLOW) continue;
+    const int t = r & 63, ta = t & 7, tb = t >> 3, ll = r >> 6, edge = side ? N - 1 : 0;
+    int src, dst;
+    if (axis == 0) { src = c_pos_zcol(edge, ta, tb); dst = (side ? C_XHI : C_XLO) + t * 2 + ll; }
+    else if (axis == 1) { src = c_pos_zcol(ta, edge, tb); dst = (side ? C_YHI : C_YLO) + tb * 16 + ll * 8 + ta; }
+    else { src = c_pos_zcol(ta, tb, edge); dst = C_ZCOL + side * 5 * SLAB + zs_pos(ll, tb, ta); }
+#pragma unroll
+    for (int v = 0; v < NV; ++v) Wl[dst + v * CVS] = Wl[src + v * CVS];
+  }
+}
+
+__global__ void __launch_bounds__(STAGE_THREADS, 2)
+corrector_kernel(const __grid_constant__ TensorMaps tm, const StageParams p) {
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  // staged primitives, 1024-byte aligned (swizzle atoms)
+  double* Wl = reinterpret_cast<double*>(smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u));
+  double* dF = Wl + C_LAND;
+  uint64_t* bar = reinterpret_cast<uint64_t*>(dF + DF_DOUBLES);
+  int* fsrc = reinterpret_cast<int*>(bar + 2);
+
+  const int tid = threadIdx.x;
+  const int last = p.first + p.count;
+  const int stride = gridDim.x;
+  int blk = p.first + blockIdx.x;
+  const uint32_t bar_a = smem_u32(bar);
+  if (tid == 0) {
+    mbar_init(bar_a, 1);
+    fence_mbar_init();
+    issue_corrector_loads(tm, p, blk, Wl, fsrc, bar_a);
+    prefetch_l2(p.Un + size_t(blk) * BLK, BLK * 8);
+    if (blk + stride < last) {
+      prefetch_l2(p.Usrc + size_t(blk + stride) * BLK, BLK * 8);
+      prefetch_l2(p.Un + size_t(blk + stride) * BLK, BLK * 8);
+    }
+  }
+  __syncthreads();
+  const double gamma = p.gamma, gm1 = p.gamma - 1.0, igm1 = 1.0 / gm1;
+  const double dt = p.dt_dev ? *p.dt_dev : p.dt;
+  const double lam = dt / p.h;
+  const int pen = tid & 63, pa = pen & 7, pb = pen >> 3, D = tid >> 6;
+  uint32_t parity = 0;
+
+  for (; blk < last; blk += stride) {
+    mbar_wait(bar_a, parity);
+    parity ^= 1;
+    if (fsrc[6]) {                                // block-uniform
+      fill_outflow_slabs(Wl, fsrc, tid);
+      __syncthreads();
+    }
+    if (D == 0) walk_corrector<0>(Wl, dF, pa, pb, gamma, igm1, p, blk, dt);
+    else if (D == 1) walk_corrector<1>(Wl, dF, pa, pb, gamma, igm1, p, blk, dt);
+    else walk_corrector<2>(Wl, dF, pa, pb, gamma, igm1, p, blk, dt);
+    double un[CR][NV];
+    load_un(p.Un + size_t(blk) * BLK, tid, un);   // in flight while the other walkers finish
+    __syncthreads();                              // the staged primitives are dead, the flux differences complete
+    if (tid == 0 && blk + stride < last) {        // the next block lands while this one is updated
+      if (fsrc[6]) fence_proxy_async();           // outflow slabs were written through the generic proxy
+      issue_corrector_loads(tm, p, blk + stride, Wl, fsrc, bar_a);
+      if (blk + 2 * stride < last) {
+        prefetch_l2(p.Usrc + size_t(blk + 2 * stride) * BLK, BLK * 8);
+        prefetch_l2(p.Un + size_t(blk + 2 * stride) * BLK, BLK * 8);
+      }
+    }
+    update_block<false>(dF, un, lam, gm1, p.Udst + size_t(blk) * BLK, tid);
+    __syncthreads();                              // the flux differences are consumed
+  }
+}
+
+static_assert(WLayout<1, 7>::TOTAL <= W_DOUBLES, "primitive array too small");
 static_assert(LAND_DOUBLES <= DF_DOUBLES, "landing area must fit in the flux-difference area");
-static_assert((W_DOUBLES * 8) % 128 == 0 && (SLAB * 8) % 128 == 0 && (BLK * 8) % 128 == 0, "TMA destinations: 128 B");
+static_assert((W_DOUBLES * 8) % 128 == 0 && (SLAB * 8) % 1024 == 0 && (BLK * 8) % 128 == 0,
+              "TMA destinations: 128 B, swizzled tiles 1024 B");
 
 static int g_stage_ctas = 2 * 148;   // persistent grid: resident CTAs per SM x SMs (set by configure_kernels)
 
 cudaError_t configure_kernels() {
+  cudaError_t e = cudaFuncSetAttribute(predictor_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGE_SMEM);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(corrector_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, CORR_SMEM);
+  if (e != cudaSuccess) return e;
+  cudaFuncSetAttribute(predictor_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+  cudaFuncSetAttribute(corrector_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
   int dev = 0, sms = 0, per_sm = 0;
   if (cudaGetDevice(&dev) == cudaSuccess &&
       cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0) {
-    cudaFuncSetAttribute(stage_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGE_SMEM);
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, stage_kernel<1>, STAGE_THREADS, STAGE_SMEM) != cudaSuccess ||
-        per_sm < 1)
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, predictor_kernel, STAGE_THREADS, STAGE_SMEM) !=
+            cudaSuccess || per_sm < 1)
       per_sm = 1;
     g_stage_ctas = sms * per_sm;
   }
-  cudaError_t e = cudaFuncSetAttribute(stage_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGE_SMEM);
-  if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(stage_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGE_SMEM);
-  if (e != cudaSuccess) return e;
-  cudaFuncSetAttribute(stage_kernel<0>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-  cudaFuncSetAttribute(stage_kernel<1>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
   return cudaSuccess;
 }
 
 cudaError_t launch_stage(int stage, const TensorMaps& tm, const StageParams& p, cudaStream_t st) {
   if (p.count <= 0) return cudaSuccess;
   const int grid = p.count < g_stage_ctas ? p.count : g_stage_ctas;
-  if (stage == 0) stage_kernel<0><<<grid, STAGE_THREADS, STAGE_SMEM, st>>>(tm, p);
-  else stage_kernel<1><<<grid, STAGE_THREADS, STAGE_SMEM, st>>>(tm, p);
+  if (stage == 0) predictor_kernel<<<grid, STAGE_THREADS, STAGE_SMEM, st>>>(tm, p);
+  else corrector_kernel<<<grid, STAGE_THREADS, CORR_SMEM, st>>>(tm, p);
   return cudaGetLastError();
 }
 

@@ -25,9 +25,15 @@ struct StageParams {
   int use_regs;          // corrector: the level has flux-register faces
 };
 
-struct TensorMaps {      // tensor maps of ONE state buffer, one per face axis (box = 2-layer slab)
-  CUtensorMap ax[3];
+struct TensorMaps {      // tensor maps of ONE state buffer seen as [5 nb][8][8][8]
+  CUtensorMap ax[3];     // one per face axis, box = the 2-layer slab {2,8,8,5} / {8,2,8,5} / {8,8,2,5}, dense in smem
+  CUtensorMap zs;        // box {8,8,2,5} (a pair of z planes of all 5 variables), 128-byte swizzled in smem
 };
+
+// Position of cell (kl, j, i) of a z-plane pair inside a 128-byte-swizzled slab [v][kl][j][i] of fp64
+// (variable stride 128): the TMA swizzle XORs byte-address bits [4,7) with bits [7,10), i.e. the
+// 16-byte chunk (i >> 1, j & 1) with (j >> 1, kl).
+__host__ __device__ inline int zs_pos(int kl, int j, int i) { return (kl << 6) | ((j ^ kl) << 3) | (i ^ (j & 6)); }
 
 struct ProlongParams {
   const double* C0;      // coarse level: role `which` (interp = 0) or role 0 (interp = 1)
@@ -42,6 +48,9 @@ struct ProlongParams {
   int first, count;      // slab range of the fine level
   int interp;
   double tau;
+  int c0_prim, c1_prim;  // the coarse copy C0 / C1 holds primitives (the half-step state)
+  int out_prim;          // write primitives, z-face slabs in the swizzled order of zs_pos (half-step fill)
+  double gamma;
 };
 
 cudaError_t launch_stage(int stage, const TensorMaps& tm, const StageParams& p, cudaStream_t st);
@@ -61,13 +70,14 @@ struct LevelInfo {
 // dt = min_l cfl*h_l/smax_l over levels with blocks; *dt_dev = dt; *t_dev += dt
 cudaError_t launch_dt_finalize(const unsigned long long* smax_bits, const LevelInfo& li, double cfl, double* dt_dev,
                                double* t_dev, cudaStream_t st);
-cudaError_t launch_count_bad(const double* U, int first, int count, double gamma, unsigned long long* nbad,
+cudaError_t launch_count_bad(const double* U, int first, int count, double gamma, int prim, unsigned long long* nbad,
                              cudaStream_t st);
 // dst[slot][...] = src[perm[slot]][...] (to_internal) or the inverse, for slots [first, first+count)
+// prim: the internal copy holds primitives (role 1); the caller's copy is always conserved
 cudaError_t launch_permute(const double* src, double* dst, const int64_t* perm, int first, int count, int to_internal,
-                           cudaStream_t st);
+                           int prim, double gamma, cudaStream_t st);
 cudaError_t launch_ghosted(const double* U, const double* ghost, const int32_t* face_src, const int64_t* perm,
-                           int first, int count, double* G, cudaStream_t st);
+                           int first, int count, int prim, double gamma, double* G, cudaStream_t st);
 cudaError_t configure_kernels();
 
 }  // namespace sfh

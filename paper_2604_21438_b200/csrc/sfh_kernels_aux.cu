@@ -64,21 +64,53 @@ __global__ void __launch_bounds__(128) prolong_kernel(const ProlongParams p) {
   bool ok = true;
 #pragma unroll
   for (int s = 0; s < 7; ++s) ok = ok && o[s] >= 0;
-  double* out = p.ghost + size_t(slot) * SLAB + r;
+  const double gm1 = p.gamma - 1.0, igm1 = 1.0 / gm1;
+  // conserved values of the 7 stencil cells (a coarse copy held as primitives is converted back)
+  double q[7][NV];
+#pragma unroll
+  for (int s = 0; s < 7; ++s) {
+    if (!ok) {
+#pragma unroll
+      for (int v = 0; v < NV; ++v) q[s][v] = nan("");
+      continue;
+    }
+    double u0[NV], u1[NV], u2[NV], t[NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) u0[v] = p.C0[o[s] + v * NC];
+    if (p.c0_prim) { prim_to_cons(u0, igm1, t);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) u0[v] = t[v]; }
+    if (p.interp) {
+#pragma unroll
+      for (int v = 0; v < NV; ++v) { u1[v] = p.C1[o[s] + v * NC]; u2[v] = p.C2[o[s] + v * NC]; }
+      if (p.c1_prim) { prim_to_cons(u1, igm1, t);
+#pragma unroll
+        for (int v = 0; v < NV; ++v) u1[v] = t[v]; }
+#pragma unroll
+      for (int v = 0; v < NV; ++v) q[s][v] = time_interp(u0[v], u1[v], u2[v], p.tau);
+    } else {
+#pragma unroll
+      for (int v = 0; v < NV; ++v) q[s][v] = u0[v];
+    }
+  }
+  double val[NV];
 #pragma unroll
   for (int v = 0; v < NV; ++v) {
-    double q[7];
+    val[v] = q[0][v];
 #pragma unroll
-    for (int s = 0; s < 7; ++s) {
-      if (!ok) { q[s] = nan(""); continue; }
-      const long long a = o[s] + v * NC;
-      q[s] = p.interp ? time_interp(p.C0[a], p.C1[a], p.C2[a], p.tau) : p.C0[a];
-    }
-    double val = q[0];
-#pragma unroll
-    for (int d = 0; d < 3; ++d) val = val + sig[d] * minmod(q[1 + 2 * d] - q[0], q[0] - q[2 + 2 * d]);
-    out[v * NG * FACE] = val;
+    for (int d = 0; d < 3; ++d) val[v] = val[v] + sig[d] * minmod(q[1 + 2 * d][v] - q[0][v], q[0][v] - q[2 + 2 * d][v]);
   }
+  int rout = r;
+  if (p.out_prim) {           // the corrector stages primitives; its z slabs are 128-byte swizzled
+    double w[NV];
+    cons_to_prim(val, gm1, w);
+#pragma unroll
+    for (int v = 0; v < NV; ++v) val[v] = w[v];
+    if (axis == 2) rout = zs_pos(r >> 6, (r >> 3) & 7, r & 7);
+  }
+  double* out = p.ghost + size_t(slot) * SLAB + rout;
+#pragma unroll
+  for (int v = 0; v < NV; ++v) out[v * NG * FACE] = val[v];
 }
 
 cudaError_t launch_prolong(const ProlongParams& p, cudaStream_t st) {
@@ -228,7 +260,7 @@ cudaError_t launch_dt_finalize(const unsigned long long* smax_bits, const LevelI
 // status: cells with rho <= 0, P <= 0 or NaN (reading R28: reported, never floored)
 // =====================================================================================================
 __global__ void __launch_bounds__(256) count_bad_kernel(const double* __restrict__ U, int first, int count, double gamma,
-                                                        unsigned long long* nbad) {
+                                                        int prim, unsigned long long* nbad) {
   const double gm1 = gamma - 1.0;
   unsigned int bad = 0;
   for (int b = blockIdx.x; b < count; b += gridDim.x) {
@@ -237,7 +269,8 @@ __global__ void __launch_bounds__(256) count_bad_kernel(const double* __restrict
       double u[5], w[5];
 #pragma unroll
       for (int v = 0; v < NV; ++v) u[v] = Ub[v * NC + c];
-      cons_to_prim(u, gm1, w);
+      if (prim) { w[0] = u[0]; w[4] = u[4]; }
+      else cons_to_prim(u, gm1, w);
       if (!(w[0] > 0.0) || !(w[4] > 0.0)) ++bad;
     }
   }
@@ -245,16 +278,17 @@ __global__ void __launch_bounds__(256) count_bad_kernel(const double* __restrict
   if ((threadIdx.x & 31) == 0 && bad) atomicAdd(nbad, (unsigned long long)bad);
 }
 
-cudaError_t launch_count_bad(const double* U, int first, int count, double gamma, unsigned long long* nbad,
+cudaError_t launch_count_bad(const double* U, int first, int count, double gamma, int prim, unsigned long long* nbad,
                              cudaStream_t st) {
   if (count <= 0) return cudaSuccess;
   const int grid = count < 148 * 8 ? count : 148 * 8;
-  count_bad_kernel<<<grid, 256, 0, st>>>(U, first, count, gamma, nbad);
+  count_bad_kernel<<<grid, 256, 0, st>>>(U, first, count, gamma, prim, nbad);
   return cudaGetLastError();
 }
 
 // =====================================================================================================
-// caller layout <-> internal layout (block permutation only; both are interior-only [5][8][8][8])
+// caller layout <-> internal layout: block permutation (both are interior-only [5][8][8][8]); role 1 is
+// held as primitives internally, so its copies convert on the way in and out.
 // =====================================================================================================
 __global__ void __launch_bounds__(256) permute_kernel(const double2* __restrict__ src, double2* __restrict__ dst,
                                                       const int64_t* __restrict__ perm, int first, int to_internal) {
@@ -265,11 +299,31 @@ __global__ void __launch_bounds__(256) permute_kernel(const double2* __restrict_
   for (int t = threadIdx.x; t < BLK / 2; t += 256) to[t] = from[t];
 }
 
+__global__ void __launch_bounds__(256) permute_prim_kernel(const double* __restrict__ src, double* __restrict__ dst,
+                                                           const int64_t* __restrict__ perm, int first, int to_internal,
+                                                           double gamma) {
+  const int s = first + blockIdx.x;
+  const size_t a = size_t(s) * BLK, b = size_t(perm[s]) * BLK;
+  const double* from = src + (to_internal ? b : a);
+  double* to = dst + (to_internal ? a : b);
+  const double gm1 = gamma - 1.0, igm1 = 1.0 / gm1;
+  for (int c = threadIdx.x; c < NC; c += 256) {
+    double x[NV], y[NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) x[v] = from[v * NC + c];
+    if (to_internal) cons_to_prim(x, gm1, y);
+    else prim_to_cons(x, igm1, y);
+#pragma unroll
+    for (int v = 0; v < NV; ++v) to[v * NC + c] = y[v];
+  }
+}
+
 cudaError_t launch_permute(const double* src, double* dst, const int64_t* perm, int first, int count, int to_internal,
-                           cudaStream_t st) {
+                           int prim, double gamma, cudaStream_t st) {
   if (count <= 0) return cudaSuccess;
-  permute_kernel<<<count, 256, 0, st>>>(reinterpret_cast<const double2*>(src), reinterpret_cast<double2*>(dst), perm,
-                                        first, to_internal);
+  if (prim) permute_prim_kernel<<<count, 256, 0, st>>>(src, dst, perm, first, to_internal, gamma);
+  else permute_kernel<<<count, 256, 0, st>>>(reinterpret_cast<const double2*>(src), reinterpret_cast<double2*>(dst), perm,
+                                             first, to_internal);
   return cudaGetLastError();
 }
 
@@ -278,43 +332,54 @@ cudaError_t launch_permute(const double* src, double* dst, const int64_t* perm, 
 // =====================================================================================================
 __global__ void __launch_bounds__(256) ghosted_kernel(const double* __restrict__ U, const double* __restrict__ ghost,
                                                       const int32_t* __restrict__ face_src,
-                                                      const int64_t* __restrict__ perm, int first,
-                                                      double* __restrict__ G) {
+                                                      const int64_t* __restrict__ perm, int first, int prim,
+                                                      double gamma, double* __restrict__ G) {
   constexpr int M = N + 2 * NG;
   const int s = first + blockIdx.x;
   double* out = G + size_t(perm[s]) * NV * M * M * M;
-  for (int t = threadIdx.x; t < NV * M * M * M; t += 256) {
-    const int v = t / (M * M * M), c = t % (M * M * M);
+  const double igm1 = 1.0 / (gamma - 1.0);
+  for (int c = threadIdx.x; c < M * M * M; c += 256) {
     const int i = c % M - NG, j = (c / M) % M - NG, k = c / (M * M) - NG;
     const int o[3] = {i < 0 ? -1 : i >= N ? 1 : 0, j < 0 ? -1 : j >= N ? 1 : 0, k < 0 ? -1 : k >= N ? 1 : 0};
     const int nout = (o[0] != 0) + (o[1] != 0) + (o[2] != 0);
-    double val;
-    if (nout == 0) val = U[size_t(s) * BLK + v * NC + (k * 8 + j) * 8 + i];
-    else if (nout > 1) val = nan("");
-    else {
+    const double* from = nullptr;   // variable 0 of the source cell
+    int vs = NC;
+    if (nout == 0) from = U + size_t(s) * BLK + (k * 8 + j) * 8 + i;
+    else if (nout == 1) {
       const int axis = o[0] ? 0 : o[1] ? 1 : 2, side = o[axis] > 0;
       const int src = face_src[s * 6 + 2 * axis + side];
       int q[3] = {i, j, k};
       if (src == SRC_OUTFLOW) {
         q[axis] = side ? N - 1 : 0;
-        val = U[size_t(s) * BLK + v * NC + (q[2] * 8 + q[1]) * 8 + q[0]];
+        from = U + size_t(s) * BLK + (q[2] * 8 + q[1]) * 8 + q[0];
       } else if (src >= 0) {
         q[axis] += side ? -N : N;
-        val = U[size_t(src) * BLK + v * NC + (q[2] * 8 + q[1]) * 8 + q[0]];
+        from = U + size_t(src) * BLK + (q[2] * 8 + q[1]) * 8 + q[0];
       } else {
         const int ll = side ? q[axis] - N : q[axis] + NG;
-        const int r = axis == 0 ? (k * 8 + j) * 2 + ll : axis == 1 ? (k * 2 + ll) * 8 + i : (ll * 8 + j) * 8 + i;
-        val = ghost[size_t(-2 - src) * SLAB + v * NG * FACE + r];
+        const int r = axis == 0 ? (k * 8 + j) * 2 + ll : axis == 1 ? (k * 2 + ll) * 8 + i
+                      : prim ? zs_pos(ll, j, i) : (ll * 8 + j) * 8 + i;
+        from = ghost + size_t(-2 - src) * SLAB + r;
+        vs = NG * FACE;
       }
     }
-    out[t] = val;
+    double x[NV], y[NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) x[v] = from ? from[v * vs] : nan("");
+    if (prim && from) prim_to_cons(x, igm1, y);
+    else {
+#pragma unroll
+      for (int v = 0; v < NV; ++v) y[v] = x[v];
+    }
+#pragma unroll
+    for (int v = 0; v < NV; ++v) out[v * M * M * M + c] = y[v];
   }
 }
 
 cudaError_t launch_ghosted(const double* U, const double* ghost, const int32_t* face_src, const int64_t* perm, int first,
-                           int count, double* G, cudaStream_t st) {
+                           int count, int prim, double gamma, double* G, cudaStream_t st) {
   if (count <= 0) return cudaSuccess;
-  ghosted_kernel<<<count, 256, 0, st>>>(U, ghost, face_src, perm, first, G);
+  ghosted_kernel<<<count, 256, 0, st>>>(U, ghost, face_src, perm, first, prim, gamma, G);
   return cudaGetLastError();
 }
 

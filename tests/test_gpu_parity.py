@@ -138,14 +138,21 @@ def test_ghost_fill_parity(name, interp):
         Gg = g.get_ghosted(which).cpu().numpy()
         fm = face_mask()
         assert np.isnan(Gg[:, :, ghost_count() >= 2]).all()      # edge/corner ghosts: no stage reads them
-        assert np.array_equal(Gg[:, :, 2:10, 2:10, 2:10], Go[:, :, 2:10, 2:10, 2:10])
         a, b = Gg[:, :, fm], Go[:, :, fm]
         assert np.isfinite(a).all()
         scale = np.abs(b).max(axis=(0, 2))[None, :, None]
         # prolongation (and eq. 16) is ~10-20 roundings; FMA contraction may move each by an ulp
         assert (np.abs(a - b) <= 4e-15 * scale).all(), np.abs((a - b) / scale).max()
-        if p.max_level == 0:
-            assert np.array_equal(a, b)          # pure copies
+        ai, bi = Gg[:, :, 2:10, 2:10, 2:10], Go[:, :, 2:10, 2:10, 2:10]
+        if which == 0:
+            assert np.array_equal(ai, bi)
+            if p.max_level == 0:
+                assert np.array_equal(a, b)      # pure copies
+        else:
+            # the library holds the half-step state as primitives: a value set
+            # and read back passes cons -> prim -> cons, a few roundings, instead of a copy
+            si = np.abs(bi).max(axis=(0, 2, 3, 4))[None, :, None, None, None]
+            assert (np.abs(ai - bi) <= 4e-15 * si).all(), np.abs((ai - bi) / si).max()
 
 
 # ------------------------------------------------------------------ the five calls, driven step by step
