@@ -28,7 +28,7 @@ CORRECTOR_BYTES_PER_CELL = 120.0   # read U^n, U^{n+1/2}, w
 PREDICTOR_BYTES_PER_CELL = 80.0    # read U^n, write U^{n+1/2}
 # dram__bytes_read.sum + dram__bytes_write.sum of one corrector launch on C2, from the ncu --set full
 # capture summarised in profiles/ (None until captured)
-CORRECTOR_TRAFFIC_BYTES_C2 = None
+CORRECTOR_TRAFFIC_BYTES_C2 = 1.551233e9 + 0.649253e9   # profiles/r1_c2_ncu.md
 
 
 def parse():
@@ -53,49 +53,82 @@ def peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks and throttle reasons during the timed region."""
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
-         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
-         "clocks_event_reasons.sw_power_cap")
+    """SM clock and throttle reasons during the timed region.  NVML is polled from a thread every
+    few ms (the timed region of the default run lasts tens of ms, shorter than one `nvidia-smi -lms`
+    period); `nvidia-smi` is the fallback when the NVML binding is missing."""
+    REASONS = (("hw_slowdown", 0x8), ("hw_thermal_slowdown", 0x40), ("sw_thermal_slowdown", 0x20),
+               ("sw_power_cap", 0x4))
 
     def __init__(self, index):
-        self.lines = []
-        self.proc = None
+        self.rows = []          # (time, sm_mhz, reasons bitmask, power W)
+        self.max_mhz = None
+        self.stop_flag = False
+        self.th = None
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
-                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
-            self.th = threading.Thread(target=self._read, daemon=True)
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self._sample()
+            self.th = threading.Thread(target=self._poll, daemon=True)
             self.th.start()
         except Exception:
-            self.proc = None
+            self.nv = None
+            self._smi(index)
 
-    def _read(self):
-        for line in self.proc.stdout:
-            self.lines.append((time.time(), line.strip()))
+    def _sample(self):
+        nv = self.nv
+        mhz = float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+        try:
+            why = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+        except Exception:
+            why = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+        try:
+            watts = nv.nvmlDeviceGetPowerUsage(self.h) / 1e3
+        except Exception:
+            watts = 0.0
+        self.rows.append((time.time(), mhz, why, watts))
+
+    def _poll(self):
+        while not self.stop_flag:
+            try:
+                self._sample()
+            except Exception:
+                break
+            time.sleep(0.002)
+
+    def _smi(self, index):
+        q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+        try:
+            res = subprocess.run(["nvidia-smi", "-i", str(index), "--query-gpu=" + q, "--format=csv,noheader,nounits"],
+                                 capture_output=True, text=True, timeout=20)
+            r = res.stdout.strip().split(", ")
+            self.max_mhz = float(r[1])
+            why = sum(bit for (_, bit), x in zip(self.REASONS, r[3:7]) if x.strip().lower() == "active")
+            self.rows.append((time.time(), float(r[0]), why, float(r[2])))
+        except Exception:
+            pass
 
     def stop(self, t0, t1):
-        if self.proc is None:
-            return None
-        time.sleep(0.15)
-        self.proc.terminate()
-        try:
-            self.proc.wait(timeout=5)
-        except Exception:
-            self.proc.kill()
-        rows = [l.split(", ") for t, l in self.lines if t0 - 0.05 <= t <= t1 + 0.15]
+        self.stop_flag = True
+        if self.th is not None:
+            self.th.join(timeout=2)
+        rows = [r for r in self.rows if t0 <= r[0] <= t1]
+        where = "timed region"
         if not rows:
-            rows = [l.split(", ") for _, l in self.lines]
+            rows, where = self.rows, "around the timed region"
         if not rows:
             return None
-        try:
-            sm = sorted(float(r[0]) for r in rows)
-            names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-            reasons = [n for i, n in enumerate(names) if any(r[3 + i].strip().lower() == "active" for r in rows)]
-            return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(rows[0][1]), "reasons": reasons,
-                    "samples": len(rows), "power_w_max": max(float(r[2]) for r in rows)}
-        except Exception:
-            return None
+        sm = sorted(r[1] for r in rows)
+        mask = 0
+        for r in rows:
+            mask |= r[2]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": self.max_mhz, "sm_mhz_min": sm[0],
+                "reasons": [n for n, bit in self.REASONS if mask & bit], "samples": len(rows), "window": where,
+                "power_w_max": max(r[3] for r in rows), "source": "nvml" if self.nv else "nvidia-smi"}
 
 
 def cell_updates(census, nupd):
@@ -240,7 +273,7 @@ def main():
     c_ms, c_n = kt["corrector"]
     corr_bytes = CORRECTOR_BYTES_PER_CELL * cu            # every cell-update passes the corrector once
     achieved = corr_bytes / (c_ms * 1e-3) / 1e9 if c_ms > 0 else 0.0
-    roofline = {"bound": "hbm", "kernel": "stage_kernel<1> (corrector)", "achieved": achieved, "peak": peak,
+    roofline = {"bound": "hbm", "kernel": "corrector_kernel", "achieved": achieved, "peak": peak,
                 "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
                 "traffic": CORRECTOR_TRAFFIC_BYTES_C2 if (args.config == "C2" and args.scale == 1) else None,
                 "algorithmic_bytes_per_launch": corr_bytes / max(c_n, 1), "launches": c_n,
