@@ -76,41 +76,50 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-// Tensor maps of one state buffer seen as a 4-D fp64 tensor [5*nb][8][8][8] (innermost = x); one map
-// per face axis, whose box is the two-layer slab {2,8,8,5}, {8,2,8,5} or {8,8,2,5}.
+// Tensor maps of one state buffer seen as a 4-D fp64 tensor [5*nb][8][8][8] (innermost = x): the
+// two-layer x-face slab {2,8,8,5}; the two-layer y-face slab over the view with j and k exchanged
+// (dimensions (i, k, j, var), box {8,8,2,5}) so that it lands as [var][ll][k][i]; and the z-plane pair.
 int make_tensor_maps(void* base, int64_t nb, TensorMaps& out) {
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
   CU(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres), "cudaGetDriverEntryPoint");
   if (!fn || qres != cudaDriverEntryPointSuccess) return fail(SFH_ECUDA, "cuTensorMapEncodeTiled not available");
   EncodeTiledFn encode = reinterpret_cast<EncodeTiledFn>(fn);
-  const cuuint64_t dims[4] = {N, N, N, cuuint64_t(NV) * cuuint64_t(nb)};
-  const cuuint64_t strides[3] = {N * 8, N * N * 8, N * N * N * 8};
+  const cuuint64_t nvb = cuuint64_t(NV) * cuuint64_t(nb);
   const cuuint32_t estr[4] = {1, 1, 1, 1};
-  for (int axis = 0; axis < 4; ++axis) {      // 3 = the swizzled z-plane-pair map
-    CUresult r;
-    if (axis < 3) {
-      cuuint32_t box[4] = {N, N, N, NV};
-      box[axis] = NG;
-      r = encode(&out.ax[axis], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, estr,
-                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
-                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    } else {
-      // 128-byte swizzle wants 128-byte rows (a 64-byte inner box would be padded to 128-byte lines,
-      // measured): view two consecutive x rows (j, j+1) as one row of 16 doubles -> [5 nb][8][4][16]
-      const cuuint64_t dims2[4] = {2 * N, N / 2, N, cuuint64_t(NV) * cuuint64_t(nb)};
-      const cuuint64_t strides2[3] = {2 * N * 8, N * N * 8, N * N * N * 8};
-      const cuuint32_t box2[4] = {2 * N, N / 2, NG, NV};
-      r = encode(&out.zs, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims2, strides2, box2, estr,
-                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
-                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    }
-    if (r != CUDA_SUCCESS) {
+  CUresult r[3];
+  {
+    const cuuint64_t dims[4] = {N, N, N, nvb};
+    const cuuint64_t strides[3] = {N * 8, N * N * 8, N * N * N * 8};
+    const cuuint32_t box[4] = {NG, N, N, NV};
+    r[0] = encode(&out.ax, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, estr,
+                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  }
+  {
+    const cuuint64_t dims[4] = {N, N, N, nvb};                        // (i, k, j, var)
+    const cuuint64_t strides[3] = {N * N * 8, N * 8, N * N * N * 8};  // of k, j, var
+    const cuuint32_t box[4] = {N, N, NG, NV};
+    r[1] = encode(&out.ay, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, estr,
+                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  }
+  {
+    // 128-byte swizzle wants 128-byte rows (a 64-byte inner box would be padded to 128-byte lines,
+    // measured): view two consecutive x rows (j, j+1) as one row of 16 doubles -> [5 nb][8][4][16]
+    const cuuint64_t dims2[4] = {2 * N, N / 2, N, nvb};
+    const cuuint64_t strides2[3] = {2 * N * 8, N * N * 8, N * N * N * 8};
+    const cuuint32_t box2[4] = {2 * N, N / 2, NG, NV};
+    r[2] = encode(&out.zs, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims2, strides2, box2, estr,
+                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  }
+  for (int q = 0; q < 3; ++q)
+    if (r[q] != CUDA_SUCCESS) {
       char buf[96];
-      snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled failed (CUresult %d)", int(r));
+      snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled failed (map %d, CUresult %d)", q, int(r[q]));
       return fail(SFH_ECUDA, buf);
     }
-  }
   return SFH_OK;
 }
 

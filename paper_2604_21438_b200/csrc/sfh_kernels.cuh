@@ -26,14 +26,23 @@ struct StageParams {
 };
 
 struct TensorMaps {      // tensor maps of ONE state buffer seen as [5 nb][8][8][8]
-  CUtensorMap ax[3];     // one per face axis, box = the 2-layer slab {2,8,8,5} / {8,2,8,5} / {8,8,2,5}, dense in smem
+  CUtensorMap ax;        // x-face slab: box {2,8,8,5} over (i, j, k, var), dense in smem: [var][k][j][ll]
+  CUtensorMap ay;        // y-face slab: box {8,8,2,5} over the PERMUTED view (i, k, j, var), dense: [var][ll][k][i]
   CUtensorMap zs;        // box {8,8,2,5} (a pair of z planes of all 5 variables), 128-byte swizzled in smem
 };
+
+// Positions inside a coarse-fine ghost slab [var][128] (variable stride 128) = the staging layout of
+// the stage kernels (sfh_kernels.cu): ll = layer (index increasing with the coordinate), (ta, tb) = the
+// two in-face coordinates, lower axis first.
+__host__ __device__ inline int slab_pos(int axis, int ll, int ta, int tb);
 
 // Position of cell (kl, j, i) of a z-plane pair inside a 128-byte-swizzled slab [v][kl][j][i] of fp64
 // (variable stride 128): the TMA swizzle XORs byte-address bits [4,7) with bits [7,10), i.e. the
 // 16-byte chunk (i >> 1, j & 1) with (j >> 1, kl).
 __host__ __device__ inline int zs_pos(int kl, int j, int i) { return (kl << 6) | ((j ^ kl) << 3) | (i ^ (j & 6)); }
+__host__ __device__ inline int slab_pos(int axis, int ll, int ta, int tb) {
+  return axis == 0 ? (tb * 8 + ta) * 2 + ll : axis == 1 ? ll * 64 + tb * 8 + ta : zs_pos(ll, tb, ta);
+}
 
 struct ProlongParams {
   const double* C0;      // coarse level: role `which` (interp = 0) or role 0 (interp = 1)
@@ -49,7 +58,7 @@ struct ProlongParams {
   int interp;
   double tau;
   int c0_prim, c1_prim;  // the coarse copy C0 / C1 holds primitives (the half-step state)
-  int out_prim;          // write primitives, z-face slabs in the swizzled order of zs_pos (half-step fill)
+  int out_prim;          // write primitives (half-step fill)
   double gamma;
 };
 

@@ -100,14 +100,15 @@ __global__ void __launch_bounds__(128) prolong_kernel(const ProlongParams p) {
 #pragma unroll
     for (int d = 0; d < 3; ++d) val[v] = val[v] + sig[d] * minmod(q[1 + 2 * d][v] - q[0][v], q[0][v] - q[2 + 2 * d][v]);
   }
-  int rout = r;
-  if (p.out_prim) {           // the corrector stages primitives; its z slabs are 128-byte swizzled
+  if (p.out_prim) {           // the corrector stages primitives
     double w[NV];
     cons_to_prim(val, gm1, w);
 #pragma unroll
     for (int v = 0; v < NV; ++v) val[v] = w[v];
-    if (axis == 2) rout = zs_pos(r >> 6, (r >> 3) & 7, r & 7);
   }
+  // the slab is written in the staging layout of the stage kernels
+  const int ll = fc[axis] < 0 ? fc[axis] + NG : fc[axis] - N;
+  const int rout = slab_pos(axis, ll, fc[axis == 0 ? 1 : 0], fc[axis == 2 ? 1 : 2]);
   double* out = p.ghost + size_t(slot) * SLAB + rout;
 #pragma unroll
   for (int v = 0; v < NV; ++v) out[v * NG * FACE] = val[v];
@@ -357,8 +358,7 @@ __global__ void __launch_bounds__(256) ghosted_kernel(const double* __restrict__
         from = U + size_t(src) * BLK + (q[2] * 8 + q[1]) * 8 + q[0];
       } else {
         const int ll = side ? q[axis] - N : q[axis] + NG;
-        const int r = axis == 0 ? (k * 8 + j) * 2 + ll : axis == 1 ? (k * 2 + ll) * 8 + i
-                      : prim ? zs_pos(ll, j, i) : (ll * 8 + j) * 8 + i;
+        const int r = slab_pos(axis, ll, axis == 0 ? j : i, axis == 2 ? j : k);
         from = ghost + size_t(-2 - src) * SLAB + r;
         vs = NG * FACE;
       }
