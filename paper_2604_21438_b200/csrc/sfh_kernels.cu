@@ -285,7 +285,10 @@ __device__ __forceinline__ void issue_loads(const TensorMaps& tm, const StagePar
 }
 
 // staged conserved cells -> primitives + c_s + E, in place (predictor): the 512 interior cells and the
-// ONE halo layer next to each face (the predictor is first order) = 896 cells, 7 per helper thread.
+// ONE halo layer next to each face (the predictor is first order) = 896 cells.  The WALKERS convert the
+// next block between two walks (12 warps finish it in a fraction of the time the 4 helper warps need,
+// and the helpers' chain staging -> conversion -> ready was what the walkers waited for): walker thread
+// t converts items t, t + 384 and (t < 128) t + 768 of the list [512 interior | z | x | y halo layers].
 __device__ __forceinline__ void convert_cell(double* __restrict__ c, double gamma, double gm1) {
   double u[5], w[5];
 #pragma unroll
@@ -297,17 +300,30 @@ __device__ __forceinline__ void convert_cell(double* __restrict__ c, double gamm
   c[5 * CVS] = c2 * rsqrt_fast(c2);
   c[6 * CVS] = u[4];                                       // total energy of the cell (eq. 8)
 }
-__device__ __forceinline__ void convert_staged(double* __restrict__ L, const int* __restrict__ fsrc, double gamma,
-                                               double gm1, int hid) {
+// halo item h in [0, 384): group g = h >> 7 (z, x, y), side = bit 6, x = h & 63.
+//   z: tile 0 layer kl = 1 (positions 64..127) / tile 5 layer kl = 0;  x: tile 6 odd positions (ll = 1) /
+//   tile 7 even positions;  y: tile 8 layer ll = 1 (positions 64..127) / tile 9 layer ll = 0
+__device__ __forceinline__ void convert_halo_item(double* __restrict__ L, const int* __restrict__ fsrc, int h,
+                                                  double gamma, double gm1) {
   constexpr int TS = Cfg<0>::TS;
-#pragma unroll
-  for (int r = 0; r < 4; ++r) convert_cell(L + (1 + r) * TS + hid, gamma, gm1);
-  const int x = hid & 63, hi = hid >> 6;                   // hi: warp-uniform
-  // z: tile 0 layer kl = 1 (positions 64..127) / tile 5 layer kl = 0;  x: tile 6 odd positions (ll = 1) /
-  // tile 7 even positions;  y: tile 8 layer ll = 1 (positions 64..127) / tile 9 layer ll = 0
-  if (fsrc[4 + hi] != SRC_OUTFLOW) convert_cell(L + (hi ? 5 * TS : 0) + (hi ? x : 64 + x), gamma, gm1);
-  if (fsrc[0 + hi] != SRC_OUTFLOW) convert_cell(L + (T_XLO + hi) * TS + 2 * x + (hi ? 0 : 1), gamma, gm1);
-  if (fsrc[2 + hi] != SRC_OUTFLOW) convert_cell(L + (T_YLO + hi) * TS + (hi ? x : 64 + x), gamma, gm1);
+  const int g = h >> 7, hi = (h >> 6) & 1, x = h & 63;     // g, hi: warp-uniform
+  const int f = (g == 0 ? 4 : g == 1 ? 0 : 2) + hi;
+  if (fsrc[f] == SRC_OUTFLOW) return;                      // nothing was staged there
+  const int pos = g == 0 ? (hi ? 5 * TS + x : 64 + x)
+                : g == 1 ? (T_XLO + hi) * TS + 2 * x + (hi ? 0 : 1)
+                         : (T_YLO + hi) * TS + (hi ? x : 64 + x);
+  convert_cell(L + pos, gamma, gm1);
+}
+__device__ __forceinline__ void convert_share(double* __restrict__ L, const int* __restrict__ fsrc, double gamma,
+                                              double gm1, int tid) {
+  constexpr int TS = Cfg<0>::TS;
+  convert_cell(L + (1 + (tid >> 7)) * TS + (tid & 127), gamma, gm1);          // interior tiles 1..3
+  if (tid < 128) {
+    convert_cell(L + 4 * TS + tid, gamma, gm1);                                // interior tile 4
+    convert_halo_item(L, fsrc, tid + 256, gamma, gm1);                         // y halos
+  } else {
+    convert_halo_item(L, fsrc, tid - 128, gamma, gm1);                         // z and x halos
+  }
 }
 
 // halo of an outflow face (reading R1): copies of the block's own edge layer
@@ -327,8 +343,6 @@ __device__ __forceinline__ void fill_outflow(double* __restrict__ L, const int* 
     for (int v = 0; v < NVW; ++v) L[dst + v * CVS] = L[src + v * CVS];
   }
 }
-
-__device__ __forceinline__ void helper_sync() { asm volatile("bar.sync 1, %0;" ::"n"(HELP_THREADS) : "memory"); }
 
 // ---- helpers: update -----------------------------------------------------------------------------------
 // U_out = U^n - lambda ((dFx + dFy) + dFz), lambda = dt/(2h) (predictor) or dt/h (corrector).
@@ -365,7 +379,8 @@ __device__ __forceinline__ void update_block(const double* __restrict__ dF, cons
 // ---- the stage kernel ------------------------------------------------------------------------------------
 // CTA c handles blocks c, c + gridDim.x, ... of the level ("iterations" it = 0, 1, ...).  Barriers:
 //   landed[s]  the TMA copies of the block staged in buffer s = it & 1 are complete (transaction count)
-//   ready[s]   the helpers have prepared buffer s (conversion, outflow halos): walkers may read it
+//   conv[s]    predictor: the walkers have converted buffer s to primitives (their share each)
+//   ready[s]   buffer s is prepared (conversion by the walkers, outflow halos by the helpers): walk it
 //   full[d]    all walkers have stored the flux differences into buffer d = it % NDF (and are done with
 //              the staging buffer, which the helpers then re-stage)
 //   empty[d]   the helpers have consumed flux-difference buffer d
@@ -377,12 +392,13 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
   double* L0 = reinterpret_cast<double*>(smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u));
   double* dF0 = L0 + 2 * C::LAND;
   uint64_t* bars = reinterpret_cast<uint64_t*>(dF0 + C::NDF * DF_DOUBLES);
-  int* fsrc0 = reinterpret_cast<int*>(bars + 8);            // [2][8]
+  int* fsrc0 = reinterpret_cast<int*>(bars + 10);           // [2][8]
   const uint32_t bar0 = smem_u32(bars);
   auto landed = [&](int s) { return bar0 + 8u * s; };
   auto ready = [&](int s) { return bar0 + 16u + 8u * s; };
   auto full = [&](int d) { return bar0 + 32u + 8u * d; };
   auto empty = [&](int d) { return bar0 + 48u + 8u * d; };
+  auto conv = [&](int s) { return bar0 + 64u + 8u * s; };   // predictor: the walkers have converted buffer s
 
   const int tid = threadIdx.x;
   const int stride = gridDim.x;
@@ -391,7 +407,8 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
   if (tid == 0) {
     for (int s = 0; s < 2; ++s) {
       mbar_init(landed(s), 1);
-      mbar_init(ready(s), HELP_WARPS);
+      mbar_init(ready(s), STAGE == 0 ? WALK_WARPS + HELP_WARPS : HELP_WARPS);
+      mbar_init(conv(s), WALK_WARPS);
       mbar_init(full(s), WALK_WARPS);
       mbar_init(empty(s), HELP_WARPS);
     }
@@ -405,13 +422,31 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
     // ------------------------------------------------------------------------------ walkers
     const double igm1 = 1.0 / gm1;
     const int D = tid >> 7, f0 = ((tid >> 6) & 1) * 4, pen = tid & 63, a = pen & 7, b = pen >> 3;
+    auto convert_next = [&](int it) {                  // predictor: my share of block it, then both arrivals
+      const int s = it & 1;
+      mbar_wait(landed(s), (it >> 1) & 1);
+      convert_share(L0 + s * C::LAND, fsrc0 + 8 * s, gamma, gm1, tid);
+      fence_proxy_async();                             // my generic-proxy writes, before a later TMA overwrites them
+      __syncwarp();
+      if ((tid & 31) == 0) { mbar_arrive(conv(s)); mbar_arrive(ready(s)); }
+    };
+    if (STAGE == 0) convert_next(0);
+#ifdef SFH_DEBUG_TIMING
+    long long tw[3] = {0, 0, 0}, t0, t1;
+#endif
     for (int it = 0; it < n; ++it) {
       const int s = it & 1, d = it % C::NDF;
+#ifdef SFH_DEBUG_TIMING
+      t0 = clock64();
+#endif
       const double* Wl = L0 + s * C::LAND;
       double* dF = dF0 + d * DF_DOUBLES;
       const bool we = it >= C::NDF;
       const uint32_t pe = ((it / C::NDF) - 1) & 1;
       mbar_wait(ready(s), (it >> 1) & 1);
+#ifdef SFH_DEBUG_TIMING
+      t1 = clock64(); tw[0] += t1 - t0;
+#endif
       if (STAGE == 0) {
         if (D == 0) walk_predictor<0>(Wl, dF, a, b, f0, igm1, empty(d), pe, we);
         else if (D == 1) walk_predictor<1>(Wl, dF, a, b, f0, igm1, empty(d), pe, we);
@@ -424,7 +459,18 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
       }
       __syncwarp();
       if ((tid & 31) == 0) mbar_arrive(full(d));
+#ifdef SFH_DEBUG_TIMING
+      tw[1] += clock64() - t1; t1 = clock64();
+#endif
+      if (STAGE == 0 && it + 1 < n) convert_next(it + 1);
+#ifdef SFH_DEBUG_TIMING
+      tw[2] += clock64() - t1;
+#endif
     }
+#ifdef SFH_DEBUG_TIMING
+    if (blockIdx.x == 5 && (tid & 127) == 0)
+      printf("stage %d walker D=%d n=%d: per block wait_ready %lld  walk(+wait_empty) %lld  convert %lld\n", STAGE, D, n, tw[0] / n, tw[1] / n, tw[2] / n);
+#endif
   } else {
     // ------------------------------------------------------------------------------ helpers
     const int hid = tid - WALK_THREADS, hw = hid >> 5;
@@ -435,14 +481,11 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
       double* L = L0 + s * C::LAND;
       const int* fsrc = fsrc0 + 8 * s;
       mbar_wait(landed(s), (it >> 1) & 1);
-      bool wrote = false;
-      if (STAGE == 0) { convert_staged(L, fsrc, gamma, gm1, hid); wrote = true; }
-      if (fsrc[6]) {                                   // block-uniform
-        if (STAGE == 0) helper_sync();                 // the edge layers are converted
+      if (fsrc[6]) {                                   // block-uniform: some face is an outflow face
+        if (STAGE == 0) mbar_wait(conv(s), (it >> 1) & 1);   // the edge layers are converted
         fill_outflow<STAGE>(L, fsrc, hid);
-        wrote = true;
+        fence_proxy_async();                           // my generic-proxy writes, before a later TMA overwrites them
       }
-      if (wrote) fence_proxy_async();                  // my generic-proxy writes, before a later TMA overwrites them
       __syncwarp();
       if (lane0) mbar_arrive(ready(s));
     };
@@ -463,9 +506,15 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
     }
     __syncwarp();
     for (int it = 0; it < 2 && it < n; ++it) prepare(it);
+#ifdef SFH_DEBUG_TIMING
+    long long th[5] = {0, 0, 0, 0, 0}, t0, t1;
+#endif
     for (int it = 0; it < n; ++it) {
       const int s = it & 1, d = it % C::NDF;
       const int blk = blk0 + it * stride;
+#ifdef SFH_DEBUG_TIMING
+      t0 = clock64();
+#endif
       // U^n of the block and the face sources of the block after next: in flight while the walkers finish
       double un[HC][NV];
       const double* Un = p.Un + size_t(blk) * BLK;
@@ -476,6 +525,9 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
       int snext[6];
       if (lane0 && it + 2 < n) load_src(it + 2, snext);
       mbar_wait(full(d), (it / C::NDF) & 1);
+#ifdef SFH_DEBUG_TIMING
+      t1 = clock64(); th[0] += t1 - t0; t0 = t1;
+#endif
       if (lane0 && it + 2 < n) {                       // the walkers are done with staging buffer s as well
         issue_loads<STAGE>(tm, p, blk + 2 * stride, snext, hw, L0 + s * C::LAND, fsrc0 + 8 * s, landed(s));
         if (hw == 3 && it + 3 < n) {
@@ -484,11 +536,27 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
         }
       }
       __syncwarp();
+#ifdef SFH_DEBUG_TIMING
+      t1 = clock64(); th[1] += t1 - t0; t0 = t1;
+#endif
       update_block<STAGE == 0>(dF0 + d * DF_DOUBLES, un, lam, gm1, p.Udst + size_t(blk) * BLK, hid);
       __syncwarp();
       if (lane0) mbar_arrive(empty(d));
+#ifdef SFH_DEBUG_TIMING
+      t1 = clock64(); th[2] += t1 - t0; t0 = t1;
+      if (it + 2 < n) mbar_wait(landed(s), ((it + 2) >> 1) & 1);
+      t1 = clock64(); th[3] += t1 - t0; t0 = t1;
+#endif
       if (it + 2 < n) prepare(it + 2);
+#ifdef SFH_DEBUG_TIMING
+      t1 = clock64(); th[4] += t1 - t0;
+#endif
     }
+#ifdef SFH_DEBUG_TIMING
+    if (blockIdx.x == 5 && lane0)
+      printf("stage %d helper warp %d n=%d: per block wait_full %lld  issue %lld  update %lld  wait_landed %lld  prepare %lld\n",
+             STAGE, hw, n, th[0] / n, th[1] / n, th[2] / n, th[3] / n, th[4] / n);
+#endif
   }
 }
 
