@@ -161,8 +161,8 @@ __device__ __forceinline__ void hllc_flux(double rL, double uL, double vL, doubl
   const double d = Ss - u, g = d * inv, rd = r * d, A = rd * inv, rdS = rd * Ss;
   Fn[0] = fma(s, A, ru);
   Fn[1] = fma(s, fma(A, Ss, rd), fma(ru, u, P));
-  Fn[2] = fma(s, A * v, ru * v);
-  Fn[3] = fma(s, A * w, ru * w);
+  Fn[2] = Fn[0] * v;                         // tangential momenta are carried by the mass flux
+  Fn[3] = Fn[0] * w;
   Fn[4] = fma(s, fma(g, EP + rdS, rdS), u * EP);
 }
 

@@ -33,7 +33,9 @@ namespace sfh {
 
 constexpr int WALK_WARPS = 12, HELP_WARPS = 4;
 constexpr int WALK_THREADS = 32 * WALK_WARPS, HELP_THREADS = 32 * HELP_WARPS;
-constexpr int STAGE_THREADS = WALK_THREADS + HELP_THREADS;   // 512
+constexpr int STAGE_THREADS = WALK_THREADS + HELP_THREADS;   // 512, launched with 128 registers each
+constexpr int WALK_REGS = 144, HELP_REGS = 80;               // corrector, after setmaxnreg
+static_assert(WALK_THREADS * WALK_REGS + HELP_THREADS * HELP_REGS <= 65536, "register file of one SM");
 constexpr int CVS = NG * FACE;                // variable stride of every tile (128 cells)
 constexpr int NTILE = 10;
 constexpr int T_XLO = 6, T_XHI = 7, T_YLO = 8, T_YHI = 9;
@@ -154,7 +156,7 @@ __device__ __forceinline__ void walk_predictor(const double* __restrict__ Wl, do
   hllc_flux<true>(w0[0], w0[1], w0[2], w0[3], w0[4], w0[5], w0[6], w1[0], w1[1], w1[2], w1[3], w1[4], w1[5], w1[6],
                   igm1, F0);                        // face f0
   if (wait_empty) mbar_wait(bar_empty, par_empty);  // the update of the block before has read dF
-#pragma unroll 1
+#pragma unroll
   for (int f = f0 + 1; f < f0 + 4; f += 2) {        // faces f (cells f-1 | f) and f+1 (cells f | f+1)
     if (D == 0) {
 #pragma unroll
@@ -218,7 +220,7 @@ __device__ __forceinline__ void walk_corrector(const double* __restrict__ Wl, do
   if (wait_empty) mbar_wait(bar_empty, par_empty);            // the update two blocks back has read this dF buffer
   // invariant at the top of a trip (f = f0+1, f0+3): wb = W_f, da = W_f - W_{f-1}, Lb = left state of
   // face f, F0 = flux of face f-1
-#pragma unroll 1
+#pragma unroll 1     // (unrolled, the three direction instantiations no longer fit the instruction cache)
   for (int f = f0 + 1; f < f0 + 4; f += 2) {
     load_two<1, D>(Wl, f + 1, a, b, wa, wc);                  // cells f+1, f+2
 #pragma unroll
@@ -420,6 +422,8 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
 
   if (tid < WALK_THREADS) {
     // ------------------------------------------------------------------------------ walkers
+    // corrector: the helpers' update needs few registers; the walkers take what they release
+    if (STAGE == 1) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(WALK_REGS));
     const double igm1 = 1.0 / gm1;
     const int D = tid >> 7, f0 = ((tid >> 6) & 1) * 4, pen = tid & 63, a = pen & 7, b = pen >> 3;
     auto convert_next = [&](int it) {                  // predictor: my share of block it, then both arrivals
@@ -473,6 +477,7 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
 #endif
   } else {
     // ------------------------------------------------------------------------------ helpers
+    if (STAGE == 1) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(HELP_REGS));
     const int hid = tid - WALK_THREADS, hw = hid >> 5;
     const bool lane0 = (tid & 31) == 0;
     const double lam = (STAGE == 0 ? 0.5 : 1.0) * dt / p.h;
