@@ -198,44 +198,62 @@ __device__ __forceinline__ void corrector_flux(const double WLs[5], const double
                    igm1, Fn);
 }
 
-template <int D>
-__device__ __forceinline__ void walk_corrector(const double* __restrict__ Wl, double* __restrict__ dF, int a, int b,
-                                               int f0, double gamma, double igm1, const StageParams& p, int blk,
-                                               double dt, uint32_t bar_empty, uint32_t par_empty, bool wait_empty) {
-  double wa[5], wb[5], wc[5], da[5], db[5], La[5], Lb[5], R[5], F0[5], F1[5];
-  // cells f0-2, f0-1, f0, f0+1: slope of cell f0-1 -> left state of face f0; slope of cell f0 -> right state
-  load_two<1, D>(Wl, f0 - 2, a, b, wa, wb);
+// ---- direction-generic corrector walk ------------------------------------------------------------------
+// The corrector walk with every direction-dependent quantity (the positions of the thread's 8 cells in the
+// landing layout, the variable offsets of the face frame, the positions of its 4 flux differences) held
+// in registers, so that the twelve walker warps run ONE straight-line body: a third of the instruction
+// footprint of three direction instantiations, and no loop-carried register rotation.
+struct WalkGeom {
+  int cp[8];     // cells f0-2 .. f0+5 of the half pencil
+  int ov[3];     // offsets of the normal and the two tangential velocities
+  int di[4];     // flux-difference positions of cells f0 .. f0+3
+};
+template <int STAGE, int D>
+__device__ __forceinline__ void walk_geom(int a, int b, int f0, WalkGeom& g) {
+  constexpr int TS = Cfg<STAGE>::TS;
 #pragma unroll
-  for (int v = 0; v < 5; ++v) da[v] = wb[v] - wa[v];          // W_{f0-1} - W_{f0-2}
-  load_two<1, D>(Wl, f0, a, b, wa, wc);                       // wa = W_f0, wc = W_{f0+1}
+  for (int cc = 0; cc < 8; ++cc) g.cp[cc] = cell_pos<TS, D>(f0 - 2 + cc, a, b);
+  g.ov[0] = (1 + D) * CVS; g.ov[1] = (1 + (D + 1) % 3) * CVS; g.ov[2] = (1 + (D + 2) % 3) * CVS;
 #pragma unroll
-  for (int v = 0; v < 5; ++v) db[v] = wa[v] - wb[v];          // W_f0 - W_{f0-1}
-  limited_states(wb, db, da, R, La);                          // La = left state of face f0
+  for (int cc = 0; cc < 4; ++cc)
+    g.di[cc] = D == 0 ? dfx_idx(f0 + cc, a, b) : D == 1 ? dfy_idx(a, f0 + cc, b) : dfz_idx(a, b, f0 + cc);
+}
+__device__ __forceinline__ void load_cell_g(const double* __restrict__ Wl, int o, const int ov[3], double w[5]) {
+  w[0] = Wl[o]; w[1] = Wl[o + ov[0]]; w[2] = Wl[o + ov[1]]; w[3] = Wl[o + ov[2]]; w[4] = Wl[o + 4 * CVS];
+}
+__device__ __forceinline__ void walk_corrector_generic(const double* __restrict__ Wl, double* __restrict__ dF,
+                                                       const WalkGeom& g, int D, int a, int b, int f0, double gamma,
+                                                       double igm1, const StageParams& p, int blk, double dt,
+                                                       uint32_t bar_empty, uint32_t par_empty, bool wait_empty) {
+  double wp[5], wc[5], wn[5], dp[5], dn[5], L[5], Ln[5], R[5], Fa[5], Fb[5];
+  load_cell_g(Wl, g.cp[0], g.ov, wp);
+  load_cell_g(Wl, g.cp[1], g.ov, wc);
+  load_cell_g(Wl, g.cp[2], g.ov, wn);
 #pragma unroll
-  for (int v = 0; v < 5; ++v) { wb[v] = wc[v]; da[v] = wb[v] - wa[v]; }   // wb = W_{f0+1}
-  limited_states(wa, da, db, R, Lb);                          // R = right state of face f0, Lb = left of face f0+1
-  corrector_flux(La, R, gamma, igm1, F0);
-  if (p.use_regs && f0 == 0)
-    store_regs(p.face_src, p.fslot, p.R, p.FH, blk, D, 0, b * 8 + a, F0[0], F0[1], F0[2], F0[3], F0[4], dt);
-  if (wait_empty) mbar_wait(bar_empty, par_empty);            // the update two blocks back has read this dF buffer
-  // invariant at the top of a trip (f = f0+1, f0+3): wb = W_f, da = W_f - W_{f-1}, Lb = left state of
-  // face f, F0 = flux of face f-1
-#pragma unroll 1     // (unrolled, the three direction instantiations no longer fit the instruction cache)
-  for (int f = f0 + 1; f < f0 + 4; f += 2) {
-    load_two<1, D>(Wl, f + 1, a, b, wa, wc);                  // cells f+1, f+2
+  for (int v = 0; v < 5; ++v) { dp[v] = wc[v] - wp[v]; dn[v] = wn[v] - wc[v]; }
+  limited_states(wc, dn, dp, R, L);                           // L = left state of face f0
 #pragma unroll
-    for (int v = 0; v < 5; ++v) db[v] = wa[v] - wb[v];
-    limited_states(wb, db, da, R, La);                        // right state of face f, left of face f+1
-    corrector_flux(Lb, R, gamma, igm1, F1);                   // face f
-    store_df<D>(dF, f - 1, a, b, F1, F0);
+  for (int ff = 0; ff < 5; ++ff) {                            // face f0+ff, between cells cc = ff+1 and ff+2
 #pragma unroll
-    for (int v = 0; v < 5; ++v) { wb[v] = wc[v]; da[v] = wb[v] - wa[v]; }
-    limited_states(wa, da, db, R, Lb);                        // right state of face f+1, left of face f+2
-    corrector_flux(La, R, gamma, igm1, F0);                   // face f+1
-    store_df<D>(dF, f, a, b, F0, F1);
+    for (int v = 0; v < 5; ++v) { wc[v] = wn[v]; dp[v] = dn[v]; }
+    load_cell_g(Wl, g.cp[ff + 3], g.ov, wn);
+#pragma unroll
+    for (int v = 0; v < 5; ++v) dn[v] = wn[v] - wc[v];
+    limited_states(wc, dn, dp, R, Ln);                        // right state of this face, left state of the next
+    corrector_flux(L, R, gamma, igm1, (ff & 1) ? Fb : Fa);
+#pragma unroll
+    for (int v = 0; v < 5; ++v) L[v] = Ln[v];
+    if (ff == 0) {
+      if (p.use_regs && f0 == 0)
+        store_regs(p.face_src, p.fslot, p.R, p.FH, blk, D, 0, b * 8 + a, Fa[0], Fa[1], Fa[2], Fa[3], Fa[4], dt);
+      if (wait_empty) mbar_wait(bar_empty, par_empty);        // the update two blocks back has read this dF buffer
+    } else {
+#pragma unroll
+      for (int q = 0; q < 5; ++q) dF[g.di[ff - 1] + q * NC] = (ff & 1) ? Fb[q] - Fa[q] : Fa[q] - Fb[q];
+    }
   }
   if (p.use_regs && f0 != 0)
-    store_regs(p.face_src, p.fslot, p.R, p.FH, blk, D, 1, b * 8 + a, F0[0], F0[1], F0[2], F0[3], F0[4], dt);
+    store_regs(p.face_src, p.fslot, p.R, p.FH, blk, D, 1, b * 8 + a, Fa[0], Fa[1], Fa[2], Fa[3], Fa[4], dt);
 }
 
 // ---- helpers: staging ----------------------------------------------------------------------------------
@@ -426,6 +444,12 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
     if (STAGE == 1) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(WALK_REGS));
     const double igm1 = 1.0 / gm1;
     const int D = tid >> 7, f0 = ((tid >> 6) & 1) * 4, pen = tid & 63, a = pen & 7, b = pen >> 3;
+    WalkGeom geom;
+    if (STAGE == 1) {
+      if (D == 0) walk_geom<1, 0>(a, b, f0, geom);
+      else if (D == 1) walk_geom<1, 1>(a, b, f0, geom);
+      else walk_geom<1, 2>(a, b, f0, geom);
+    }
     auto convert_next = [&](int it) {                  // predictor: my share of block it, then both arrivals
       const int s = it & 1;
       mbar_wait(landed(s), (it >> 1) & 1);
@@ -457,9 +481,7 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
         else walk_predictor<2>(Wl, dF, a, b, f0, igm1, empty(d), pe, we);
       } else {
         const int blk = blk0 + it * stride;
-        if (D == 0) walk_corrector<0>(Wl, dF, a, b, f0, gamma, igm1, p, blk, dt, empty(d), pe, we);
-        else if (D == 1) walk_corrector<1>(Wl, dF, a, b, f0, gamma, igm1, p, blk, dt, empty(d), pe, we);
-        else walk_corrector<2>(Wl, dF, a, b, f0, gamma, igm1, p, blk, dt, empty(d), pe, we);
+        walk_corrector_generic(Wl, dF, geom, D, a, b, f0, gamma, igm1, p, blk, dt, empty(d), pe, we);
       }
       __syncwarp();
       if ((tid & 31) == 0) mbar_arrive(full(d));
