@@ -29,6 +29,11 @@ struct sfh_mesh {
   unsigned long long* smax = nullptr;   // [MAX_LEVELS] bit patterns of the per-level maximum speed
   double *dt_dev = nullptr, *t_dev = nullptr;
   unsigned long long* nbad = nullptr;
+  // per-block maximum CFL speed: written by the corrector for U^{n+1} (role 2), rewritten by the restriction and
+  // the reflux for the blocks they change.  pending[l]: the entries of level l describe its role-2 state;
+  // valid[l]: they describe its role-0 state (after the rotation), so the CFL reduction need not re-read it.
+  double* bmax = nullptr;
+  bool bmax_pending[MAX_LEVELS] = {false}, bmax_valid[MAX_LEVELS] = {false};
   int role[MAX_LEVELS][3];              // role -> physical state buffer, per level
   TensorMaps tm[3];                     // per physical state buffer
   int64_t launches = 0;
@@ -45,7 +50,7 @@ constexpr size_t ALIGN = 256;
 inline size_t up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct WorkLayout {
-  size_t ghost, R, FH, scalars, total;
+  size_t ghost, R, FH, bmax, scalars, total;
 };
 WorkLayout work_layout(const HostMesh& hm) {
   WorkLayout w;
@@ -53,7 +58,8 @@ WorkLayout work_layout(const HostMesh& hm) {
   w.ghost = 0;
   w.R = up(w.ghost + ncf * SLAB * 8);
   w.FH = up(w.R + ncf * REG * 8);
-  w.scalars = up(w.FH + size_t(hm.nfh) * REG * 8);
+  w.bmax = up(w.FH + size_t(hm.nfh) * REG * 8);
+  w.scalars = up(w.bmax + size_t(hm.nb) * 8);
   w.total = w.scalars + 4096;
   return w;
 }
@@ -203,6 +209,8 @@ int stage_level(sfh_mesh* m, int l, int stage, Dt dt, cudaStream_t st) {
   p.dt_dev = dt.dev; p.dt = dt.host; p.h = hm.h[l]; p.gamma = hm.cfg.gamma;
   p.first = int(hm.lev_first[l]); p.count = int(hm.lev_count[l]);
   p.use_regs = stage == 1 && (hm.cf_count[l] > 0 || hm.reflux_count[l] > 0);
+  p.bmax = stage == 1 ? m->bmax : nullptr;
+  if (stage == 1) m->bmax_pending[l] = true;
   {
     Timed tmr(m, stage, st);
     CU(launch_stage(stage, m->tm[m->role[l][src_role]], p, st), "stage_kernel");
@@ -233,25 +241,33 @@ int flux_correct_level(sfh_mesh* m, int lc, Dt dt, cudaStream_t st) {
   {
     Timed tmr(m, 3, st);
     CU(launch_restrict(role_buf(m, lc + 1, 0), role_buf(m, lc, 2), m->d_restrict_list + hm.restrict_first[lc],
-                       m->d_child0, int(hm.restrict_count[lc]), st), "restrict_kernel");
+                       m->d_child0, int(hm.restrict_count[lc]), hm.cfg.gamma, m->bmax, st), "restrict_kernel");
   }
   m->launches += hm.restrict_count[lc] > 0;
   {
     Timed tmr(m, 4, st);
     CU(launch_reflux(role_buf(m, lc, 2), m->R, m->FH, m->d_reflux_list + hm.reflux_first[lc], m->d_fslot,
-                     m->d_fh_src, int(hm.reflux_count[lc]), hm.h[lc], dt.host, dt.dev, st), "reflux_kernel");
+                     m->d_fh_src, int(hm.reflux_count[lc]), hm.h[lc], dt.host, dt.dev, hm.cfg.gamma, m->bmax, st),
+       "reflux_kernel");
   }
   m->launches += hm.reflux_count[lc] > 0;
   return SFH_OK;
 }
 
-void rotate(sfh_mesh* m, int l) { std::swap(m->role[l][0], m->role[l][2]); }
+void rotate(sfh_mesh* m, int l) {
+  std::swap(m->role[l][0], m->role[l][2]);
+  m->bmax_valid[l] = m->bmax_pending[l];     // the old U^n becomes scratch
+  m->bmax_pending[l] = false;
+}
 
 int max_speed_level(sfh_mesh* m, int l, cudaStream_t st) {
   const HostMesh& hm = m->hm;
   Timed tmr(m, 5, st);
-  CU(launch_max_speed(role_buf(m, l, 0), int(hm.lev_first[l]), int(hm.lev_count[l]), hm.cfg.gamma, m->smax + l, st),
-     "max_speed_kernel");
+  if (m->bmax_valid[l])
+    CU(launch_max_cached(m->bmax, int(hm.lev_first[l]), int(hm.lev_count[l]), m->smax + l, st), "max_cached_kernel");
+  else
+    CU(launch_max_speed(role_buf(m, l, 0), int(hm.lev_first[l]), int(hm.lev_count[l]), hm.cfg.gamma, m->smax + l, st),
+       "max_speed_kernel");
   m->launches += hm.lev_count[l] > 0;
   return SFH_OK;
 }
@@ -448,6 +464,8 @@ int sfh_bind(sfh_mesh* m, void* d_state0, void* d_state1, void* d_state2, void* 
   m->ghost = reinterpret_cast<double*>(wb + w.ghost);
   m->R = reinterpret_cast<double*>(wb + w.R);
   m->FH = reinterpret_cast<double*>(wb + w.FH);
+  m->bmax = reinterpret_cast<double*>(wb + w.bmax);
+  for (int l = 0; l < MAX_LEVELS; ++l) m->bmax_pending[l] = m->bmax_valid[l] = false;
   m->smax = reinterpret_cast<unsigned long long*>(wb + w.scalars);
   m->dt_dev = reinterpret_cast<double*>(wb + w.scalars + 256);
   m->t_dev = reinterpret_cast<double*>(wb + w.scalars + 512);
@@ -466,6 +484,8 @@ int sfh_set_state(sfh_mesh* m, int which, const double* d_U, void* stream) {
   if (rc) return rc;
   if (which < 0 || which > 2 || !d_U) return fail(SFH_EINVAL, "bad argument");
   for (int l = 0; l < m->hm.nlev; ++l) {
+    if (which == 0) m->bmax_valid[l] = false;
+    if (which == 2) m->bmax_pending[l] = false;
     CU(launch_permute(d_U, role_buf(m, l, which), m->d_perm, int(m->hm.lev_first[l]), int(m->hm.lev_count[l]), 1,
                       which == 1, m->hm.cfg.gamma, S(stream)), "permute_kernel");
     m->launches += m->hm.lev_count[l] > 0;
@@ -544,9 +564,12 @@ int sfh_restrict(sfh_mesh* m, int coarse_level, int src_role, int dst_role, void
   if (src_role == 1 || dst_role == 1)
     return fail(SFH_EINVAL, "the half-step state (role 1) is never restricted (DESIGN.md reading R10)");
   if (coarse_level + 1 >= hm.nlev || hm.restrict_count[coarse_level] == 0) return SFH_OK;
+  // the cached block maxima follow a restriction into U^{n+1} (role 2); one into U^n invalidates them
+  if (dst_role == 0) m->bmax_valid[coarse_level] = false;
   CU(launch_restrict(role_buf(m, coarse_level + 1, src_role), role_buf(m, coarse_level, dst_role),
                      m->d_restrict_list + hm.restrict_first[coarse_level], m->d_child0,
-                     int(hm.restrict_count[coarse_level]), S(stream)), "restrict_kernel");
+                     int(hm.restrict_count[coarse_level]), hm.cfg.gamma, dst_role == 2 ? m->bmax : nullptr, S(stream)),
+     "restrict_kernel");
   m->launches += 1;
   return SFH_OK;
 }

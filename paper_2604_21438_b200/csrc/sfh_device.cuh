@@ -131,6 +131,22 @@ __device__ __forceinline__ double sound_speed(double gamma, double P, double rho
   return gP * rsqrt_fast(gP * rho);
 }
 
+// CFL speed of one cell (reading R16): max_d |v_d| + c_s, from the conserved state.  Every kernel that
+// produces a block's maximum speed calls this, so the cached per-block maxima and the reduction over
+// whole states agree bit for bit.
+__device__ __forceinline__ double cell_speed(const double u[5], double gamma, double gm1) {
+  double w[5];
+  cons_to_prim(u, gm1, w);
+  const double cs = sound_speed(gamma, w[4], w[0]);
+  return fmax(fmax(fabs(w[1]), fabs(w[2])), fabs(w[3])) + cs;
+}
+
+__device__ __forceinline__ double warp_max(double x) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) x = fmax(x, __shfl_xor_sync(0xffffffffu, x, o));
+  return x;
+}
+
 // HLLC flux (Toro et al. 1994 as cited; Davis wave speeds, reading R6) in the face
 // frame: u = normal velocity, v, w = the two tangential ones; Fn = (mass, normal momentum, tangential
 // momenta, energy).  cL, cR = sound speeds of the two states; igm1 = 1/(gamma-1).

@@ -34,7 +34,7 @@ namespace sfh {
 constexpr int WALK_WARPS = 12, HELP_WARPS = 4;
 constexpr int WALK_THREADS = 32 * WALK_WARPS, HELP_THREADS = 32 * HELP_WARPS;
 constexpr int STAGE_THREADS = WALK_THREADS + HELP_THREADS;   // 512, launched with 128 registers each
-constexpr int WALK_REGS = 144, HELP_REGS = 80;               // corrector, after setmaxnreg
+constexpr int WALK_REGS = 136, HELP_REGS = 104;              // corrector, after setmaxnreg
 static_assert(WALK_THREADS * WALK_REGS + HELP_THREADS * HELP_REGS <= 65536, "register file of one SM");
 constexpr int CVS = NG * FACE;                // variable stride of every tile (128 cells)
 constexpr int NTILE = 10;
@@ -369,29 +369,36 @@ __device__ __forceinline__ void fill_outflow(double* __restrict__ L, const int* 
 // The flux differences are stored in the face frame (mass, normal, tangential 1, tangential 2,
 // energy): variable v of axis D is entry q with 1 + (D + q - 1) % 3 == v, q = 1..3.
 // PRIM_OUT: store primitives (the half-step state).
-template <bool PRIM_OUT>
-__device__ __forceinline__ void update_block(const double* __restrict__ dF, const double un[HC][NV], double lam,
-                                             double gm1, double* __restrict__ Uo, int hid) {
+// Two steps, so that the flux-difference buffer goes back to the walkers as early as possible:
+// combine_fluxes turns un into the updated conserved cells (the only shared-memory reads), store_block
+// writes them out (PRIM_OUT: as primitives, the half-step state).
+__device__ __forceinline__ void combine_fluxes(const double* __restrict__ dF, double un[HC][NV], double lam, int hid) {
 #pragma unroll
   for (int r = 0; r < HC; ++r) {
     const int cell = hid + r * HELP_THREADS;
     const int i = cell & 7, j = (cell >> 3) & 7, k = cell >> 6;
     const int cx = dfx_idx(i, j, k), cy = dfy_idx(i, j, k), cz = dfz_idx(i, j, k);
-    double u[NV];
 #pragma unroll
     for (int v = 0; v < NV; ++v) {
       const int qx = v, qy = (v == 0 || v == 4) ? v : 1 + (v + 1) % 3, qz = (v == 0 || v == 4) ? v : 1 + v % 3;
       const double sum = (dF[qx * NC + cx] + dF[qy * NC + cy]) + dF[qz * NC + cz];
-      u[v] = un[r][v] - lam * sum;
+      un[r][v] = un[r][v] - lam * sum;
     }
+  }
+}
+template <bool PRIM_OUT>
+__device__ __forceinline__ void store_block(const double u[HC][NV], double gm1, double* __restrict__ Uo, int hid) {
+#pragma unroll
+  for (int r = 0; r < HC; ++r) {
+    const int cell = hid + r * HELP_THREADS;
     if (PRIM_OUT) {
       double w[NV];
-      cons_to_prim(u, gm1, w);
+      cons_to_prim(u[r], gm1, w);
 #pragma unroll
       for (int v = 0; v < NV; ++v) Uo[v * NC + cell] = w[v];
     } else {
 #pragma unroll
-      for (int v = 0; v < NV; ++v) Uo[v * NC + cell] = u[v];
+      for (int v = 0; v < NV; ++v) Uo[v * NC + cell] = u[r][v];
     }
   }
 }
@@ -413,6 +420,7 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
   double* dF0 = L0 + 2 * C::LAND;
   uint64_t* bars = reinterpret_cast<uint64_t*>(dF0 + C::NDF * DF_DOUBLES);
   int* fsrc0 = reinterpret_cast<int*>(bars + 10);           // [2][8]
+  double* hmax = reinterpret_cast<double*>(bars + 20);      // [2][4] per-helper-warp maximum speed, double buffered
   const uint32_t bar0 = smem_u32(bars);
   auto landed = [&](int s) { return bar0 + 8u * s; };
   auto ready = [&](int s) { return bar0 + 16u + 8u * s; };
@@ -566,9 +574,10 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
 #ifdef SFH_DEBUG_TIMING
       t1 = clock64(); th[1] += t1 - t0; t0 = t1;
 #endif
-      update_block<STAGE == 0>(dF0 + d * DF_DOUBLES, un, lam, gm1, p.Udst + size_t(blk) * BLK, hid);
+      combine_fluxes(dF0 + d * DF_DOUBLES, un, lam, hid);
       __syncwarp();
-      if (lane0) mbar_arrive(empty(d));
+      if (lane0) mbar_arrive(empty(d));                // the walkers may store the next flux differences
+      store_block<STAGE == 0>(un, gm1, p.Udst + size_t(blk) * BLK, hid);
 #ifdef SFH_DEBUG_TIMING
       t1 = clock64(); th[2] += t1 - t0; t0 = t1;
       if (it + 2 < n) mbar_wait(landed(s), ((it + 2) >> 1) & 1);
@@ -578,6 +587,18 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
 #ifdef SFH_DEBUG_TIMING
       t1 = clock64(); th[4] += t1 - t0;
 #endif
+      if (STAGE == 1 && p.bmax) {
+        // Off the walkers' critical path (everything they wait for has been handed over): the block's maximum
+        // CFL speed for the next step's dt (reading R16) from the updated cells still in registers.
+        double sp[HC];
+#pragma unroll
+        for (int r = 0; r < HC; ++r) sp[r] = cell_speed(un[r], gamma, gm1);   // four independent chains
+        const double s = warp_max(fmax(fmax(sp[0], sp[1]), fmax(sp[2], sp[3])));
+        double* hm = hmax + 4 * (it & 1);
+        if (lane0) hm[hw] = s;
+        asm volatile("bar.sync 1, %0;" ::"n"(HELP_THREADS) : "memory");
+        if (hid == 0) p.bmax[blk] = fmax(fmax(hm[0], hm[1]), fmax(hm[2], hm[3]));
+      }
     }
 #ifdef SFH_DEBUG_TIMING
     if (blockIdx.x == 5 && lane0)

@@ -23,6 +23,7 @@ struct StageParams {
   double gamma;
   int first, count;      // slot range of the level
   int use_regs;          // corrector: the level has flux-register faces
+  double* bmax;          // corrector: per-block maximum CFL speed of U^{n+1} (or null)
 };
 
 struct TensorMaps {      // tensor maps of ONE state buffer seen as [5 nb][8][8][8]
@@ -64,13 +65,16 @@ struct ProlongParams {
 
 cudaError_t launch_stage(int stage, const TensorMaps& tm, const StageParams& p, cudaStream_t st);
 cudaError_t launch_prolong(const ProlongParams& p, cudaStream_t st);
+// bmax (nullable): per-block maximum CFL speed, rewritten for the blocks the kernel changes
 cudaError_t launch_restrict(const double* Ufine, double* Ucoarse, const int32_t* list, const int32_t* child0,
-                            int count, cudaStream_t st);
+                            int count, double gamma, double* bmax, cudaStream_t st);
 cudaError_t launch_reflux(double* U, const double* R, const double* FH, const int32_t* list, const int32_t* fslot,
                           const int32_t* fh_src, int count, double h, double dt, const double* dt_dev,
-                          cudaStream_t st);
+                          double gamma, double* bmax, cudaStream_t st);
 cudaError_t launch_max_speed(const double* U, int first, int count, double gamma, unsigned long long* smax_bits,
                              cudaStream_t st);
+cudaError_t launch_max_cached(const double* bmax, int first, int count, unsigned long long* smax_bits,
+                              cudaStream_t st);
 struct LevelInfo {
   double h[MAX_LEVELS];
   int has[MAX_LEVELS];

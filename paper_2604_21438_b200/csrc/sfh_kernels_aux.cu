@@ -7,6 +7,20 @@
 
 namespace sfh {
 
+// maximum over the CTA (NW warps); the result is valid in thread 0.  wm: NW doubles of shared memory
+template <int NW>
+__device__ __forceinline__ double cta_max(double x, double* wm) {
+  x = warp_max(x);
+  if ((threadIdx.x & 31) == 0) wm[threadIdx.x >> 5] = x;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    x = threadIdx.x < NW ? wm[threadIdx.x] : 0.0;
+    x = warp_max(x);
+  }
+  return x;
+}
+
+
 // =====================================================================================================
 // a3: ghost slabs of coarse-fine faces.  One CTA of 128 threads per slab, one thread per ghost cell.
 // Fine ghost cell -> coarse cell (index >> 1) of the parent's neighbourhood; per variable the coarse
@@ -126,27 +140,35 @@ cudaError_t launch_prolong(const ProlongParams& p, cudaStream_t st) {
 // =====================================================================================================
 __global__ void __launch_bounds__(NC) restrict_kernel(const double* __restrict__ Uf, double* __restrict__ Uc,
                                                       const int32_t* __restrict__ list,
-                                                      const int32_t* __restrict__ child0) {
+                                                      const int32_t* __restrict__ child0, double gamma,
+                                                      double* __restrict__ bmax) {
   const int b = list[blockIdx.x];
   const int t = threadIdx.x, i = t & 7, j = (t >> 3) & 7, k = t >> 6;
   const int child = child0[b] + (i >> 2) + 2 * (j >> 2) + 4 * (k >> 2);
   const int fi = 2 * (i & 3), fj = 2 * (j & 3), fk = 2 * (k & 3);
   const double* src = Uf + size_t(child) * BLK;
   double* dst = Uc + size_t(b) * BLK + t;
+  double u[NV];
 #pragma unroll
   for (int v = 0; v < NV; ++v) {
     double sum = 0.0;
 #pragma unroll
     for (int c = 0; c < 8; ++c)
       sum += src[v * NC + ((fk + ((c >> 2) & 1)) * 8 + fj + ((c >> 1) & 1)) * 8 + fi + (c & 1)];
-    dst[v * NC] = 0.125 * sum;
+    u[v] = 0.125 * sum;
+    dst[v * NC] = u[v];
+  }
+  if (bmax) {                       // the block's cached maximum speed follows its new contents
+    __shared__ double wm[NC / 32];
+    const double s = cta_max<NC / 32>(cell_speed(u, gamma, gamma - 1.0), wm);
+    if (t == 0) bmax[b] = s;
   }
 }
 
 cudaError_t launch_restrict(const double* Ufine, double* Ucoarse, const int32_t* list, const int32_t* child0, int count,
-                            cudaStream_t st) {
+                            double gamma, double* bmax, cudaStream_t st) {
   if (count <= 0) return cudaSuccess;
-  restrict_kernel<<<count, NC, 0, st>>>(Ufine, Ucoarse, list, child0);
+  restrict_kernel<<<count, NC, 0, st>>>(Ufine, Ucoarse, list, child0, gamma, bmax);
   return cudaGetLastError();
 }
 
@@ -160,7 +182,8 @@ __global__ void __launch_bounds__(FACE) reflux_kernel(double* __restrict__ U, co
                                                       const int32_t* __restrict__ list,
                                                       const int32_t* __restrict__ fslot,
                                                       const int32_t* __restrict__ fh_src, double h, double dt_host,
-                                                      const double* __restrict__ dt_dev) {
+                                                      const double* __restrict__ dt_dev, double gamma,
+                                                      double* __restrict__ bmax) {
   const int b = list[blockIdx.x];
   const int t = threadIdx.x, ta = t & 7, tb = t >> 3;
   const double dt = dt_dev ? *dt_dev : dt_host;
@@ -185,13 +208,27 @@ __global__ void __launch_bounds__(FACE) reflux_kernel(double* __restrict__ U, co
     }
     __syncthreads();
   }
+  if (bmax) {                       // the block's cached maximum speed follows its corrected cells
+    const double gm1 = gamma - 1.0;
+    double smax = 0.0;
+#pragma unroll
+    for (int c = t; c < NC; c += FACE) {
+      double u[NV];
+#pragma unroll
+      for (int v = 0; v < NV; ++v) u[v] = Ub[v * NC + c];
+      smax = fmax(smax, cell_speed(u, gamma, gm1));
+    }
+    __shared__ double wm[FACE / 32];
+    smax = cta_max<FACE / 32>(smax, wm);
+    if (t == 0) bmax[b] = smax;
+  }
 }
 
 cudaError_t launch_reflux(double* U, const double* R, const double* FH, const int32_t* list, const int32_t* fslot,
                           const int32_t* fh_src, int count, double h, double dt, const double* dt_dev,
-                          cudaStream_t st) {
+                          double gamma, double* bmax, cudaStream_t st) {
   if (count <= 0) return cudaSuccess;
-  reflux_kernel<<<count, FACE, 0, st>>>(U, R, FH, list, fslot, fh_src, h, dt, dt_dev);
+  reflux_kernel<<<count, FACE, 0, st>>>(U, R, FH, list, fslot, fh_src, h, dt, dt_dev, gamma, bmax);
   return cudaGetLastError();
 }
 
@@ -199,12 +236,6 @@ cudaError_t launch_reflux(double* U, const double* R, const double* FH, const in
 // a10: CFL reduction ("grid-level reductions"; reading R16).  Per-thread running max,
 // warp-shuffle max, one atomicMax per CTA on the bit pattern (positive doubles order like integers).
 // =====================================================================================================
-__device__ __forceinline__ double warp_max(double x) {
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) x = fmax(x, __shfl_xor_sync(0xffffffffu, x, o));
-  return x;
-}
-
 __global__ void __launch_bounds__(256) max_speed_kernel(const double* __restrict__ U, int first, int count, double gamma,
                                                         unsigned long long* smax_bits) {
   const double gm1 = gamma - 1.0;
@@ -213,24 +244,35 @@ __global__ void __launch_bounds__(256) max_speed_kernel(const double* __restrict
     const double* Ub = U + size_t(first + b) * BLK;
 #pragma unroll
     for (int c = threadIdx.x; c < NC; c += 256) {
-      double u[5], w[5];
+      double u[5];
 #pragma unroll
       for (int v = 0; v < NV; ++v) u[v] = Ub[v * NC + c];
-      cons_to_prim(u, gm1, w);
-      const double cs = sound_speed(gamma, w[4], w[0]);
-      const double s = fmax(fmax(fabs(w[1]), fabs(w[2])), fabs(w[3])) + cs;
+      const double s = cell_speed(u, gamma, gm1);
       if (s > smax) smax = s;
     }
   }
-  smax = warp_max(smax);
   __shared__ double wm[8];
-  if ((threadIdx.x & 31) == 0) wm[threadIdx.x >> 5] = smax;
-  __syncthreads();
-  if (threadIdx.x < 32) {
-    double x = threadIdx.x < 8 ? wm[threadIdx.x] : 0.0;
-    x = warp_max(x);
-    if (threadIdx.x == 0) atomicMax(smax_bits, (unsigned long long)__double_as_longlong(x));
-  }
+  smax = cta_max<8>(smax, wm);
+  if (threadIdx.x == 0) atomicMax(smax_bits, (unsigned long long)__double_as_longlong(smax));
+}
+
+// the same maximum from the per-block maxima the corrector, the restriction and the reflux leave behind
+__global__ void __launch_bounds__(256) max_cached_kernel(const double* __restrict__ bmax, int first, int count,
+                                                         unsigned long long* smax_bits) {
+  double smax = 0.0;
+  for (int b = blockIdx.x * 256 + threadIdx.x; b < count; b += gridDim.x * 256) smax = fmax(smax, bmax[first + b]);
+  __shared__ double wm[8];
+  smax = cta_max<8>(smax, wm);
+  if (threadIdx.x == 0) atomicMax(smax_bits, (unsigned long long)__double_as_longlong(smax));
+}
+
+cudaError_t launch_max_cached(const double* bmax, int first, int count, unsigned long long* smax_bits,
+                              cudaStream_t st) {
+  cudaError_t e = cudaMemsetAsync(smax_bits, 0, sizeof(unsigned long long), st);
+  if (e != cudaSuccess || count <= 0) return e;
+  const int need = (count + 2047) / 2048;
+  max_cached_kernel<<<need < 148 ? need : 148, 256, 0, st>>>(bmax, first, count, smax_bits);
+  return cudaGetLastError();
 }
 
 cudaError_t launch_max_speed(const double* U, int first, int count, double gamma, unsigned long long* smax_bits,
