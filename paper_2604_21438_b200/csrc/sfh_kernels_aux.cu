@@ -22,18 +22,92 @@ __device__ __forceinline__ double cta_max(double x, double* wm) {
 
 
 // =====================================================================================================
-// a3: ghost slabs of coarse-fine faces.  One CTA of 128 threads per slab, one thread per ghost cell.
-// Fine ghost cell -> coarse cell (index >> 1) of the parent's neighbourhood; per variable the coarse
-// value and its 6 axis neighbours (each optionally interpolated in time, eq. 16) give minmod slopes
-// and the fine value Q + sum_d (+-1/4) slope_d (reading R3).
+// a3: ghost slabs of coarse-fine faces.  One CTA of 128 threads per slab (2 layers x 8 x 8 fine cells
+// behind one coarse layer of 4 x 4 cells).  Step 1: the 68 coarse cells any of the 7-point stencils
+// touches -- the coarse layer with a one-cell rim (6 x 6, corners unused) and the 4 x 4 cells on either
+// side of it along the face normal -- are gathered once, interpolated in time (eq. 16) and, where the
+// coarse copy holds primitives, converted back to conserved variables, into shared memory.  Step 2: one
+// thread per fine ghost cell: minmod slopes of the coarse cell and the fine value
+// Q + sum_d (+-1/4) slope_d (reading R3).
 // =====================================================================================================
+constexpr int PR_RIM = 36, PR_CELLS = PR_RIM + 2 * 16;   // [6 x 6 layer | 4 x 4 below | 4 x 4 above]
+
 __global__ void __launch_bounds__(128) prolong_kernel(const ProlongParams p) {
+  __shared__ double q[PR_CELLS][NV];
+  __shared__ int missing;
   const int slot = p.first + blockIdx.x;
   const int F = p.cf_block[slot], f = p.cf_face[slot], axis = f >> 1, side = f & 1;
   const int P = p.parent[F];
-  const int oct[3] = {p.coord[3 * F] & 1, p.coord[3 * F + 1] & 1, p.coord[3 * F + 2] & 1};
+  const int t1ax = axis == 0 ? 1 : 0, t2ax = axis == 2 ? 1 : 2;    // the two in-face axes, lower first
+  int oct[3];
+#pragma unroll
+  for (int d = 0; d < 3; ++d) oct[d] = p.coord[3 * F + d] & 1;
   const int r = threadIdx.x;
-  int fc[3];   // fine local coordinates of this ghost cell, slab layouts as staged by the stage kernels
+  if (r == 0) missing = 0;
+  __syncthreads();
+  const double gm1 = p.gamma - 1.0, igm1 = 1.0 / gm1;
+
+  // ---- step 1: thread r < 68 gathers coarse cell r of the stencil region
+  if (r < PR_CELLS) {
+    int ca, c1, c2;                       // offsets from (coarse layer, first coarse cell of the octant)
+    bool needed = true;
+    if (r < PR_RIM) {
+      ca = 0; c1 = r % 6 - 1; c2 = r / 6 - 1;
+      needed = !((c1 < 0 || c1 > 3) && (c2 < 0 || c2 > 3));
+    } else {
+      const int e = (r - PR_RIM) & 15;
+      ca = r < PR_RIM + 16 ? -1 : 1; c1 = e & 3; c2 = e >> 2;
+    }
+    if (needed) {
+      int c[3], rg[3];
+      c[axis] = (side ? oct[axis] * 4 + 4 : oct[axis] * 4 - 1) + ca;
+      c[t1ax] = oct[t1ax] * 4 + c1;
+      c[t2ax] = oct[t2ax] * 4 + c2;
+      const int32_t* nb = p.nbr27 + size_t(P) * 27;
+      // does the parent touch an outflow boundary?  (face-region codes)
+      const bool out_lo[3] = {nb[12] == NBR_OUTSIDE, nb[10] == NBR_OUTSIDE, nb[4] == NBR_OUTSIDE};
+      const bool out_hi[3] = {nb[14] == NBR_OUTSIDE, nb[16] == NBR_OUTSIDE, nb[22] == NBR_OUTSIDE};
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {
+        rg[d] = 0;
+        if (c[d] < 0) { if (out_lo[d]) c[d] = 0; else { rg[d] = -1; c[d] += N; } }
+        else if (c[d] >= N) { if (out_hi[d]) c[d] = N - 1; else { rg[d] = 1; c[d] -= N; } }
+      }
+      const int Q = nb[(rg[2] + 1) * 9 + (rg[1] + 1) * 3 + (rg[0] + 1)];
+      if (Q < 0) {
+        missing = 1;                      // (a mesh sfh_create_mesh accepts never gets here)
+      } else {
+        const size_t o = size_t(Q) * BLK + (c[2] * 8 + c[1]) * 8 + c[0];
+        double u0[NV], u1[NV], u2[NV], t[NV];
+#pragma unroll
+        for (int v = 0; v < NV; ++v) u0[v] = p.C0[o + v * NC];
+        if (p.interp) {
+#pragma unroll
+          for (int v = 0; v < NV; ++v) { u1[v] = p.C1[o + v * NC]; u2[v] = p.C2[o + v * NC]; }
+        }
+        if (p.c0_prim) {
+          prim_to_cons(u0, igm1, t);
+#pragma unroll
+          for (int v = 0; v < NV; ++v) u0[v] = t[v];
+        }
+        if (p.interp) {
+          if (p.c1_prim) {
+            prim_to_cons(u1, igm1, t);
+#pragma unroll
+            for (int v = 0; v < NV; ++v) u1[v] = t[v];
+          }
+#pragma unroll
+          for (int v = 0; v < NV; ++v) u0[v] = time_interp(u0[v], u1[v], u2[v], p.tau);
+        }
+#pragma unroll
+        for (int v = 0; v < NV; ++v) q[r][v] = u0[v];
+      }
+    }
+  }
+  __syncthreads();
+
+  // ---- step 2: thread r computes fine ghost cell r of the slab (slab layouts as staged by the stage kernels)
+  int fc[3];
   if (axis == 0) {
     const int ll = r & 1;
     fc[0] = side ? N + ll : ll - NG; fc[1] = (r >> 1) & 7; fc[2] = r >> 4;
@@ -44,75 +118,26 @@ __global__ void __launch_bounds__(128) prolong_kernel(const ProlongParams p) {
     const int ll = r >> 6;
     fc[0] = r & 7; fc[1] = (r >> 3) & 7; fc[2] = side ? N + ll : ll - NG;
   }
-  int cc[3];
-  double sig[3];
-#pragma unroll
-  for (int d = 0; d < 3; ++d) {
-    cc[d] = oct[d] * 4 + (fc[d] >> 1);          // arithmetic shift: -2,-1 -> -1
-    sig[d] = (fc[d] & 1) ? 0.25 : -0.25;
-  }
-  const int32_t* nb = p.nbr27 + size_t(P) * 27;
-  // does the parent touch an outflow boundary?  (face-region codes)
-  bool out_lo[3], out_hi[3];
-  out_lo[0] = nb[12] == NBR_OUTSIDE; out_hi[0] = nb[14] == NBR_OUTSIDE;
-  out_lo[1] = nb[10] == NBR_OUTSIDE; out_hi[1] = nb[16] == NBR_OUTSIDE;
-  out_lo[2] = nb[4] == NBR_OUTSIDE;  out_hi[2] = nb[22] == NBR_OUTSIDE;
-
-  auto locate = [&](int c0, int c1, int c2) -> long long {   // offset of variable 0 of a coarse cell, or -1
-    int c[3] = {c0, c1, c2}, rg[3];
-#pragma unroll
-    for (int d = 0; d < 3; ++d) {
-      rg[d] = 0;
-      if (c[d] < 0) { if (out_lo[d]) c[d] = 0; else { rg[d] = -1; c[d] += N; } }
-      else if (c[d] >= N) { if (out_hi[d]) c[d] = N - 1; else { rg[d] = 1; c[d] -= N; } }
-    }
-    const int Q = nb[(rg[2] + 1) * 9 + (rg[1] + 1) * 3 + (rg[0] + 1)];
-    if (Q < 0) return -1;
-    return (long long)Q * BLK + (c[2] * 8 + c[1]) * 8 + c[0];
-  };
-  long long o[7];
-  o[0] = locate(cc[0], cc[1], cc[2]);
-  o[1] = locate(cc[0] + 1, cc[1], cc[2]); o[2] = locate(cc[0] - 1, cc[1], cc[2]);
-  o[3] = locate(cc[0], cc[1] + 1, cc[2]); o[4] = locate(cc[0], cc[1] - 1, cc[2]);
-  o[5] = locate(cc[0], cc[1], cc[2] + 1); o[6] = locate(cc[0], cc[1], cc[2] - 1);
-  bool ok = true;
-#pragma unroll
-  for (int s = 0; s < 7; ++s) ok = ok && o[s] >= 0;
-  const double gm1 = p.gamma - 1.0, igm1 = 1.0 / gm1;
-  // conserved values of the 7 stencil cells (a coarse copy held as primitives is converted back)
-  double q[7][NV];
-#pragma unroll
-  for (int s = 0; s < 7; ++s) {
-    if (!ok) {
-#pragma unroll
-      for (int v = 0; v < NV; ++v) q[s][v] = nan("");
-      continue;
-    }
-    double u0[NV], u1[NV], u2[NV], t[NV];
-#pragma unroll
-    for (int v = 0; v < NV; ++v) u0[v] = p.C0[o[s] + v * NC];
-    if (p.c0_prim) { prim_to_cons(u0, igm1, t);
-#pragma unroll
-      for (int v = 0; v < NV; ++v) u0[v] = t[v]; }
-    if (p.interp) {
-#pragma unroll
-      for (int v = 0; v < NV; ++v) { u1[v] = p.C1[o[s] + v * NC]; u2[v] = p.C2[o[s] + v * NC]; }
-      if (p.c1_prim) { prim_to_cons(u1, igm1, t);
-#pragma unroll
-        for (int v = 0; v < NV; ++v) u1[v] = t[v]; }
-#pragma unroll
-      for (int v = 0; v < NV; ++v) q[s][v] = time_interp(u0[v], u1[v], u2[v], p.tau);
-    } else {
-#pragma unroll
-      for (int v = 0; v < NV; ++v) q[s][v] = u0[v];
-    }
-  }
+  const int c1 = fc[t1ax] >> 1, c2 = fc[t2ax] >> 1;
+  const int ctr = (c2 + 1) * 6 + (c1 + 1);
+  int nbp[3], nbm[3];                     // stencil neighbours +d / -d, per axis d
+  nbp[axis] = PR_RIM + 16 + c2 * 4 + c1; nbm[axis] = PR_RIM + c2 * 4 + c1;
+  nbp[t1ax] = ctr + 1; nbm[t1ax] = ctr - 1;
+  nbp[t2ax] = ctr + 6; nbm[t2ax] = ctr - 6;
   double val[NV];
 #pragma unroll
   for (int v = 0; v < NV; ++v) {
-    val[v] = q[0][v];
+    const double q0 = q[ctr][v];
+    val[v] = q0;
 #pragma unroll
-    for (int d = 0; d < 3; ++d) val[v] = val[v] + sig[d] * minmod(q[1 + 2 * d][v] - q[0][v], q[0][v] - q[2 + 2 * d][v]);
+    for (int d = 0; d < 3; ++d) {
+      const double sig = (fc[d] & 1) ? 0.25 : -0.25;
+      val[v] = val[v] + sig * minmod(q[nbp[d]][v] - q0, q0 - q[nbm[d]][v]);
+    }
+  }
+  if (missing) {
+#pragma unroll
+    for (int v = 0; v < NV; ++v) val[v] = nan("");
   }
   if (p.out_prim) {           // the corrector stages primitives
     double w[NV];

@@ -16,8 +16,12 @@ SEED = 20260421
 CONFIG_NAMES = ("C1", "C2", "C3", "C4", "C5")
 # C5: density contrast (relative to the mean) above which a level-0 block is refined; level l uses
 # RHO_C5 * 4^l (Jeans length < 8 cells with G = c_s = 1 after the amplitude normalisation of
-# DESIGN.md reading R22).  Calibrated once (seed SEED+30) so that the padded tree has ~1.8e5 blocks.
-RHO_C5 = 1.30
+# DESIGN.md reading R22).  Calibrated once (seed SEED+30) so that the padded tree of the full-size case
+# has ~1.8e5 blocks (census 32768 / 114672 / 30928 / 3504 / 136 = 182008).  The shrunken parity cases
+# use RHO_C5_SMALL: their base fields have less dynamic range, and the lower threshold keeps all four
+# refinement levels populated.
+RHO_C5 = 8.0
+RHO_C5_SMALL = 1.30
 
 
 @dataclass
@@ -187,5 +191,5 @@ def make_config(name, scale=1):
     if name == "C4":
         return amr_sphere(nb=16 // scale)
     if name == "C5":
-        return gmc(n=256 // scale, mach=10.0 / scale)
+        return gmc(n=256 // scale, mach=10.0 / scale, rho_c=RHO_C5 if scale == 1 else RHO_C5_SMALL)
     raise ValueError(name)
