@@ -76,14 +76,15 @@ int64_t sfh_num_blocks(const sfh_mesh* m);
 int sfh_level_range(const sfh_mesh* m, int level, int64_t* first, int64_t* count);
 /* perm[s] = caller index of the block stored in library slot s (host array [nblocks]). */
 int sfh_block_order(const sfh_mesh* m, int64_t* perm);
-/* Number of coarse-fine block faces (fine side; one ghost slab and one flux register each) and of
+/* Number of coarse-fine block faces (fine side; two ghost slabs -- of U^n and of the
+ * half-step state -- and one flux register each) and of
  * coarse-leaf faces that receive a flux correction. */
 int sfh_num_faces(const sfh_mesh* m, int64_t* n_fine_faces, int64_t* n_coarse_faces);
 /* Cell width of a level. */
 double sfh_cell_width(const sfh_mesh* m, int level);
 
 /* Bytes of ONE state copy in the internal layout, and of the work buffer (coarse-fine ghost
- * slabs, flux registers, reduction scratch). */
+ * slabs, flux registers, per-block maximum speeds, reduction scratch). */
 int64_t sfh_state_bytes(const sfh_mesh* m);
 int64_t sfh_work_bytes(const sfh_mesh* m);
 

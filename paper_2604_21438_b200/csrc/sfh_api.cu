@@ -25,7 +25,7 @@ struct sfh_mesh {
           *d_restrict_list = nullptr, *d_reflux_list = nullptr;
   int64_t* d_perm = nullptr;
   double* state[3] = {nullptr, nullptr, nullptr};
-  double *ghost = nullptr, *R = nullptr, *FH = nullptr;
+  double *ghost = nullptr, *ghost1 = nullptr, *R = nullptr, *FH = nullptr;   // ghost: slabs of U^n, ghost1: of U^{n+1/2}
   unsigned long long* smax = nullptr;   // [MAX_LEVELS] bit patterns of the per-level maximum speed
   double *dt_dev = nullptr, *t_dev = nullptr;
   unsigned long long* nbad = nullptr;
@@ -56,7 +56,7 @@ WorkLayout work_layout(const HostMesh& hm) {
   WorkLayout w;
   const size_t ncf = hm.cf_block.size();
   w.ghost = 0;
-  w.R = up(w.ghost + ncf * SLAB * 8);
+  w.R = up(w.ghost + 2 * ncf * SLAB * 8);      // two slab sets: the fill of U^n and of the half-step state
   w.FH = up(w.R + ncf * REG * 8);
   w.bmax = up(w.FH + size_t(hm.nfh) * REG * 8);
   w.scalars = up(w.bmax + size_t(hm.nb) * 8);
@@ -172,13 +172,18 @@ struct Dt {   // a step known on the host, or to be read from device memory
   const double* dev;
 };
 
-int fill_level(sfh_mesh* m, int l, int which, int interp, double tau, cudaStream_t st) {
+// which = 1 fills the half-step slabs (ghost1), else the U^n slabs.  dual (interp only): one gather fills both,
+// the U^n slabs at tau and the half-step slabs at tau1.
+int fill_level(sfh_mesh* m, int l, int which, int interp, double tau, cudaStream_t st, bool dual = false,
+               double tau1 = 0.0) {
   const HostMesh& hm = m->hm;
   if (l == 0 || hm.cf_count[l] == 0) return SFH_OK;
   ProlongParams p;
   if (interp) { p.C0 = role_buf(m, l - 1, 0); p.C1 = role_buf(m, l - 1, 1); p.C2 = role_buf(m, l - 1, 2); }
   else { p.C0 = p.C1 = p.C2 = role_buf(m, l - 1, which); }
-  p.ghost = m->ghost;
+  p.ghost = which == 1 ? m->ghost1 : m->ghost;
+  p.ghost1 = dual ? m->ghost1 : nullptr;
+  p.tau1 = tau1;
   p.cf_block = m->d_cf_block; p.cf_face = m->d_cf_face; p.parent = m->d_parent; p.coord = m->d_coord;
   p.nbr27 = m->d_nbr27;
   p.first = int(hm.cf_first[l]); p.count = int(hm.cf_count[l]);
@@ -204,7 +209,7 @@ int stage_level(sfh_mesh* m, int l, int stage, Dt dt, cudaStream_t st) {
   p.Usrc = role_buf(m, l, src_role);
   p.Un = role_buf(m, l, 0);
   p.Udst = role_buf(m, l, stage == 0 ? 1 : 2);
-  p.ghost = m->ghost; p.R = m->R; p.FH = m->FH;
+  p.ghost = stage == 0 ? m->ghost : m->ghost1; p.R = m->R; p.FH = m->FH;
   p.face_src = m->d_face_src; p.fslot = m->d_fslot;
   p.dt_dev = dt.dev; p.dt = dt.host; p.h = hm.h[l]; p.gamma = hm.cfg.gamma;
   p.first = int(hm.lev_first[l]); p.count = int(hm.lev_count[l]);
@@ -227,11 +232,12 @@ int zero_fine_registers(sfh_mesh* m, int coarse_level, cudaStream_t st) {   // r
   return SFH_OK;
 }
 
-int hydro_level(sfh_mesh* m, int l, Dt dt, int interp, double tau, double dtau, cudaStream_t st) {
+int hydro_level(sfh_mesh* m, int l, Dt dt, int interp, double tau, double dtau, cudaStream_t st,
+                bool half_filled = false) {
   int rc;
   if ((rc = zero_fine_registers(m, l, st))) return rc;
   if ((rc = stage_level(m, l, 0, dt, st))) return rc;
-  if ((rc = fill_level(m, l, 1, interp, tau + 0.5 * dtau, st))) return rc;
+  if (!half_filled && (rc = fill_level(m, l, 1, interp, tau + 0.5 * dtau, st))) return rc;
   return stage_level(m, l, 1, dt, st);
 }
 
@@ -302,8 +308,9 @@ int advance_adaptive(sfh_mesh* m, int l, double dt, double tau, double dtau, int
   const HostMesh& hm = m->hm;
   const int interp = l > 0;
   int rc;
-  if ((rc = fill_level(m, l, 0, interp, tau, st))) return rc;
-  if ((rc = hydro_level(m, l, Dt{dt, nullptr}, interp, tau, dtau, st))) return rc;
+  // the coarser level has finished its step: its three time copies give both ghost fills in one gather
+  if ((rc = fill_level(m, l, 0, interp, tau, st, interp != 0, tau + 0.5 * dtau))) return rc;
+  if ((rc = hydro_level(m, l, Dt{dt, nullptr}, interp, tau, dtau, st, interp != 0))) return rc;
   if (nupd) nupd[l] += 1;
   if (l + 1 < hm.nlev && hm.lev_count[l + 1] > 0) {
     double dtc;
@@ -462,6 +469,7 @@ int sfh_bind(sfh_mesh* m, void* d_state0, void* d_state1, void* d_state2, void* 
   char* wb = static_cast<char*>(d_work);
   CU(cudaMemset(wb, 0, w.total), "zero work buffer");
   m->ghost = reinterpret_cast<double*>(wb + w.ghost);
+  m->ghost1 = m->ghost + hm.cf_block.size() * SLAB;
   m->R = reinterpret_cast<double*>(wb + w.R);
   m->FH = reinterpret_cast<double*>(wb + w.FH);
   m->bmax = reinterpret_cast<double*>(wb + w.bmax);
@@ -519,7 +527,7 @@ int sfh_get_ghosted(sfh_mesh* m, int which, double* d_G, void* stream) {
   if (rc) return rc;
   if (which < 0 || which > 2 || !d_G) return fail(SFH_EINVAL, "bad argument");
   for (int l = 0; l < m->hm.nlev; ++l) {
-    CU(launch_ghosted(role_buf(m, l, which), m->ghost, m->d_face_src, m->d_perm, int(m->hm.lev_first[l]),
+    CU(launch_ghosted(role_buf(m, l, which), which == 1 ? m->ghost1 : m->ghost, m->d_face_src, m->d_perm, int(m->hm.lev_first[l]),
                       int(m->hm.lev_count[l]), which == 1, m->hm.cfg.gamma, d_G, S(stream)), "ghosted_kernel");
     m->launches += m->hm.lev_count[l] > 0;
   }

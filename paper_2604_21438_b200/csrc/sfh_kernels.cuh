@@ -61,6 +61,9 @@ struct ProlongParams {
   int c0_prim, c1_prim;  // the coarse copy C0 / C1 holds primitives (the half-step state)
   int out_prim;          // write primitives (half-step fill)
   double gamma;
+  // dual fill (interp = 1 only): the same gather also yields the half-step slab at tau1, as primitives
+  double* ghost1;        // or null
+  double tau1;
 };
 
 cudaError_t launch_stage(int stage, const TensorMaps& tm, const StageParams& p, cudaStream_t st);

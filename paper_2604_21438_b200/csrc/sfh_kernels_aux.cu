@@ -34,6 +34,7 @@ constexpr int PR_RIM = 36, PR_CELLS = PR_RIM + 2 * 16;   // [6 x 6 layer | 4 x 4
 
 __global__ void __launch_bounds__(128) prolong_kernel(const ProlongParams p) {
   __shared__ double q[PR_CELLS][NV];
+  __shared__ double q1[PR_CELLS][NV];      // dual fill: the same cells at tau1
   __shared__ int missing;
   const int slot = p.first + blockIdx.x;
   const int F = p.cf_block[slot], f = p.cf_face[slot], axis = f >> 1, side = f & 1;
@@ -96,6 +97,10 @@ __global__ void __launch_bounds__(128) prolong_kernel(const ProlongParams p) {
 #pragma unroll
             for (int v = 0; v < NV; ++v) u1[v] = t[v];
           }
+          if (p.ghost1) {
+#pragma unroll
+            for (int v = 0; v < NV; ++v) q1[r][v] = time_interp(u0[v], u1[v], u2[v], p.tau1);
+          }
 #pragma unroll
           for (int v = 0; v < NV; ++v) u0[v] = time_interp(u0[v], u1[v], u2[v], p.tau);
         }
@@ -124,33 +129,37 @@ __global__ void __launch_bounds__(128) prolong_kernel(const ProlongParams p) {
   nbp[axis] = PR_RIM + 16 + c2 * 4 + c1; nbm[axis] = PR_RIM + c2 * 4 + c1;
   nbp[t1ax] = ctr + 1; nbm[t1ax] = ctr - 1;
   nbp[t2ax] = ctr + 6; nbm[t2ax] = ctr - 6;
-  double val[NV];
-#pragma unroll
-  for (int v = 0; v < NV; ++v) {
-    const double q0 = q[ctr][v];
-    val[v] = q0;
-#pragma unroll
-    for (int d = 0; d < 3; ++d) {
-      const double sig = (fc[d] & 1) ? 0.25 : -0.25;
-      val[v] = val[v] + sig * minmod(q[nbp[d]][v] - q0, q0 - q[nbm[d]][v]);
-    }
-  }
-  if (missing) {
-#pragma unroll
-    for (int v = 0; v < NV; ++v) val[v] = nan("");
-  }
-  if (p.out_prim) {           // the corrector stages primitives
-    double w[NV];
-    cons_to_prim(val, gm1, w);
-#pragma unroll
-    for (int v = 0; v < NV; ++v) val[v] = w[v];
-  }
-  // the slab is written in the staging layout of the stage kernels
   const int ll = fc[axis] < 0 ? fc[axis] + NG : fc[axis] - N;
   const int rout = slab_pos(axis, ll, fc[axis == 0 ? 1 : 0], fc[axis == 2 ? 1 : 2]);
-  double* out = p.ghost + size_t(slot) * SLAB + rout;
+  auto fine_value = [&](const double (*qq)[NV], bool prim, double* __restrict__ ghost) {
+    double val[NV];
 #pragma unroll
-  for (int v = 0; v < NV; ++v) out[v * NG * FACE] = val[v];
+    for (int v = 0; v < NV; ++v) {
+      const double q0 = qq[ctr][v];
+      val[v] = q0;
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {
+        const double sig = (fc[d] & 1) ? 0.25 : -0.25;
+        val[v] = val[v] + sig * minmod(qq[nbp[d]][v] - q0, q0 - qq[nbm[d]][v]);
+      }
+    }
+    if (missing) {
+#pragma unroll
+      for (int v = 0; v < NV; ++v) val[v] = nan("");
+    }
+    if (prim) {               // the corrector stages primitives
+      double w[NV];
+      cons_to_prim(val, gm1, w);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) val[v] = w[v];
+    }
+    // the slab is written in the staging layout of the stage kernels
+    double* out = ghost + size_t(slot) * SLAB + rout;
+#pragma unroll
+    for (int v = 0; v < NV; ++v) out[v * NG * FACE] = val[v];
+  };
+  fine_value(q, p.out_prim != 0, p.ghost);
+  if (p.ghost1) fine_value(q1, true, p.ghost1);
 }
 
 cudaError_t launch_prolong(const ProlongParams& p, cudaStream_t st) {
