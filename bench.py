@@ -273,7 +273,7 @@ def main():
     c_ms, c_n = kt["corrector"]
     corr_bytes = CORRECTOR_BYTES_PER_CELL * cu            # every cell-update passes the corrector once
     achieved = corr_bytes / (c_ms * 1e-3) / 1e9 if c_ms > 0 else 0.0
-    roofline = {"bound": "hbm", "kernel": "corrector_kernel", "achieved": achieved, "peak": peak,
+    roofline = {"bound": "hbm", "kernel": "stage_kernel<1> (corrector)", "achieved": achieved, "peak": peak,
                 "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
                 "traffic": CORRECTOR_TRAFFIC_BYTES_C2 if (args.config == "C2" and args.scale == 1) else None,
                 "algorithmic_bytes_per_launch": corr_bytes / max(c_n, 1), "launches": c_n,
