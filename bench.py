@@ -28,7 +28,11 @@ CORRECTOR_BYTES_PER_CELL = 120.0   # read U^n, U^{n+1/2}, w
 PREDICTOR_BYTES_PER_CELL = 80.0    # read U^n, write U^{n+1/2}
 # dram__bytes_read.sum + dram__bytes_write.sum of one corrector launch on C2, from the ncu --set full
 # capture summarised in profiles/ (None until captured)
-CORRECTOR_TRAFFIC_BYTES_C2 = 1.551233e9 + 0.649253e9   # profiles/r1_c2_ncu.md
+CORRECTOR_TRAFFIC_BYTES_C2 = 1.492733e9 + 0.646058e9   # profiles/r1_c2_ncu_final.md
+# fp64 instructions (DFMA + DMUL + DADD + DSETP) per cell-update of the two stage kernels, counted on the ncu
+# source page (profiles/r1_c2_ncu_final.md), and the measured DFMA issue rate of this B200 (profiles/r1_fp64_peak.txt)
+FP64_INST_PER_CELL_UPDATE = 236.0 + 380.0
+FP64_PEAK_INST_PER_S = 17.069e12
 
 
 def parse():
@@ -281,6 +285,13 @@ def main():
                 "kernel_ms": {k: round(v[0], 4) for k, v in kt.items()},
                 "kernel_launches": {k: v[1] for k, v in kt.items()},
                 "step_hbm_GBps_at_200B_per_update": 200.0 * cu / (ms * 1e-3) / 1e9}
+    # the second ceiling: the stage kernels are bound by fp64 instruction issue, not by HBM
+    stage_ms = kt["predictor"][0] + kt["corrector"][0]
+    f64 = FP64_INST_PER_CELL_UPDATE * cu / (stage_ms * 1e-3) if stage_ms > 0 else 0.0
+    roofline_fp64 = {"bound": "alu", "kernel": "stage_kernel<0> + stage_kernel<1>", "achieved": f64,
+                     "peak": FP64_PEAK_INST_PER_S, "unit": "fp64 inst/s", "frac": f64 / FP64_PEAK_INST_PER_S,
+                     "inst_per_cell_update": FP64_INST_PER_CELL_UPDATE,
+                     "peak_source": "measured DFMA issue rate (profiles/r1_fp64_peak.txt)"}
 
     if rank != 0:
         if world > 1:
@@ -314,6 +325,7 @@ def main():
                 "d2h_bytes_per_step": state_bytes, "ms_per_step": ms_e2e / args.steps},
         "gpu_launches": int(launches),
         "roofline": roofline,
+        "roofline_fp64": roofline_fp64,
         "cpu_baseline": cpu,
     }
     print(json.dumps(out))
