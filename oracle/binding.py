@@ -51,6 +51,8 @@ def lib():
         L.orc_time_interp.argtypes = [C.c_double] * 4
         L.orc_time_interp.restype = C.c_double
         L.orc_hllc.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_void_p]
+        L.orc_roe.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_void_p]
+        L.orc_set_riemann.argtypes = [C.c_void_p, C.c_int]
         L.orc_minmod.argtypes = [C.c_double, C.c_double]
         L.orc_minmod.restype = C.c_double
         L.orc_get.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p]
@@ -78,6 +80,14 @@ def hllc(WL, WR, d, gamma):
     WR = np.ascontiguousarray(WR, dtype=np.float64)
     F = np.zeros(NV)
     lib().orc_hllc(WL.ctypes.data, WR.ctypes.data, int(d), float(gamma), F.ctypes.data)
+    return F
+
+
+def roe(WL, WR, d, gamma):
+    WL = np.ascontiguousarray(WL, dtype=np.float64)
+    WR = np.ascontiguousarray(WR, dtype=np.float64)
+    F = np.zeros(NV)
+    lib().orc_roe(WL.ctypes.data, WR.ctypes.data, int(d), float(gamma), F.ctypes.data)
     return F
 
 
@@ -156,6 +166,10 @@ class OracleMesh:
 
     def set_reflux(self, on):
         self.L.orc_set_reflux(self.h, int(on))
+
+    def set_riemann(self, solver):
+        """0 / "hllc": HLLC, 1 / "roe": Roe (PAPER.md:126)."""
+        self._chk(self.L.orc_set_riemann(self.h, {"hllc": 0, "roe": 1}.get(solver, solver)))
 
     def advance(self, nsteps, mode=0, dt_fixed=0.0):
         self._chk(self.L.orc_advance(self.h, nsteps, mode, dt_fixed, C.byref(self.t), self.nupd.ctypes.data))

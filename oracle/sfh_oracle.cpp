@@ -20,7 +20,8 @@
 // prolong/restrict identities, 1-D invariance, contact advection, 2nd-order convergence.
 // Parity unpinned by the paper (any reasonable choice passes every pin; fixed only by
 // DESIGN.md): Davis wave speeds (R6), first-order predictor (R8), primitive-variable
-// reconstruction (R11), minmod limiter (R12), CFL speed definition (R16).
+// reconstruction (R11), minmod limiter (R12), CFL speed definition (R16), the entropy-fix width of
+// the Roe solver (R30; the Roe flux itself is pinned by tests/test_oracle_roe_pins.py).
 //
 // Passages followed: PAPER.md:39-44,58 (Euler equations, E of eq. 8); :96 (blocks, levels);
 // :108-120 (time marching, eq. 14-15); :126 (MUSCL, predictor-corrector, HLLC);
@@ -72,6 +73,7 @@ struct Mesh {
   std::vector<int> rslot, fslot;     // [nb*6] -> slot or -1
   std::vector<double> R, FH;         // [slot][NV][8][8]
   int reflux_on = 1;
+  int riemann = 0;                   // 0 HLLC, 1 Roe (PAPER.md:126 names both)
   char err[256] = {0};
 };
 
@@ -231,6 +233,59 @@ void hllc(const double WLin[NV], const double WRin[NV], int d, double gamma, dou
   F[0] = Fn[0]; F[n] = Fn[1]; F[t1] = Fn[2]; F[t2] = Fn[3]; F[4] = Fn[4];
 }
 
+// ------------------------------------------------------------------ Roe ("the method of Roe (1981)"; reading R30)
+// Roe's linearised Riemann solver as in Roe (1981), written with the wave strengths and right
+// eigenvectors of the Roe-averaged state (rho~ = sqrt(rhoL rhoR); u~, v~, w~, H~ weighted by sqrt(rho)):
+//   F = (F_L + F_R)/2 - (1/2) sum_k |lambda_k| alpha_k K_k,
+//   lambda = (u~ - c~, u~, u~, u~, u~ + c~),  c~^2 = (gamma-1)(H~ - |v~|^2/2),
+//   alpha_1,5 = (dP -/+ rho~ c~ du)/(2 c~^2), alpha_2 = drho - dP/c~^2, alpha_3 = rho~ dv, alpha_4 = rho~ dw,
+//   K_1,5 = (1, u~ -/+ c~, v~, w~, H~ -/+ u~ c~), K_2 = (1, u~, v~, w~, |v~|^2/2), K_3 = (0,0,1,0,v~), K_4 = (0,0,0,1,w~).
+// The paper gives no entropy fix; reading R30: Harten's (1983) on the two acoustic waves,
+// |lambda| -> (lambda^2 + delta^2)/(2 delta) where |lambda| < delta, delta = c~/10.  PARITY UNPINNED (delta).
+void roe(const double WLin[NV], const double WRin[NV], int d, double gamma, double F[NV]) {
+  const int n = 1 + d, t1 = 1 + (d + 1) % 3, t2 = 1 + (d + 2) % 3;
+  const double rL = WLin[0], uL = WLin[n], vL = WLin[t1], wL = WLin[t2], PL = WLin[4];
+  const double rR = WRin[0], uR = WRin[n], vR = WRin[t1], wR = WRin[t2], PR = WRin[4];
+  const double EL = PL / (gamma - 1.0) + 0.5 * rL * (uL * uL + vL * vL + wL * wL);
+  const double ER = PR / (gamma - 1.0) + 0.5 * rR * (uR * uR + vR * vR + wR * wR);
+  const double HL = (EL + PL) / rL, HR = (ER + PR) / rR;
+  const double sL = std::sqrt(rL), sR = std::sqrt(rR), sw = sL + sR;
+  const double rt = sL * sR;
+  const double ut = (sL * uL + sR * uR) / sw, vt = (sL * vL + sR * vR) / sw, wt = (sL * wL + sR * wR) / sw;
+  const double Ht = (sL * HL + sR * HR) / sw;
+  const double q2 = ut * ut + vt * vt + wt * wt;
+  const double c2 = (gamma - 1.0) * (Ht - 0.5 * q2);
+  const double ct = std::sqrt(c2);
+  const double dr = rR - rL, du = uR - uL, dv = vR - vL, dw = wR - wL, dP = PR - PL;
+  const double a1 = (dP - rt * ct * du) / (2.0 * c2);
+  const double a2 = dr - dP / c2;
+  const double a3 = rt * dv, a4 = rt * dw;
+  const double a5 = (dP + rt * ct * du) / (2.0 * c2);
+  const double delta = 0.1 * ct;
+  auto fixed = [delta](double lam) {
+    const double al = std::fabs(lam);
+    return al < delta ? (lam * lam + delta * delta) / (2.0 * delta) : al;
+  };
+  const double l1 = fixed(ut - ct), l2 = std::fabs(ut), l5 = fixed(ut + ct);
+  const double K1[NV] = {1.0, ut - ct, vt, wt, Ht - ut * ct};
+  const double K2[NV] = {1.0, ut, vt, wt, 0.5 * q2};
+  const double K3[NV] = {0.0, 0.0, 1.0, 0.0, vt};
+  const double K4[NV] = {0.0, 0.0, 0.0, 1.0, wt};
+  const double K5[NV] = {1.0, ut + ct, vt, wt, Ht + ut * ct};
+  const double FL[NV] = {rL * uL, rL * uL * uL + PL, rL * uL * vL, rL * uL * wL, uL * (EL + PL)};
+  const double FR[NV] = {rR * uR, rR * uR * uR + PR, rR * uR * vR, rR * uR * wR, uR * (ER + PR)};
+  double Fn[NV];
+  for (int c = 0; c < NV; ++c)
+    Fn[c] = 0.5 * (FL[c] + FR[c]) -
+            0.5 * (l1 * a1 * K1[c] + l2 * (a2 * K2[c] + a3 * K3[c] + a4 * K4[c]) + l5 * a5 * K5[c]);
+  F[0] = Fn[0]; F[n] = Fn[1]; F[t1] = Fn[2]; F[t2] = Fn[3]; F[4] = Fn[4];
+}
+
+inline void riemann_flux(const Mesh& m, const double WL[NV], const double WR[NV], int d, double F[NV]) {
+  if (m.riemann == 1) roe(WL, WR, d, m.cfg.gamma, F);
+  else hllc(WL, WR, d, m.cfg.gamma, F);
+}
+
 inline int fidx(int v, int f, int a, int b) { return ((v * 9 + f) * N + b) * N + a; }  // face f=0..8, tangential (a fastest)
 
 inline void cell_of(int d, int c, int a, int b, int& i, int& j, int& k) {
@@ -261,7 +316,7 @@ void predictor_block(Mesh& m, int b, double dt) {
       cell_of(d, f, ta, tb, i1, j1, k1);
       double WL[NV], WR[NV], Ff[NV];
       for (int v = 0; v < NV; ++v) { WL[v] = W[gidx(v, i0, j0, k0)]; WR[v] = W[gidx(v, i1, j1, k1)]; }
-      hllc(WL, WR, d, gamma, Ff);
+      riemann_flux(m, WL, WR, d, Ff);
       for (int v = 0; v < NV; ++v) F[d * NV * 9 * N * N + fidx(v, f, ta, tb)] = Ff[v];
     }
   const double lam = 0.5 * dt / h;
@@ -300,7 +355,7 @@ void corrector_block(Mesh& m, int b, double dt) {
         WL[v] = w[1] + 0.5 * dl;
         WR[v] = w[2] - 0.5 * dr;
       }
-      hllc(WL, WR, d, gamma, Ff);
+      riemann_flux(m, WL, WR, d, Ff);
       for (int v = 0; v < NV; ++v) F[d * NV * 9 * N * N + fidx(v, f, ta, tb)] = Ff[v];
     }
   const double lam = dt / h;
@@ -533,6 +588,7 @@ int64_t orc_state_doubles(const Mesh* m) { return m->nb * BLK; }
 
 int orc_bind(Mesh* m, double* U0, double* U1, double* U2) { m->U[0] = U0; m->U[1] = U1; m->U[2] = U2; return 0; }
 void orc_set_reflux(Mesh* m, int on) { m->reflux_on = on; }
+int orc_set_riemann(Mesh* m, int solver) { if (solver != 0 && solver != 1) return -1; m->riemann = solver; return 0; }
 int orc_is_leaf(const Mesh* m, int64_t b) { return m->leaf[b]; }
 double orc_cell_width(const Mesh* m, int l) { return h_of(*m, l); }
 int64_t orc_num_registers(const Mesh* m, int which) {
@@ -573,6 +629,7 @@ double orc_max_speed(Mesh* m, int level, int copy) { return max_speed_level(*m, 
 int orc_substep_exponent(double dtH, double dt_cfl_h) { return substep_exponent(dtH, dt_cfl_h); }
 double orc_time_interp(double U0, double Uh, double U1, double tau) { return time_interp(U0, Uh, U1, tau); }
 void orc_hllc(const double* WL, const double* WR, int d, double gamma, double* F) { hllc(WL, WR, d, gamma, F); }
+void orc_roe(const double* WL, const double* WR, int d, double gamma, double* F) { roe(WL, WR, d, gamma, F); }
 double orc_minmod(double a, double b) { return minmod(a, b); }
 int orc_get(Mesh* m, int level, int I, int J, int K, int which, double* out) {   // sync-mode accessor
   std::vector<Src> srcs(m->nlev, Src{0, which, 0.0});
