@@ -42,6 +42,8 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="C2", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--scale", type=int, default=1, help="shrink the base grid (debugging only; invalid as a bench value)")
+    ap.add_argument("--riemann", default="hllc", choices=["hllc", "roe"],
+                    help="Riemann solver (PAPER.md:126); the paper's benchmarks and BASELINE.json use HLLC")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -139,7 +141,7 @@ def cell_updates(census, nupd):
     return float(sum(512 * c * int(n) for c, n in zip(census, nupd)))
 
 
-def oracle_sample(config, scale_hint):
+def oracle_sample(config, scale_hint, riemann="hllc"):
     """The oracle on a bounded sample of the same workload: the same recipe on a smaller base grid."""
     sys.path.insert(0, os.path.join(ROOT, "tests"))
     from helpers import oracle_for
@@ -147,6 +149,7 @@ def oracle_sample(config, scale_hint):
     sample_scale = {"C1": 1, "C2": 1, "C3": 2, "C4": 2, "C5": 4}[config] * max(1, scale_hint)
     p = make_config(config, sample_scale)
     o = oracle_for(p)
+    o.set_riemann(riemann)
     o.restrict_all(0)
     n = p.nb0[0] * 8
     what = "%s recipe at base %d^3 (1/%d of the base cells), blocks/level %s" % (config, n, sample_scale ** 3, p.census())
@@ -157,7 +160,7 @@ def run_reference(args):
     """--impl reference: the CPU oracle as it stands, on the host cores (rank 0 only)."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
-    p, o, what = oracle_sample(args.config, args.scale)
+    p, o, what = oracle_sample(args.config, args.scale, args.riemann)
     cores = len(os.sched_getaffinity(0))
     for _ in range(args.warmup):
         o.advance(1, p.mode)
@@ -172,7 +175,8 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": p.notes.get("workload", p.name), "config": args.config, "sample": sample},
+        "config": {"workload": p.notes.get("workload", p.name), "config": args.config, "sample": sample,
+                   "riemann": args.riemann},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
@@ -202,6 +206,7 @@ def main():
     p = make_config(args.config, args.scale)
     census = p.census()
     g = sfh.Mesh.from_problem(p, device=dev)
+    g.set_riemann(args.riemann)
     U0 = torch.from_numpy(p.U).pin_memory()
     Ud = U0.to(dev)
 
@@ -279,7 +284,8 @@ def main():
     achieved = corr_bytes / (c_ms * 1e-3) / 1e9 if c_ms > 0 else 0.0
     roofline = {"bound": "hbm", "kernel": "stage_kernel<1> (corrector)", "achieved": achieved, "peak": peak,
                 "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
-                "traffic": CORRECTOR_TRAFFIC_BYTES_C2 if (args.config == "C2" and args.scale == 1) else None,
+                "traffic": CORRECTOR_TRAFFIC_BYTES_C2 if (args.config == "C2" and args.scale == 1 and
+                                                          args.riemann == "hllc") else None,
                 "algorithmic_bytes_per_launch": corr_bytes / max(c_n, 1), "launches": c_n,
                 "avg_launch_ms": c_ms / max(c_n, 1),
                 "kernel_ms": {k: round(v[0], 4) for k, v in kt.items()},
@@ -292,6 +298,8 @@ def main():
                      "peak": FP64_PEAK_INST_PER_S, "unit": "fp64 inst/s", "frac": f64 / FP64_PEAK_INST_PER_S,
                      "inst_per_cell_update": FP64_INST_PER_CELL_UPDATE,
                      "peak_source": "measured DFMA issue rate (profiles/r1_fp64_peak.txt)"}
+    if args.riemann != "hllc":
+        roofline_fp64 = None          # the instruction count was taken with the HLLC kernels
 
     if rank != 0:
         if world > 1:
@@ -302,7 +310,7 @@ def main():
     if world == 1 and not args.no_cpu_baseline:
         # the oracle as it stands on this box's host cores, on a bounded sample: whole coarse steps of
         # the same recipe (at a smaller base grid for the large configs) until ~12 s have passed
-        ps, o, what = oracle_sample(args.config, args.scale)
+        ps, o, what = oracle_sample(args.config, args.scale, args.riemann)
         tt, nst = time.perf_counter(), 0
         while nst < max(args.steps, 1) and (nst == 0 or time.perf_counter() - tt < 12.0):
             o.advance(1, ps.mode)
@@ -316,6 +324,7 @@ def main():
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": p.notes.get("workload", p.name), "config": args.config, "scale": args.scale,
+                   "riemann": args.riemann,
                    "blocks_per_level": census, "updates_per_level": [int(x) for x in nupd],
                    "mode": "adaptive" if p.mode else "synchronous",
                    "l2": "inputs larger than L2 (one state copy %.0f MB vs 126 MB L2)" % (state_bytes / 1e6),

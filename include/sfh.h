@@ -71,6 +71,15 @@ int sfh_create_mesh(const sfh_config* cfg, int64_t nblocks, const int32_t* level
                     sfh_mesh** out);
 int sfh_destroy_mesh(sfh_mesh* m);
 
+/* Riemann solver of the predictor and corrector fluxes: "either the HLLC scheme (Toro et al. 1994) or the
+ * method of Roe (1981)".  SFH_RIEMANN_HLLC is the default (the paper's benchmarks use it,
+ * PAPER.md:536); SFH_RIEMANN_ROE is Roe's linearised solver with Harten's entropy fix on the acoustic
+ * waves (reading R30).  Host-side switch, takes effect at the next stage launch; any other
+ * value gives SFH_EINVAL. */
+#define SFH_RIEMANN_HLLC 0
+#define SFH_RIEMANN_ROE 1
+int sfh_set_riemann(sfh_mesh* m, int solver);
+
 int64_t sfh_num_blocks(const sfh_mesh* m);
 /* Blocks of `level` occupy library slots [first, first+count). */
 int sfh_level_range(const sfh_mesh* m, int level, int64_t* first, int64_t* count);

@@ -53,6 +53,7 @@ def load_library(path=None):
     sig = {
         "sfh_create_mesh": (i32, [C.POINTER(SfhConfig), i64, vp, vp, C.POINTER(vp)]),
         "sfh_destroy_mesh": (i32, [vp]),
+        "sfh_set_riemann": (i32, [vp, i32]),
         "sfh_num_blocks": (i64, [vp]),
         "sfh_level_range": (i32, [vp, i32, C.POINTER(i64), C.POINTER(i64)]),
         "sfh_block_order": (i32, [vp, vp]),
@@ -163,6 +164,10 @@ class Mesh:
 
     def launch_count(self):
         return self.L.sfh_launch_count(self.h)
+
+    def set_riemann(self, solver):
+        """0 / "hllc" or 1 / "roe" (PAPER.md:126)."""
+        self._chk(self.L.sfh_set_riemann(self.h, {"hllc": 0, "roe": 1}.get(solver, solver)))
 
     # ---- device
     def bind(self):

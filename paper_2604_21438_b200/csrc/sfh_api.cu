@@ -19,6 +19,7 @@ void set_error(const std::string& s) { g_err = s; }
 struct sfh_mesh {
   HostMesh hm;
   bool bound = false;
+  int riemann = SFH_RIEMANN_HLLC;
   char* dev_tables = nullptr;
   int32_t *d_face_src = nullptr, *d_fslot = nullptr, *d_nbr27 = nullptr, *d_parent = nullptr, *d_child0 = nullptr,
           *d_coord = nullptr, *d_cf_block = nullptr, *d_cf_face = nullptr, *d_fh_src = nullptr,
@@ -214,6 +215,7 @@ int stage_level(sfh_mesh* m, int l, int stage, Dt dt, cudaStream_t st) {
   p.dt_dev = dt.dev; p.dt = dt.host; p.h = hm.h[l]; p.gamma = hm.cfg.gamma;
   p.first = int(hm.lev_first[l]); p.count = int(hm.lev_count[l]);
   p.use_regs = stage == 1 && (hm.cf_count[l] > 0 || hm.reflux_count[l] > 0);
+  p.riemann = m->riemann;
   p.bmax = stage == 1 ? m->bmax : nullptr;
   if (stage == 1) m->bmax_pending[l] = true;
   {
@@ -390,6 +392,13 @@ int sfh_destroy_mesh(sfh_mesh* m) {
   for (cudaEvent_t e : m->event_pool) cudaEventDestroy(e);
   if (m->dev_tables) cudaFree(m->dev_tables);
   delete m;
+  return SFH_OK;
+}
+
+int sfh_set_riemann(sfh_mesh* m, int solver) {
+  if (!m) return fail(SFH_EINVAL, "null mesh");
+  if (solver != SFH_RIEMANN_HLLC && solver != SFH_RIEMANN_ROE) return fail(SFH_EINVAL, "unknown Riemann solver");
+  m->riemann = solver;
   return SFH_OK;
 }
 

@@ -182,4 +182,52 @@ __device__ __forceinline__ void hllc_flux(double rL, double uL, double vL, doubl
   Fn[4] = fma(s, fma(g, EP + rdS, rdS), u * EP);
 }
 
+// Roe flux ("the method of Roe (1981)"; reading R30) in the face frame, same conventions as
+// hllc_flux.  Roe averages weighted by sqrt(rho) (1/sqrt(rho) from the hardware seed: sqrt(rho) = rho rsqrt(rho),
+// sqrt(rho) H = (E + P) rsqrt(rho)); wave strengths alpha_k and eigenvectors K_k of the averaged state;
+// Harten's entropy fix on the two acoustic waves, delta = c~/10;
+//   F = ((F_L + F_R) - sum_k |lambda_k| alpha_k K_k) / 2,
+// with the five dissipation components summed wave by wave: b_k = |lambda_k| alpha_k,
+//   D = (b1+b2+b5, b1 (u-c) + b2 u + b5 (u+c), D0 v + b3, D0 w + b4, b1 (H - u c) + b2 q^2/2 + b3 v + b4 w + b5 (H + u c)).
+template <bool HAVE_E>
+__device__ __forceinline__ void roe_flux(double rL, double uL, double vL, double wL, double PL, double EL, double rR,
+                                         double uR, double vR, double wR, double PR, double ER, double gm1, double igm1,
+                                         double Fn[5]) {
+  const double eL = HAVE_E ? EL : fma(PL, igm1, (0.5 * rL) * fma(wL, wL, fma(vL, vL, uL * uL)));
+  const double eR = HAVE_E ? ER : fma(PR, igm1, (0.5 * rR) * fma(wR, wR, fma(vR, vR, uR * uR)));
+  const double iL = rsqrt_fast(rL), iR = rsqrt_fast(rR);
+  const double sL = rL * iL, sR = rR * iR;
+  const double iw = rcp_fast(sL + sR);
+  const double aL = sL * iw, aR = sR * iw;
+  const double ut = fma(aL, uL, aR * uR), vt = fma(aL, vL, aR * vR), wt = fma(aL, wL, aR * wR);
+  const double epL = eL + PL, epR = eR + PR;
+  const double Ht = fma(epL, iL, epR * iR) * iw;
+  const double q2 = fma(wt, wt, fma(vt, vt, ut * ut));
+  const double c2 = gm1 * fma(-0.5, q2, Ht);
+  const double ic = rsqrt_fast(c2), ct = c2 * ic, ic2 = ic * ic;
+  const double rt = sL * sR;
+  const double dr = rR - rL, du = uR - uL, dv = vR - vL, dw = wR - wL, dP = PR - PL;
+  const double rcu = (rt * ct) * du, hic2 = 0.5 * ic2;
+  const double a1 = (dP - rcu) * hic2, a5 = (dP + rcu) * hic2;
+  const double a2 = fma(-dP, ic2, dr);
+  const double delta = 0.1 * ct, idel = 10.0 * ic;
+  const double lm = ut - ct, lp = ut + ct;
+  const double fm = 0.5 * fma(lm * lm, idel, delta), fp = 0.5 * fma(lp * lp, idel, delta);
+  const double l1 = fabs(lm) < delta ? fm : fabs(lm);
+  const double l5 = fabs(lp) < delta ? fp : fabs(lp);
+  const double l2 = fabs(ut);
+  const double b1 = l1 * a1, b5 = l5 * a5, b2 = l2 * a2, b3 = l2 * (rt * dv), b4 = l2 * (rt * dw);
+  const double D0 = (b1 + b2) + b5;
+  const double D1 = fma(b5, lp, fma(b1, lm, b2 * ut));
+  const double D2 = fma(D0, vt, b3), D3 = fma(D0, wt, b4);
+  const double uc = ut * ct;
+  const double D4 = fma(b5, Ht + uc, fma(b1, Ht - uc, fma(b2, 0.5 * q2, fma(b3, vt, b4 * wt))));
+  const double mL = rL * uL, mR = rR * uR;
+  Fn[0] = 0.5 * ((mL + mR) - D0);
+  Fn[1] = 0.5 * ((fma(mL, uL, PL) + fma(mR, uR, PR)) - D1);
+  Fn[2] = 0.5 * (fma(mL, vL, mR * vR) - D2);
+  Fn[3] = 0.5 * (fma(mL, wL, mR * wR) - D3);
+  Fn[4] = 0.5 * (fma(uL, epL, uR * epR) - D4);
+}
+
 }  // namespace sfh

@@ -139,11 +139,20 @@ __device__ __noinline__ void store_regs(const int32_t* face_src, const int32_t* 
 // A half pencil: faces f0 .. f0+4 and cells f0 .. f0+3, f0 = 0 or 4.  Face f lies between cells f-1 and f.
 // The loops are unrolled by two so that the carried cell/face state ping-pongs between registers.
 
-// predictor: first-order HLLC on the cell-centred states (reading R8)
-template <int D>
+// flux of the cell-centred states w0 | w1 = (rho, u, v, w, P, c_s, E) with Riemann solver RS (0 HLLC, 1 Roe)
+template <int RS>
+__device__ __forceinline__ void cell_flux(const double w0[7], const double w1[7], double gm1, double igm1, double F[5]) {
+  if (RS == 0)
+    hllc_flux<true>(w0[0], w0[1], w0[2], w0[3], w0[4], w0[5], w0[6], w1[0], w1[1], w1[2], w1[3], w1[4], w1[5], w1[6], igm1, F);
+  else
+    roe_flux<true>(w0[0], w0[1], w0[2], w0[3], w0[4], w0[6], w1[0], w1[1], w1[2], w1[3], w1[4], w1[6], gm1, igm1, F);
+}
+
+// predictor: first-order fluxes of the cell-centred states (reading R8)
+template <int RS, int D>
 __device__ __forceinline__ void walk_predictor(const double* __restrict__ Wl, double* __restrict__ dF, int a, int b,
-                                               int f0, double igm1, uint32_t bar_empty, uint32_t par_empty,
-                                               bool wait_empty) {
+                                               int f0, double gm1, double igm1, uint32_t bar_empty,
+                                               uint32_t par_empty, bool wait_empty) {
   constexpr int TS = Cfg<0>::TS;
   double w0[7], w1[7], wn[7], F0[5], F1[5];
   if (D == 0) {
@@ -153,8 +162,7 @@ __device__ __forceinline__ void walk_predictor(const double* __restrict__ Wl, do
     load_cell<7, D>(Wl, cell_pos<TS, D>(f0 - 1, a, b), w0);
     load_cell<7, D>(Wl, cell_pos<TS, D>(f0, a, b), w1);
   }
-  hllc_flux<true>(w0[0], w0[1], w0[2], w0[3], w0[4], w0[5], w0[6], w1[0], w1[1], w1[2], w1[3], w1[4], w1[5], w1[6],
-                  igm1, F0);                        // face f0
+  cell_flux<RS>(w0, w1, gm1, igm1, F0);             // face f0
   if (wait_empty) mbar_wait(bar_empty, par_empty);  // the update of the block before has read dF
 #pragma unroll
   for (int f = f0 + 1; f < f0 + 4; f += 2) {        // faces f (cells f-1 | f) and f+1 (cells f | f+1)
@@ -164,13 +172,11 @@ __device__ __forceinline__ void walk_predictor(const double* __restrict__ Wl, do
     } else {
       load_cell<7, D>(Wl, cell_pos<TS, D>(f, a, b), w0);
     }
-    hllc_flux<true>(w1[0], w1[1], w1[2], w1[3], w1[4], w1[5], w1[6], w0[0], w0[1], w0[2], w0[3], w0[4], w0[5], w0[6],
-                    igm1, F1);
+    cell_flux<RS>(w1, w0, gm1, igm1, F1);
     store_df<D>(dF, f - 1, a, b, F1, F0);
     if (D == 0) load_two<0, 0>(Wl, f + 1, a, b, w1, wn);
     else load_cell<7, D>(Wl, cell_pos<TS, D>(f + 1, a, b), w1);
-    hllc_flux<true>(w0[0], w0[1], w0[2], w0[3], w0[4], w0[5], w0[6], w1[0], w1[1], w1[2], w1[3], w1[4], w1[5], w1[6],
-                    igm1, F0);
+    cell_flux<RS>(w0, w1, gm1, igm1, F0);
     store_df<D>(dF, f, a, b, F0, F1);
   }
 }
@@ -190,12 +196,18 @@ __device__ __forceinline__ void limited_states(const double wc[5], const double 
     Lnext[v] = fma(k, m, wc[v]);
   }
 }
+template <int RS>
 __device__ __forceinline__ void corrector_flux(const double WLs[5], const double WRs[5], double gamma, double igm1,
                                                double Fn[5]) {
-  const double cL = sound_speed(gamma, WLs[4], WLs[0]);
-  const double cR = sound_speed(gamma, WRs[4], WRs[0]);
-  hllc_flux<false>(WLs[0], WLs[1], WLs[2], WLs[3], WLs[4], cL, 0.0, WRs[0], WRs[1], WRs[2], WRs[3], WRs[4], cR, 0.0,
-                   igm1, Fn);
+  if (RS == 0) {
+    const double cL = sound_speed(gamma, WLs[4], WLs[0]);
+    const double cR = sound_speed(gamma, WRs[4], WRs[0]);
+    hllc_flux<false>(WLs[0], WLs[1], WLs[2], WLs[3], WLs[4], cL, 0.0, WRs[0], WRs[1], WRs[2], WRs[3], WRs[4], cR, 0.0,
+                     igm1, Fn);
+  } else {
+    roe_flux<false>(WLs[0], WLs[1], WLs[2], WLs[3], WLs[4], 0.0, WRs[0], WRs[1], WRs[2], WRs[3], WRs[4], 0.0,
+                    gamma - 1.0, igm1, Fn);
+  }
 }
 
 // ---- direction-generic corrector walk ------------------------------------------------------------------
@@ -221,6 +233,7 @@ __device__ __forceinline__ void walk_geom(int a, int b, int f0, WalkGeom& g) {
 __device__ __forceinline__ void load_cell_g(const double* __restrict__ Wl, int o, const int ov[3], double w[5]) {
   w[0] = Wl[o]; w[1] = Wl[o + ov[0]]; w[2] = Wl[o + ov[1]]; w[3] = Wl[o + ov[2]]; w[4] = Wl[o + 4 * CVS];
 }
+template <int RS>
 __device__ __forceinline__ void walk_corrector_generic(const double* __restrict__ Wl, double* __restrict__ dF,
                                                        const WalkGeom& g, int D, int a, int b, int f0, double gamma,
                                                        double igm1, const StageParams& p, int blk, double dt,
@@ -240,7 +253,7 @@ __device__ __forceinline__ void walk_corrector_generic(const double* __restrict_
 #pragma unroll
     for (int v = 0; v < 5; ++v) dn[v] = wn[v] - wc[v];
     limited_states(wc, dn, dp, R, Ln);                        // right state of this face, left state of the next
-    corrector_flux(L, R, gamma, igm1, (ff & 1) ? Fb : Fa);
+    corrector_flux<RS>(L, R, gamma, igm1, (ff & 1) ? Fb : Fa);
 #pragma unroll
     for (int v = 0; v < 5; ++v) L[v] = Ln[v];
     if (ff == 0) {
@@ -411,7 +424,7 @@ __device__ __forceinline__ void store_block(const double u[HC][NV], double gm1, 
 //   full[d]    all walkers have stored the flux differences into buffer d = it % NDF (and are done with
 //              the staging buffer, which the helpers then re-stage)
 //   empty[d]   the helpers have consumed flux-difference buffer d
-template <int STAGE>
+template <int STAGE, int RS>
 __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_constant__ TensorMaps tm,
                                                                   const StageParams p) {
   using C = Cfg<STAGE>;
@@ -484,12 +497,12 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
       t1 = clock64(); tw[0] += t1 - t0;
 #endif
       if (STAGE == 0) {
-        if (D == 0) walk_predictor<0>(Wl, dF, a, b, f0, igm1, empty(d), pe, we);
-        else if (D == 1) walk_predictor<1>(Wl, dF, a, b, f0, igm1, empty(d), pe, we);
-        else walk_predictor<2>(Wl, dF, a, b, f0, igm1, empty(d), pe, we);
+        if (D == 0) walk_predictor<RS, 0>(Wl, dF, a, b, f0, gm1, igm1, empty(d), pe, we);
+        else if (D == 1) walk_predictor<RS, 1>(Wl, dF, a, b, f0, gm1, igm1, empty(d), pe, we);
+        else walk_predictor<RS, 2>(Wl, dF, a, b, f0, gm1, igm1, empty(d), pe, we);
       } else {
         const int blk = blk0 + it * stride;
-        walk_corrector_generic(Wl, dF, geom, D, a, b, f0, gamma, igm1, p, blk, dt, empty(d), pe, we);
+        walk_corrector_generic<RS>(Wl, dF, geom, D, a, b, f0, gamma, igm1, p, blk, dt, empty(d), pe, we);
       }
       __syncwarp();
       if ((tid & 31) == 0) mbar_arrive(full(d));
@@ -610,11 +623,16 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
 
 static int g_stage_ctas = 148;   // persistent grid: one CTA per SM (set by configure_kernels)
 
+template <int STAGE, int RS>
+static cudaError_t configure_one() {
+  return cudaFuncSetAttribute(stage_kernel<STAGE, RS>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<STAGE>::SMEM);
+}
+
 cudaError_t configure_kernels() {
-  cudaError_t e = cudaFuncSetAttribute(stage_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<0>::SMEM);
-  if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(stage_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<1>::SMEM);
-  if (e != cudaSuccess) return e;
+  cudaError_t e;
+  if ((e = configure_one<0, 0>()) != cudaSuccess || (e = configure_one<1, 0>()) != cudaSuccess ||
+      (e = configure_one<0, 1>()) != cudaSuccess || (e = configure_one<1, 1>()) != cudaSuccess)
+    return e;
   int dev = 0, sms = 0;
   if (cudaGetDevice(&dev) == cudaSuccess &&
       cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
@@ -625,8 +643,13 @@ cudaError_t configure_kernels() {
 cudaError_t launch_stage(int stage, const TensorMaps& tm, const StageParams& p, cudaStream_t st) {
   if (p.count <= 0) return cudaSuccess;
   const int grid = p.count < g_stage_ctas ? p.count : g_stage_ctas;
-  if (stage == 0) stage_kernel<0><<<grid, STAGE_THREADS, Cfg<0>::SMEM, st>>>(tm, p);
-  else stage_kernel<1><<<grid, STAGE_THREADS, Cfg<1>::SMEM, st>>>(tm, p);
+  if (p.riemann == 0) {
+    if (stage == 0) stage_kernel<0, 0><<<grid, STAGE_THREADS, Cfg<0>::SMEM, st>>>(tm, p);
+    else stage_kernel<1, 0><<<grid, STAGE_THREADS, Cfg<1>::SMEM, st>>>(tm, p);
+  } else {
+    if (stage == 0) stage_kernel<0, 1><<<grid, STAGE_THREADS, Cfg<0>::SMEM, st>>>(tm, p);
+    else stage_kernel<1, 1><<<grid, STAGE_THREADS, Cfg<1>::SMEM, st>>>(tm, p);
+  }
   return cudaGetLastError();
 }
 

@@ -23,6 +23,7 @@ struct StageParams {
   double gamma;
   int first, count;      // slot range of the level
   int use_regs;          // corrector: the level has flux-register faces
+  int riemann;           // 0 HLLC, 1 Roe
   double* bmax;          // corrector: per-block maximum CFL speed of U^{n+1} (or null)
 };
 

@@ -20,7 +20,7 @@ def gaussian_random_field(n, slope, seed):
     amp[band] = k2[band] ** (slope / 4.0)          # sqrt(P) = k^(slope/2) = (k^2)^(slope/4)
     fk *= amp
     del amp, k2, band
-    f = np.fft.irfftn(fk, s=(n, n, n))
+    f = np.fft.irfftn(fk, s=(n, n, n), axes=(0, 1, 2))
     del fk
     f -= f.mean()
     f /= f.std()

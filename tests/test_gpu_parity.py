@@ -262,3 +262,39 @@ def test_status_counts_bad_cells_and_e2e_host_path():
     g.advance_host(hin, hout, 2, 0)
     assert torch.equal(hout, ref.reshape(hout.shape))
     assert g.launch_count() > 0
+
+
+# ------------------------------------------------------------------ Roe solver (R30)
+@pytest.mark.parametrize("name", ["C1", "C2/4", "C4/4", "C5/8", "amr-small", "amr-outflow", "ragged"])
+def test_roe_solver_parity(name):
+    """The same runs with sfh_set_riemann(SFH_RIEMANN_ROE) on both sides: one step at 1e-12, the
+    configured run (>= 10 steps) at 1e-10, equal sub-cycling counts."""
+    p = PROBLEMS[name]()
+    o, g = both(p)
+    o.set_riemann("roe")
+    g.set_riemann("roe")
+    o.advance(1, p.mode)
+    g.advance(1, p.mode)
+    assert abs(g.t.value - o.t.value) <= TOLDT * o.t.value
+    compare(o, g, p.gamma, TOL1)
+    n = max(p.nsteps, 10) - 1
+    o.advance(n, p.mode)
+    g.advance(n, p.mode)
+    assert np.array_equal(o.nupd, g.nupd), (o.nupd, g.nupd)
+    assert o.status() == 0 and g.status() == 0
+    compare(o, g, p.gamma, TOL10)
+    # and the switch really changes the scheme
+    o2, g2 = both(p)
+    g2.advance(1, p.mode)
+    g3 = gpu_for(p)
+    g3.restrict_all(0)
+    g3.set_riemann("roe")
+    g3.advance(1, p.mode)
+    assert not np.array_equal(g2.get_state().cpu().numpy(), g3.get_state().cpu().numpy())
+
+
+def test_set_riemann_rejects_unknown_solver():
+    p = PROBLEMS["one-block"]()
+    g = gpu_for(p)
+    with pytest.raises(sfh.SfhError):
+        g.set_riemann(7)
