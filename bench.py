@@ -141,6 +141,22 @@ def cell_updates(census, nupd):
     return float(sum(512 * c * int(n) for c, n in zip(census, nupd)))
 
 
+def max_over_ranks(ms, world, device="cpu"):
+    """The job's time is the slowest rank's (device time, max over ranks)."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(cu_per_rank, ms, world):
+    """N independent replicas of the same workload: the units all ranks processed / the time."""
+    return world * cu_per_rank / (ms * 1e-3)
+
+
 def oracle_sample(config, scale_hint, riemann="hllc"):
     """The oracle on a bounded sample of the same workload: the same recipe on a smaller base grid."""
     sys.path.insert(0, os.path.join(ROOT, "tests"))
@@ -250,11 +266,8 @@ def main():
     nupd = g.nupd.copy()
     cu = cell_updates(census, nupd)
     bad = g.status()
-    if world > 1:
-        t = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * cu / (ms * 1e-3)
+    ms = max_over_ranks(ms, world, dev)
+    value = whole_job_value(cu, ms, world)
 
     # ---- end to end through sfh_advance_host: pinned host buffers, H2D and D2H every step
     reset()
@@ -271,10 +284,7 @@ def main():
     barrier()
     ms_e2e = e0.elapsed_time(e1)
     cu_e2e = cell_updates(census, g.nupd)
-    if world > 1:
-        t = torch.tensor([ms_e2e], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_e2e = float(t.item())
+    ms_e2e = max_over_ranks(ms_e2e, world, dev)
     state_bytes = int(U0.numel() * 8)
 
     # ---- roofline of the dominant kernel (the corrector stage), CUDA events around each launch
@@ -330,7 +340,7 @@ def main():
                    "l2": "inputs larger than L2 (one state copy %.0f MB vs 126 MB L2)" % (state_bytes / 1e6),
                    "parallelism": "replicas x%d" % world, "bad_cells": int(bad), "bad_cells_after_warmup": int(bad_warm)},
         "clocks": clocks,
-        "e2e": {"value": world * cu_e2e / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": state_bytes,
+        "e2e": {"value": whole_job_value(cu_e2e, ms_e2e, world), "unit": UNIT, "h2d_bytes_per_step": state_bytes,
                 "d2h_bytes_per_step": state_bytes, "ms_per_step": ms_e2e / args.steps},
         "gpu_launches": int(launches),
         "roofline": roofline,

@@ -99,6 +99,11 @@ def test_mesh_validation_rejects_bad_trees():
     with pytest.raises(sfh.SfhError) as e:
         sfh.Mesh(t.nb0, t.max_level, ((0, 1),) * 3, (1.0, 1.0, 1.0), 1.4, 0.4, level, ijk, **kw)
     assert e.value.code == -1
+    # empty block list: a defined error, not a crash
+    with pytest.raises(sfh.SfhError) as e:
+        sfh.Mesh((1, 1, 1), 0, ((0, 0),) * 3, (1.0, 1.0, 1.0), 1.4, 0.4, np.zeros(0, np.int32),
+                 np.zeros((0, 3), np.int32), **kw)
+    assert e.value.code == -1
 
 
 def test_compute_calls_fail_loudly_without_binding():

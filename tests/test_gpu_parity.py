@@ -52,7 +52,15 @@ PROBLEMS = {
     "amr-outflow": lambda: problem_from_tree(small_amr_tree(periodic=(False, True, False), offset=(-1, 0, 1)), mode=1),
     "ragged": lambda: problem_from_tree(uniform_tree((3, 1, 5)), gamma=1.4),
     "one-block": lambda: problem_from_tree(uniform_tree((1, 1, 1))),
+    "empty-levels": lambda: empty_levels_problem(),
 }
+
+
+def empty_levels_problem():
+    """max_level = 3 declared, levels 2 and 3 hold no block (degenerate case of the level driver)."""
+    p = problem_from_tree(small_amr_tree(max_level=1), mode=1)
+    p.max_level = 3
+    return p
 
 
 @pytest.mark.parametrize("name", list(PROBLEMS))
