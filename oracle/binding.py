@@ -58,6 +58,7 @@ def lib():
         L.orc_get.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p]
         L.orc_advance.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.POINTER(C.c_double), C.c_void_p]
         L.orc_status.argtypes = [C.c_void_p, C.c_int]
+        L.orc_refine_indicator.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_void_p]
         L.orc_status.restype = C.c_int64
         _lib = L
     return _lib
@@ -177,6 +178,12 @@ class OracleMesh:
 
     def status(self, copy=0):
         return self.L.orc_status(self.h, copy)
+
+    def refine_indicator(self, criterion=0, which=0, G=1.0):
+        """Per-block refinement indicator (0: eq. 33-34 curvature, 1: h / Jeans length); ghosts must be filled."""
+        out = np.zeros(self.nb)
+        self._chk(self.L.orc_refine_indicator(self.h, which, criterion, float(G), out.ctypes.data))
+        return out
 
     def get(self, level, I, J, K, which=0):
         out = np.zeros(NV)

@@ -669,4 +669,51 @@ int64_t orc_status(Mesh* m, int copy) {   // cells with rho<=0 or P<=0 (or NaN),
   return bad;
 }
 
+// ------------------------------------------------------------------ refinement indicators
+// criterion 0, eq. (33)-(34) PAPER.md:277-285: per block, max over interior cells of max(E(rho), E(P)),
+//   E(q) = |d2x q + d2y q + d2z q| h^2 / q  with centred second differences (the h^2 cancels);
+//   a block is refined where this is >= 1e-2 (the comparison is the caller's).
+// criterion 1, "the Jeans length is resolved by at least 8 cells": per block, max over
+//   interior cells of h / lambda_J, lambda_J = c_s sqrt(pi / (G rho)), c_s^2 = gamma P / rho (reading R31);
+//   a block is refined where this is > 1/8.
+// Reads the ghost cells (one layer, faces) of copy `which`: call orc_fill_ghosts first.
+int orc_refine_indicator(Mesh* m, int which, int criterion, double G, double* out) {
+  if (which < 0 || which > 2 || (criterion != 0 && criterion != 1)) return -1;
+  const double gamma = m->cfg.gamma;
+  const double pi = 3.14159265358979323846;
+  for (int64_t b = 0; b < m->nb; ++b) {
+    const double* U = m->U[which] + b * BLK;
+    const double h = h_of(*m, m->lev[b]);
+    auto prim = [&](int i, int j, int k, double& rho, double& P) {
+      double u[NV], w[NV];
+      for (int v = 0; v < NV; ++v) u[v] = U[gidx(v, i, j, k)];
+      cons_to_prim(u, gamma, w);
+      rho = w[0]; P = w[4];
+    };
+    double best = 0.0;
+    for (int k = 0; k < N; ++k) for (int j = 0; j < N; ++j) for (int i = 0; i < N; ++i) {
+      double r0, P0;
+      prim(i, j, k, r0, P0);
+      double val;
+      if (criterion == 0) {
+        double lr = 0.0, lP = 0.0;
+        for (int d = 0; d < 3; ++d) {
+          double rp, Pp, rm, Pm;
+          prim(i + (d == 0), j + (d == 1), k + (d == 2), rp, Pp);
+          prim(i - (d == 0), j - (d == 1), k - (d == 2), rm, Pm);
+          lr += (rp - 2.0 * r0) + rm;
+          lP += (Pp - 2.0 * P0) + Pm;
+        }
+        val = std::max(std::fabs(lr) / r0, std::fabs(lP) / P0);
+      } else {
+        const double cs = std::sqrt(gamma * P0 / r0);
+        val = h / (cs * std::sqrt(pi / (G * r0)));
+      }
+      if (val > best) best = val;
+    }
+    out[b] = best;
+  }
+  return 0;
+}
+
 }  // extern "C"
