@@ -125,6 +125,20 @@ int sfh_fill_ghosts(sfh_mesh* m, int level, int which, int interp, double tau, v
  * corner ghost cells, which no stage reads, are set to NaN.  For parity tests of the ghost fill. */
 int sfh_get_ghosted(sfh_mesh* m, int which, double* d_G, void* stream);
 
+/* Refinement indicators, one double per block in CALLER order to d_out (device,
+ * [nblocks]); the caller compares with its threshold and rebuilds the mesh (no regrid inside the library).
+ *   SFH_REFINE_CURVATURE  eq. (33)-(34): max over the block's interior cells of
+ *                         max(E(rho), E(P)), E(q) = |d2x q + d2y q + d2z q| h^2 / q with centred second
+ *                         differences (the paper refines where this is >= 1e-2);
+ *   SFH_REFINE_JEANS      PAPER.md:641: max over the cells of h / lambda_J, lambda_J = c_s sqrt(pi / (G rho))
+ *                         (the paper refines where the Jeans length spans fewer than 8 cells: > 1/8).
+ * Reads one ghost layer of state copy `which`: same-level and outflow halos are gathered, coarse-fine
+ * halos come from the slabs of the last sfh_fill_ghosts(which) -- call that first on refined meshes.
+ * Asynchronous on `stream`.  SFH_EINVAL for an unknown criterion or G <= 0 with the Jeans criterion. */
+#define SFH_REFINE_CURVATURE 0
+#define SFH_REFINE_JEANS 1
+int sfh_refine_indicator(sfh_mesh* m, int which, int criterion, double G, double* d_out, void* stream);
+
 /* CFL time step (reading R16): dt = cfl * h_l / max over all cells of level l of
  * (max_d |v_d| + c_s), c_s = sqrt(gamma P / rho), from role 0; level = -1: minimum over levels
  * ("grid-level reductions").  Warp-shuffle + atomic-max reduction

@@ -67,6 +67,7 @@ def load_library(path=None):
         "sfh_fill_ghosts": (i32, [vp, i32, i32, i32, dbl, vp]),
         "sfh_get_ghosted": (i32, [vp, i32, vp, vp]),
         "sfh_cfl_dt": (i32, [vp, i32, C.POINTER(dbl), vp]),
+        "sfh_refine_indicator": (i32, [vp, i32, i32, dbl, vp, vp]),
         "sfh_hydro_step": (i32, [vp, i32, dbl, i32, dbl, dbl, vp]),
         "sfh_flux_correct": (i32, [vp, i32, dbl, vp]),
         "sfh_restrict": (i32, [vp, i32, i32, i32, vp]),
@@ -258,6 +259,14 @@ class Mesh:
         cnt = np.zeros(6, dtype=np.int64)
         self._chk(self.L.sfh_kernel_times(self.h, ms.ctypes.data, cnt.ctypes.data))
         return {k: (float(ms[i]), int(cnt[i])) for i, k in enumerate(self.KERNEL_CLASSES)}
+
+    def refine_indicator(self, criterion=0, which=0, G=1.0):
+        """Per-block refinement indicator (0: eq. 33-34 curvature, 1: h / Jeans length), caller order; fill the
+        ghosts of `which` first on refined meshes."""
+        import torch
+        out = torch.empty(self.nb, dtype=torch.float64, device=self.device)
+        self._chk(self.L.sfh_refine_indicator(self.h, which, criterion, float(G), out.data_ptr(), _stream()))
+        return out
 
     def status(self, which=0):
         n = C.c_int64()

@@ -543,6 +543,21 @@ int sfh_get_ghosted(sfh_mesh* m, int which, double* d_G, void* stream) {
   return SFH_OK;
 }
 
+int sfh_refine_indicator(sfh_mesh* m, int which, int criterion, double G, double* d_out, void* stream) {
+  int rc = check_bound(m);
+  if (rc) return rc;
+  if (which < 0 || which > 2 || !d_out) return fail(SFH_EINVAL, "bad argument");
+  if (criterion != SFH_REFINE_CURVATURE && criterion != SFH_REFINE_JEANS) return fail(SFH_EINVAL, "unknown criterion");
+  if (criterion == SFH_REFINE_JEANS && !(G > 0.0)) return fail(SFH_EINVAL, "G must be positive");
+  for (int l = 0; l < m->hm.nlev; ++l) {
+    CU(launch_refine_indicator(role_buf(m, l, which), which == 1 ? m->ghost1 : m->ghost, m->d_face_src, m->d_perm,
+                               int(m->hm.lev_first[l]), int(m->hm.lev_count[l]), which == 1, m->hm.cfg.gamma, criterion,
+                               G, m->hm.h[l], d_out, S(stream)), "refine_indicator_kernel");
+    m->launches += m->hm.lev_count[l] > 0;
+  }
+  return SFH_OK;
+}
+
 int sfh_cfl_dt(sfh_mesh* m, int level, double* dt_host, void* stream) {
   int rc = check_bound(m);
   if (rc || (rc = check_level(m, level))) return rc;

@@ -95,6 +95,10 @@ cudaError_t launch_permute(const double* src, double* dst, const int64_t* perm, 
                            int prim, double gamma, cudaStream_t st);
 cudaError_t launch_ghosted(const double* U, const double* ghost, const int32_t* face_src, const int64_t* perm,
                            int first, int count, int prim, double gamma, double* G, cudaStream_t st);
+// per-block refinement indicator (criterion 0: eq. 33-34, 1: h / Jeans length) of slots [first, first+count), caller order
+cudaError_t launch_refine_indicator(const double* U, const double* ghost, const int32_t* face_src, const int64_t* perm,
+                                    int first, int count, int prim, double gamma, int criterion, double G, double h,
+                                    double* out, cudaStream_t st);
 cudaError_t configure_kernels();
 
 }  // namespace sfh

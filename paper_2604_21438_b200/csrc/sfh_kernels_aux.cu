@@ -459,4 +459,90 @@ cudaError_t launch_ghosted(const double* U, const double* ghost, const int32_t* 
   return cudaGetLastError();
 }
 
+// =====================================================================================================
+// Refinement indicators.  One CTA of 256 threads per block: density and pressure of
+// the block and of one ghost layer behind each face (gathered like the stage kernels do: the neighbour's
+// interior, the block's own edge layer at an outflow face, the prolonged slab at a coarse-fine face) go to
+// shared memory; then per interior cell
+//   criterion 0, eq. (33)-(34) PAPER.md:277-285:  max(E(rho), E(P)),  E(q) = |sum_d (q_+d - 2 q + q_-d)| / q
+//   criterion 1, PAPER.md:641 (reading R31):      h / lambda_J = h rho sqrt(G / (pi gamma P))
+// and the maximum over the block, written in caller order.
+// =====================================================================================================
+__global__ void __launch_bounds__(256) refine_indicator_kernel(const double* __restrict__ U,
+                                                               const double* __restrict__ ghost,
+                                                               const int32_t* __restrict__ face_src,
+                                                               const int64_t* __restrict__ perm, int first, int prim,
+                                                               double gamma, int criterion, double G, double h,
+                                                               double* __restrict__ out) {
+  constexpr int M1 = N + 2;                    // one ghost layer
+  __shared__ double rho[M1 * M1 * M1], prs[M1 * M1 * M1];
+  __shared__ double wm[8];
+  const int s = first + blockIdx.x;
+  const double gm1 = gamma - 1.0;
+  for (int c = threadIdx.x; c < M1 * M1 * M1; c += 256) {
+    const int i = c % M1 - 1, j = (c / M1) % M1 - 1, k = c / (M1 * M1) - 1;
+    const int o[3] = {i < 0 ? -1 : i >= N ? 1 : 0, j < 0 ? -1 : j >= N ? 1 : 0, k < 0 ? -1 : k >= N ? 1 : 0};
+    const int nout = (o[0] != 0) + (o[1] != 0) + (o[2] != 0);
+    if (nout > 1) continue;                    // edges and corners: no stencil reads them
+    const double* from;
+    int vs = NC;
+    if (nout == 0) from = U + size_t(s) * BLK + (k * 8 + j) * 8 + i;
+    else {
+      const int axis = o[0] ? 0 : o[1] ? 1 : 2, side = o[axis] > 0;
+      const int src = face_src[s * 6 + 2 * axis + side];
+      int q[3] = {i, j, k};
+      if (src == SRC_OUTFLOW) {
+        q[axis] = side ? N - 1 : 0;
+        from = U + size_t(s) * BLK + (q[2] * 8 + q[1]) * 8 + q[0];
+      } else if (src >= 0) {
+        q[axis] += side ? -N : N;
+        from = U + size_t(src) * BLK + (q[2] * 8 + q[1]) * 8 + q[0];
+      } else {
+        const int ll = side ? 0 : NG - 1;      // the slab layer next to the face
+        from = ghost + size_t(-2 - src) * SLAB + slab_pos(axis, ll, axis == 0 ? j : i, axis == 2 ? j : k);
+        vs = NG * FACE;
+      }
+    }
+    double x[NV], w[NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) x[v] = from[v * vs];
+    if (prim) { w[0] = x[0]; w[4] = x[4]; }
+    else cons_to_prim(x, gm1, w);
+    rho[c] = w[0];
+    prs[c] = w[4];
+  }
+  __syncthreads();
+  double best = 0.0;
+  for (int c = threadIdx.x; c < NC; c += 256) {
+    const int i = c & 7, j = (c >> 3) & 7, k = c >> 6;
+    const int m = ((k + 1) * M1 + (j + 1)) * M1 + (i + 1);
+    const double r0 = rho[m], P0 = prs[m];
+    double val;
+    if (criterion == 0) {
+      double lr = 0.0, lP = 0.0;
+      const int st[3] = {1, M1, M1 * M1};
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {
+        lr += (rho[m + st[d]] - 2.0 * r0) + rho[m - st[d]];
+        lP += (prs[m + st[d]] - 2.0 * P0) + prs[m - st[d]];
+      }
+      val = fmax(fabs(lr) / r0, fabs(lP) / P0);
+    } else {
+      const double cs = sqrt(gamma * P0 / r0);
+      val = h / (cs * sqrt(3.14159265358979323846 / (G * r0)));
+    }
+    best = fmax(best, val);
+  }
+  best = cta_max<8>(best, wm);
+  if (threadIdx.x == 0) out[perm[s]] = best;
+}
+
+cudaError_t launch_refine_indicator(const double* U, const double* ghost, const int32_t* face_src, const int64_t* perm,
+                                    int first, int count, int prim, double gamma, int criterion, double G, double h,
+                                    double* out, cudaStream_t st) {
+  if (count <= 0) return cudaSuccess;
+  refine_indicator_kernel<<<count, 256, 0, st>>>(U, ghost, face_src, perm, first, prim, gamma, criterion, G, h, out);
+  return cudaGetLastError();
+}
+
 }  // namespace sfh

@@ -306,3 +306,32 @@ def test_set_riemann_rejects_unknown_solver():
     g = gpu_for(p)
     with pytest.raises(sfh.SfhError):
         g.set_riemann(7)
+
+
+# ------------------------------------------------------------------ refinement indicators
+@pytest.mark.parametrize("name", ["C1", "C2/4", "C4/4", "C5/8", "amr-small", "amr-outflow", "ragged", "one-block"])
+@pytest.mark.parametrize("criterion", [0, 1])
+def test_refine_indicator_parity(name, criterion):
+    p = PROBLEMS[name]()
+    o, g = both(p)
+    o.fill_ghosts(-1, 0, 0, 0.0)
+    g.fill_ghosts(-1, 0, 0, 0.0)
+    a = g.refine_indicator(criterion, 0, 2.5).cpu().numpy()
+    b = o.refine_indicator(criterion, 0, 2.5)
+    assert np.isfinite(a).all() and a.shape == b.shape
+    # second differences cancel: the error is absolute, a few ulp of the cell values over the cell value
+    assert (np.abs(a - b) <= 1e-12 * np.abs(b).max() + 1e-13).all(), np.abs(a - b).max()
+    if criterion == 0 and p.max_level > 0:
+        assert b.max() > 1e-3          # the test problems do have structure to flag
+    # the decision the caller takes from it: same flags wherever the oracle is not within rounding of the threshold
+    thr = np.median(b)
+    clear = np.abs(b - thr) > 1e-10 * max(thr, 1e-300)
+    assert np.array_equal((a >= thr)[clear], (b >= thr)[clear])
+
+
+def test_refine_indicator_rejects_bad_arguments():
+    g = gpu_for(PROBLEMS["one-block"]())
+    with pytest.raises(sfh.SfhError):
+        g.refine_indicator(5)
+    with pytest.raises(sfh.SfhError):
+        g.refine_indicator(1, 0, -1.0)
