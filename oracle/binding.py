@@ -59,6 +59,7 @@ def lib():
         L.orc_advance.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.POINTER(C.c_double), C.c_void_p]
         L.orc_status.argtypes = [C.c_void_p, C.c_int]
         L.orc_refine_indicator.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_void_p]
+        L.orc_transfer_state.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int]
         L.orc_status.restype = C.c_int64
         _lib = L
     return _lib
@@ -178,6 +179,10 @@ class OracleMesh:
 
     def status(self, copy=0):
         return self.L.orc_status(self.h, copy)
+
+    def transfer_from(self, src, which=0):
+        """State copy `which` of this (new) mesh from the old mesh `src` after a regrid: copies and prolongations."""
+        self._chk(self.L.orc_transfer_state(src.h, which, self.h, which))
 
     def refine_indicator(self, criterion=0, which=0, G=1.0):
         """Per-block refinement indicator (0: eq. 33-34 curvature, 1: h / Jeans length); ghosts must be filled."""

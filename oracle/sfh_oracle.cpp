@@ -716,4 +716,31 @@ int orc_refine_indicator(Mesh* m, int which, int criterion, double G, double* ou
   return 0;
 }
 
+// ------------------------------------------------------------------ regrid: state transfer
+// The state of a NEW mesh from an OLD one after a regrid ("blocks are refined ... subdivided into
+// eight child blocks"): every interior cell of every block of `dst` is the value of that cell in the old
+// hierarchy, get(src, level, I, J, K): a copy where the block existed, the slope-limited conservative
+// prolongation of reading R3 from the old coarser level(s) where it is new.  Blocks that disappear are
+// dropped: their parents exist in both meshes and already hold the restricted data.
+int orc_transfer_state(const Mesh* src, int src_which, Mesh* dst, int dst_which) {
+  if (src_which < 0 || src_which > 2 || dst_which < 0 || dst_which > 2) return -1;
+  for (int d = 0; d < 3; ++d)
+    if (src->cfg.nb0[d] != dst->cfg.nb0[d] || src->cfg.bc[d][0] != dst->cfg.bc[d][0] ||
+        src->cfg.bc[d][1] != dst->cfg.bc[d][1]) return -1;
+  std::vector<Src> srcs(std::max(src->nlev, dst->nlev), Src{0, src_which, 0.0});
+  int bad = 0;
+#pragma omp parallel for schedule(dynamic, 8) reduction(+ : bad)
+  for (int64_t b = 0; b < dst->nb; ++b) {
+    const int l = dst->lev[b];
+    double* out = dst->U[dst_which] + b * BLK;
+    double val[NV];
+    for (int k = 0; k < N; ++k) for (int j = 0; j < N; ++j) for (int i = 0; i < N; ++i) {
+      if (!get(*src, l, dst->bx[b] * N + i, dst->by[b] * N + j, dst->bz[b] * N + k, srcs.data(), val)) { bad++; continue; }
+      for (int v = 0; v < NV; ++v) out[gidx(v, i, j, k)] = val[v];
+    }
+  }
+  if (bad) { snprintf(dst->err, sizeof dst->err, "transfer_state: %d cells could not be resolved", bad); return -2; }
+  return 0;
+}
+
 }  // extern "C"
