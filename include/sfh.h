@@ -139,6 +139,16 @@ int sfh_get_ghosted(sfh_mesh* m, int which, double* d_G, void* stream);
 #define SFH_REFINE_JEANS 1
 int sfh_refine_indicator(sfh_mesh* m, int which, int criterion, double G, double* d_out, void* stream);
 
+/* Regrid: fills state copy dst_which of the NEW mesh `dst` from copy src_which of the OLD
+ * mesh `src` (both bound, same domain): a block present in both is copied; a new block is created from its old
+ * parent by the slope-limited conservative prolongation of reading R3 (so restricting the new children gives the
+ * parent back); blocks that disappear are dropped (their parents hold the restricted data).  A new block whose
+ * parent is not in the old mesh gives SFH_EMESH: refine by one level per regrid.  Only the conserved copies
+ * (0 and 2).  Reads the old mesh's coarse-fine ghost slabs: call sfh_fill_ghosts(src, -1, src_which, 0, 0) first.
+ * The caller builds `dst` (sfh_create_mesh from the flags of sfh_refine_indicator, padded to 2:1) and binds it.
+ * Synchronous (it uploads a block map and waits for the copy). */
+int sfh_transfer_state(sfh_mesh* src, int src_which, sfh_mesh* dst, int dst_which, void* stream);
+
 /* CFL time step (reading R16): dt = cfl * h_l / max over all cells of level l of
  * (max_d |v_d| + c_s), c_s = sqrt(gamma P / rho), from role 0; level = -1: minimum over levels
  * ("grid-level reductions").  Warp-shuffle + atomic-max reduction

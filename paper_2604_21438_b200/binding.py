@@ -68,6 +68,7 @@ def load_library(path=None):
         "sfh_get_ghosted": (i32, [vp, i32, vp, vp]),
         "sfh_cfl_dt": (i32, [vp, i32, C.POINTER(dbl), vp]),
         "sfh_refine_indicator": (i32, [vp, i32, i32, dbl, vp, vp]),
+        "sfh_transfer_state": (i32, [vp, i32, vp, i32, vp]),
         "sfh_hydro_step": (i32, [vp, i32, dbl, i32, dbl, dbl, vp]),
         "sfh_flux_correct": (i32, [vp, i32, dbl, vp]),
         "sfh_restrict": (i32, [vp, i32, i32, i32, vp]),
@@ -259,6 +260,11 @@ class Mesh:
         cnt = np.zeros(6, dtype=np.int64)
         self._chk(self.L.sfh_kernel_times(self.h, ms.ctypes.data, cnt.ctypes.data))
         return {k: (float(ms[i]), int(cnt[i])) for i, k in enumerate(self.KERNEL_CLASSES)}
+
+    def transfer_from(self, src, which=0):
+        """Regrid: state copy `which` of this (new) mesh from the old mesh `src` (copies and prolongations); fill
+        the old mesh's ghosts of `which` first."""
+        self._chk(self.L.sfh_transfer_state(src.h, which, self.h, which, _stream()))
 
     def refine_indicator(self, criterion=0, which=0, G=1.0):
         """Per-block refinement indicator (0: eq. 33-34 curvature, 1: h / Jeans length), caller order; fill the

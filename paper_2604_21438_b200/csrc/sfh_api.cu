@@ -5,6 +5,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <unordered_map>
 #include <vector>
 
 #include "sfh_kernels.cuh"
@@ -554,6 +555,69 @@ int sfh_refine_indicator(sfh_mesh* m, int which, int criterion, double G, double
                                int(m->hm.lev_first[l]), int(m->hm.lev_count[l]), which == 1, m->hm.cfg.gamma, criterion,
                                G, m->hm.h[l], d_out, S(stream)), "refine_indicator_kernel");
     m->launches += m->hm.lev_count[l] > 0;
+  }
+  return SFH_OK;
+}
+
+int sfh_transfer_state(sfh_mesh* src, int src_which, sfh_mesh* dst, int dst_which, void* stream) {
+  int rc = check_bound(src);
+  if (rc || (rc = check_bound(dst))) return rc;
+  if ((src_which != 0 && src_which != 2) || (dst_which != 0 && dst_which != 2))
+    return fail(SFH_EINVAL, "state transfer works on the conserved copies (roles 0 and 2)");
+  const HostMesh &hs = src->hm, &hd = dst->hm;
+  for (int d = 0; d < 3; ++d)
+    if (hs.cfg.nb0[d] != hd.cfg.nb0[d] || hs.cfg.bc[d][0] != hd.cfg.bc[d][0] || hs.cfg.bc[d][1] != hd.cfg.bc[d][1] ||
+        hs.cfg.box_len[d] != hd.cfg.box_len[d])
+      return fail(SFH_EINVAL, "the two meshes describe different domains");
+  auto key = [](int l, const int32_t* c) {
+    return (uint64_t(l) << 60) | (uint64_t(uint32_t(c[0]) & 0xFFFFF) << 40) | (uint64_t(uint32_t(c[1]) & 0xFFFFF) << 20) |
+           uint64_t(uint32_t(c[2]) & 0xFFFFF);
+  };
+  std::vector<int32_t> tsrc;
+  try {
+    std::unordered_map<uint64_t, int32_t> old;
+    old.reserve(size_t(hs.nb) * 2);
+    for (int64_t b = 0; b < hs.nb; ++b) old.emplace(key(hs.lev[b], &hs.coord[3 * b]), int32_t(b));
+    tsrc.resize(size_t(hd.nb));
+    for (int64_t b = 0; b < hd.nb; ++b) {
+      const int l = hd.lev[b];
+      auto it = old.find(key(l, &hd.coord[3 * b]));
+      if (it != old.end()) { tsrc[b] = it->second; continue; }
+      const int32_t pc[3] = {hd.coord[3 * b] >> 1, hd.coord[3 * b + 1] >> 1, hd.coord[3 * b + 2] >> 1};
+      it = l > 0 ? old.find(key(l - 1, pc)) : old.end();
+      if (it == old.end())
+        return fail(SFH_EMESH, "a block of the new mesh has neither itself nor its parent in the old mesh "
+                               "(refine by one level per regrid)");
+      tsrc[b] = -2 - it->second;
+    }
+  } catch (const std::bad_alloc&) {
+    return fail(SFH_ENOMEM, "out of host memory");
+  }
+  cudaStream_t st = S(stream);
+  int32_t* d_tsrc = nullptr;
+  if (cudaMalloc((void**)&d_tsrc, tsrc.size() * 4) != cudaSuccess) return fail(SFH_ENOMEM, "cudaMalloc of the transfer table failed");
+  cudaError_t e = cudaMemcpyAsync(d_tsrc, tsrc.data(), tsrc.size() * 4, cudaMemcpyHostToDevice, st);
+  // all levels of the old mesh share one physical buffer per role (the roles rotate together per level only within
+  // a step; between steps every level's role r sits in buffer role[l][r]): transfer level by level
+  for (int l = 0; l < hd.nlev && e == cudaSuccess; ++l) {
+    // a new block of level l reads old level l (copy) or old level l-1 (prolongation)
+    const int ls = l < hs.nlev ? l : hs.nlev - 1;
+    if (l > 0 && l < hs.nlev && src->role[l][src_which] != src->role[l - 1][src_which]) {
+      cudaFree(d_tsrc);
+      return fail(SFH_ESTATE, "the old mesh's levels hold the requested copy in different buffers (finish the step first)");
+    }
+    const int64_t first = hd.lev_first[l], count = hd.lev_count[l];
+    e = launch_transfer(role_buf(src, ls, src_which), src_which == 1 ? src->ghost1 : src->ghost, src->d_face_src,
+                        d_tsrc + first, dst->d_coord + 3 * first, role_buf(dst, l, dst_which) + size_t(first) * BLK,
+                        int(count), st);
+    dst->launches += count > 0;
+  }
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  cudaFree(d_tsrc);
+  if (e != cudaSuccess) return cuda_fail(e, "transfer_kernel");
+  for (int l = 0; l < hd.nlev; ++l) {
+    if (dst_which == 0) dst->bmax_valid[l] = false;
+    else dst->bmax_pending[l] = false;
   }
   return SFH_OK;
 }

@@ -545,4 +545,78 @@ cudaError_t launch_refine_indicator(const double* U, const double* ghost, const 
   return cudaGetLastError();
 }
 
+// =====================================================================================================
+// Regrid: state of a new mesh from an old one.  One CTA per block of
+// the new mesh.  tsrc[d] >= 0: the block exists in the old mesh, slot tsrc[d]: copy.  tsrc[d] <= -2: it is
+// new; its parent is old slot -2 - tsrc[d]: every fine cell is the slope-limited conservative prolongation
+// (reading R3) of the parent's cell and its six neighbours, which lie in the parent, in its same-level
+// neighbour, behind an outflow face (zero gradient) or in the old mesh's prolonged ghost slab.
+// =====================================================================================================
+__global__ void __launch_bounds__(256) transfer_kernel(const double* __restrict__ Us, const double* __restrict__ ghost_s,
+                                                       const int32_t* __restrict__ face_src_s,
+                                                       const int32_t* __restrict__ tsrc,
+                                                       const int32_t* __restrict__ coord_d, double* __restrict__ Ud) {
+  const int d = blockIdx.x;
+  const int t = tsrc[d];
+  double* out = Ud + size_t(d) * BLK;
+  if (t >= 0) {
+    const double2* from = reinterpret_cast<const double2*>(Us + size_t(t) * BLK);
+    double2* to = reinterpret_cast<double2*>(out);
+    for (int q = threadIdx.x; q < BLK / 2; q += 256) to[q] = from[q];
+    return;
+  }
+  const int P = -2 - t;
+  const int oct[3] = {coord_d[3 * d] & 1, coord_d[3 * d + 1] & 1, coord_d[3 * d + 2] & 1};
+  const double* Up = Us + size_t(P) * BLK;
+  auto fetch = [&](int c0, int c1, int c2, double q[NV]) {       // coarse cell of the parent's neighbourhood
+    int c[3] = {c0, c1, c2};
+    const double* from;
+    int vs = NC;
+    const int axis = (c0 < 0 || c0 >= N) ? 0 : (c1 < 0 || c1 >= N) ? 1 : (c2 < 0 || c2 >= N) ? 2 : -1;
+    if (axis < 0) from = Up + (c[2] * 8 + c[1]) * 8 + c[0];
+    else {
+      const int side = c[axis] >= N;
+      const int src = face_src_s[P * 6 + 2 * axis + side];
+      if (src == SRC_OUTFLOW) {
+        c[axis] = side ? N - 1 : 0;
+        from = Up + (c[2] * 8 + c[1]) * 8 + c[0];
+      } else if (src >= 0) {
+        c[axis] += side ? -N : N;
+        from = Us + size_t(src) * BLK + (c[2] * 8 + c[1]) * 8 + c[0];
+      } else {
+        from = ghost_s + size_t(-2 - src) * SLAB +
+               slab_pos(axis, side ? 0 : NG - 1, axis == 0 ? c[1] : c[0], axis == 2 ? c[1] : c[2]);
+        vs = NG * FACE;
+      }
+    }
+#pragma unroll
+    for (int v = 0; v < NV; ++v) q[v] = from[v * vs];
+  };
+  for (int cell = threadIdx.x; cell < NC; cell += 256) {
+    const int f[3] = {cell & 7, (cell >> 3) & 7, cell >> 6};
+    const int c[3] = {oct[0] * 4 + (f[0] >> 1), oct[1] * 4 + (f[1] >> 1), oct[2] * 4 + (f[2] >> 1)};
+    double Q[NV], Qp[NV], Qm[NV], val[NV];
+    fetch(c[0], c[1], c[2], Q);
+#pragma unroll
+    for (int v = 0; v < NV; ++v) val[v] = Q[v];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      fetch(c[0] + (a == 0), c[1] + (a == 1), c[2] + (a == 2), Qp);
+      fetch(c[0] - (a == 0), c[1] - (a == 1), c[2] - (a == 2), Qm);
+      const double sig = (f[a] & 1) ? 0.25 : -0.25;
+#pragma unroll
+      for (int v = 0; v < NV; ++v) val[v] = val[v] + sig * minmod(Qp[v] - Q[v], Q[v] - Qm[v]);
+    }
+#pragma unroll
+    for (int v = 0; v < NV; ++v) out[v * NC + cell] = val[v];
+  }
+}
+
+cudaError_t launch_transfer(const double* Us, const double* ghost_s, const int32_t* face_src_s, const int32_t* tsrc,
+                            const int32_t* coord_d, double* Ud, int count, cudaStream_t st) {
+  if (count <= 0) return cudaSuccess;
+  transfer_kernel<<<count, 256, 0, st>>>(Us, ghost_s, face_src_s, tsrc, coord_d, Ud);
+  return cudaGetLastError();
+}
+
 }  // namespace sfh

@@ -335,3 +335,70 @@ def test_refine_indicator_rejects_bad_arguments():
         g.refine_indicator(5)
     with pytest.raises(sfh.SfhError):
         g.refine_indicator(1, 0, -1.0)
+
+
+# ------------------------------------------------------------------ regrid state transfer
+def regrid_pair():
+    """An old 3-level mesh and a new one: one more root block refined, the level-2 patch moved by
+    one level-1 block (new level-2 blocks appear, old ones disappear)."""
+    old = small_amr_tree()
+    t = Tree((4, 4, 4), 2, (True, True, True))
+    f0 = np.zeros_like(t.exists[0])
+    f0[1:3, 1:3, 1:3] = True
+    f0[0, 1, 1] = True
+    t.refine(0, f0)
+    f1 = np.zeros_like(t.exists[1])
+    f1[4:6, 3:5, 3:5] = True
+    t.refine(1, f1)
+    return old, t.pad_2to1()
+
+
+def test_regrid_transfer_parity_and_restart():
+    told, tnew = regrid_pair()
+    p = problem_from_tree(told, mode=1)
+    q = problem_from_tree(tnew, mode=1)
+    o, g = both(p)
+    o.advance(2, 1)
+    g.advance(2, 1)                       # a state with structure on every level
+    o.fill_ghosts(-1, 0, 0, 0.0)
+    g.fill_ghosts(-1, 0, 0, 0.0)
+    o2 = oracle_for(q)
+    g2 = sfh.Mesh.from_problem(q)
+    o2.transfer_from(o)
+    g2.transfer_from(g)
+    Uo, Ug = o2.get_state(), g2.get_state().cpu().numpy()
+    err = parity_errors(Ug, Uo, p.gamma)
+    assert (err <= TOL10).all(), err
+    # blocks present in both meshes are copies of the CUDA path's own state, bit for bit
+    key = lambda lv, ijk: [(int(l), *map(int, c)) for l, c in zip(lv, ijk)]
+    old = {k: n for n, k in enumerate(key(p.level, p.ijk))}
+    Ugo = g.get_state().cpu().numpy()
+    created = 0
+    for n, k in enumerate(key(q.level, q.ijk)):
+        if k in old:
+            assert np.array_equal(Ug[n], Ugo[old[k]])
+        else:
+            created += 1
+    assert created >= 16
+    # the new hierarchy is restriction-consistent (conservative prolongation) and steps on
+    g2.restrict_all(0)
+    scale = np.abs(Ug).max(axis=(0, 2, 3, 4))[None, :, None, None, None]
+    assert (np.abs(g2.get_state().cpu().numpy() - Ug) <= 6e-16 * scale).all()
+    o2.restrict_all(0)
+    o2.advance(2, 1)
+    g2.advance(2, 1)
+    assert np.array_equal(o2.nupd, g2.nupd)
+    compare(o2, g2, p.gamma, TOL10)
+
+
+def test_regrid_transfer_rejects_two_levels_at_once_and_other_domains():
+    u = problem_from_tree(uniform_tree((4, 4, 4), 2), mode=1)
+    p = problem_from_tree(small_amr_tree(), mode=1)
+    gu, gp = gpu_for(u), sfh.Mesh.from_problem(p)
+    with pytest.raises(sfh.SfhError) as e:
+        gp.transfer_from(gu)              # the level-2 blocks have no parent in the uniform mesh
+    assert e.value.code == -2
+    other = sfh.Mesh.from_problem(problem_from_tree(uniform_tree((2, 2, 2), 0)))
+    with pytest.raises(sfh.SfhError) as e:
+        other.transfer_from(gu)
+    assert e.value.code == -1
