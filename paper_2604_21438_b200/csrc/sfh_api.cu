@@ -597,17 +597,12 @@ int sfh_transfer_state(sfh_mesh* src, int src_which, sfh_mesh* dst, int dst_whic
   int32_t* d_tsrc = nullptr;
   if (cudaMalloc((void**)&d_tsrc, tsrc.size() * 4) != cudaSuccess) return fail(SFH_ENOMEM, "cudaMalloc of the transfer table failed");
   cudaError_t e = cudaMemcpyAsync(d_tsrc, tsrc.data(), tsrc.size() * 4, cudaMemcpyHostToDevice, st);
-  // all levels of the old mesh share one physical buffer per role (the roles rotate together per level only within
-  // a step; between steps every level's role r sits in buffer role[l][r]): transfer level by level
+  // a new block of level l reads old level l (copy) or old level l-1 (prolongation); the roles rotate per level,
+  // so the two may sit in different physical buffers
   for (int l = 0; l < hd.nlev && e == cudaSuccess; ++l) {
-    // a new block of level l reads old level l (copy) or old level l-1 (prolongation)
-    const int ls = l < hs.nlev ? l : hs.nlev - 1;
-    if (l > 0 && l < hs.nlev && src->role[l][src_which] != src->role[l - 1][src_which]) {
-      cudaFree(d_tsrc);
-      return fail(SFH_ESTATE, "the old mesh's levels hold the requested copy in different buffers (finish the step first)");
-    }
+    const int lc = l < hs.nlev ? l : hs.nlev - 1, lp = l > 0 ? (l - 1 < hs.nlev ? l - 1 : hs.nlev - 1) : 0;
     const int64_t first = hd.lev_first[l], count = hd.lev_count[l];
-    e = launch_transfer(role_buf(src, ls, src_which), src_which == 1 ? src->ghost1 : src->ghost, src->d_face_src,
+    e = launch_transfer(role_buf(src, lc, src_which), role_buf(src, lp, src_which), src->ghost, src->d_face_src,
                         d_tsrc + first, dst->d_coord + 3 * first, role_buf(dst, l, dst_which) + size_t(first) * BLK,
                         int(count), st);
     dst->launches += count > 0;

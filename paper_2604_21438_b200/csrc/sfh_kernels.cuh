@@ -100,8 +100,9 @@ cudaError_t launch_refine_indicator(const double* U, const double* ghost, const 
                                     int first, int count, int prim, double gamma, int criterion, double G, double h,
                                     double* out, cudaStream_t st);
 // regrid: block d of the new mesh <- old slot tsrc[d] (copy) or prolongation from old parent -2 - tsrc[d]
-cudaError_t launch_transfer(const double* Us, const double* ghost_s, const int32_t* face_src_s, const int32_t* tsrc,
-                            const int32_t* coord_d, double* Ud, int count, cudaStream_t st);
+// Uc / Us: the old buffers holding the block's own level (copies) and its parent level (prolongation)
+cudaError_t launch_transfer(const double* Uc, const double* Us, const double* ghost_s, const int32_t* face_src_s,
+                            const int32_t* tsrc, const int32_t* coord_d, double* Ud, int count, cudaStream_t st);
 cudaError_t configure_kernels();
 
 }  // namespace sfh

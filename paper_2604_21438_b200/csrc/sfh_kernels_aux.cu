@@ -552,7 +552,9 @@ cudaError_t launch_refine_indicator(const double* U, const double* ghost, const 
 // (reading R3) of the parent's cell and its six neighbours, which lie in the parent, in its same-level
 // neighbour, behind an outflow face (zero gradient) or in the old mesh's prolonged ghost slab.
 // =====================================================================================================
-__global__ void __launch_bounds__(256) transfer_kernel(const double* __restrict__ Us, const double* __restrict__ ghost_s,
+// Uc: the old buffer that holds the block's own level (copies), Us: the one that holds the parent level.
+__global__ void __launch_bounds__(256) transfer_kernel(const double* __restrict__ Uc, const double* __restrict__ Us,
+                                                       const double* __restrict__ ghost_s,
                                                        const int32_t* __restrict__ face_src_s,
                                                        const int32_t* __restrict__ tsrc,
                                                        const int32_t* __restrict__ coord_d, double* __restrict__ Ud) {
@@ -560,7 +562,7 @@ __global__ void __launch_bounds__(256) transfer_kernel(const double* __restrict_
   const int t = tsrc[d];
   double* out = Ud + size_t(d) * BLK;
   if (t >= 0) {
-    const double2* from = reinterpret_cast<const double2*>(Us + size_t(t) * BLK);
+    const double2* from = reinterpret_cast<const double2*>(Uc + size_t(t) * BLK);
     double2* to = reinterpret_cast<double2*>(out);
     for (int q = threadIdx.x; q < BLK / 2; q += 256) to[q] = from[q];
     return;
@@ -612,10 +614,10 @@ __global__ void __launch_bounds__(256) transfer_kernel(const double* __restrict_
   }
 }
 
-cudaError_t launch_transfer(const double* Us, const double* ghost_s, const int32_t* face_src_s, const int32_t* tsrc,
-                            const int32_t* coord_d, double* Ud, int count, cudaStream_t st) {
+cudaError_t launch_transfer(const double* Uc, const double* Us, const double* ghost_s, const int32_t* face_src_s,
+                            const int32_t* tsrc, const int32_t* coord_d, double* Ud, int count, cudaStream_t st) {
   if (count <= 0) return cudaSuccess;
-  transfer_kernel<<<count, 256, 0, st>>>(Us, ghost_s, face_src_s, tsrc, coord_d, Ud);
+  transfer_kernel<<<count, 256, 0, st>>>(Uc, Us, ghost_s, face_src_s, tsrc, coord_d, Ud);
   return cudaGetLastError();
 }
 

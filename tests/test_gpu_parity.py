@@ -402,3 +402,44 @@ def test_regrid_transfer_rejects_two_levels_at_once_and_other_domains():
     with pytest.raises(sfh.SfhError) as e:
         other.transfer_from(gu)
     assert e.value.code == -1
+
+
+def test_dynamic_regrid_cycle_matches_the_oracle():
+    """step -> refinement indicator -> flags -> new mesh (2:1 padded) -> state transfer -> step, twice,
+    on both sides; the flags are taken where the indicator is clear of the threshold, and must agree."""
+    from sfh_inputs.configs import Problem
+    p = problem_from_tree(small_amr_tree(), mode=1)
+    o, g = both(p)
+    for cycle in range(2):
+        o.advance(1, 1)
+        g.advance(1, 1)
+        o.fill_ghosts(-1, 0, 0, 0.0)
+        g.fill_ghosts(-1, 0, 0, 0.0)
+        io = o.refine_indicator(0)
+        ig = g.refine_indicator(0).cpu().numpy()
+        s = np.sort(io)
+        k = int(0.6 * len(s))
+        k = k + int(np.argmax(np.diff(s[k:k + 12])))        # the widest gap near the 60 % quantile
+        thr = 0.5 * (s[k] + s[k + 1])
+        assert s[k + 1] - s[k] > 1e-9 * thr
+        assert np.array_equal(io >= thr, ig >= thr)
+        t = Tree(p.nb0, p.max_level, (True, True, True))
+        for l in range(p.max_level):
+            f = np.zeros_like(t.exists[l])
+            sel = (p.level == l) & (ig >= thr)
+            f[p.ijk[sel, 0], p.ijk[sel, 1], p.ijk[sel, 2]] = True
+            t.refine(l, f)
+        t.pad_2to1()
+        level, ijk = t.block_list()
+        q = Problem("regrid%d" % cycle, p.nb0, p.max_level, p.bc, p.box_len, p.gamma, p.cfl, 1, 1, level, ijk,
+                    np.zeros((len(level), 5, 8, 8, 8)))
+        assert q.census() != p.census()
+        o2, g2 = oracle_for(q), sfh.Mesh.from_problem(q)
+        o2.transfer_from(o)
+        g2.transfer_from(g)
+        o, g, p = o2, g2, q
+        compare(o, g, p.gamma, TOL10)
+    o.advance(2, 1)
+    g.advance(2, 1)
+    assert np.array_equal(o.nupd, g.nupd)
+    compare(o, g, p.gamma, TOL10)
