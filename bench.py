@@ -46,6 +46,8 @@ def parse():
                     help="Riemann solver (PAPER.md:126); the paper's benchmarks and BASELINE.json use HLLC")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--extras", action="store_true",
+                    help="also time the regrid pieces (refinement indicators, state transfer) on this config")
     return ap.parse_args()
 
 
@@ -322,6 +324,35 @@ def main():
             dist.destroy_process_group()
         return
 
+    extras = None
+    if args.extras and world == 1:
+        # the indicator kernel reads the state once (40 B/cell + halos through L2); the
+        # transfer onto an identical mesh copies it (80 B/cell)
+        reset()
+        g.fill_ghosts(-1, 0, 0, 0.0)
+        ncell = 512.0 * sum(census)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+
+        def timed(fn, reps=5):
+            fn()
+            torch.cuda.synchronize()
+            ev[0].record()
+            for _ in range(reps):
+                fn()
+            ev[1].record()
+            torch.cuda.synchronize()
+            return ev[0].elapsed_time(ev[1]) / reps
+
+        ms_c = timed(lambda: g.refine_indicator(0))
+        ms_j = timed(lambda: g.refine_indicator(1))
+        g2 = sfh.Mesh.from_problem(p, device=dev)
+        ms_t = timed(lambda: g2.transfer_from(g), reps=3)
+        extras = {"refine_indicator_curvature": {"ms": ms_c, "GBps_at_40B_per_cell": 40.0 * ncell / ms_c / 1e6},
+                  "refine_indicator_jeans": {"ms": ms_j, "GBps_at_40B_per_cell": 40.0 * ncell / ms_j / 1e6},
+                  "transfer_state_identity": {"ms": ms_t, "GBps_at_80B_per_cell": 80.0 * ncell / ms_t / 1e6,
+                                              "note": "includes building and uploading the block map on the host"}}
+        del g2
+
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         # the oracle as it stands on this box's host cores, on a bounded sample: whole coarse steps of
@@ -352,6 +383,7 @@ def main():
         "gpu_launches": int(launches),
         "roofline": roofline,
         "roofline_fp64": roofline_fp64,
+        "extras": extras,
         "cpu_baseline": cpu,
     }
     print(json.dumps(out))
