@@ -115,19 +115,17 @@ __device__ __forceinline__ void store_df(double* __restrict__ dF, int c, int a, 
   for (int q = 0; q < 5; ++q) dF[ci + q * NC] = Fa[q] - Fb[q];
 }
 
-// flux registers at coarse-fine faces (a7; reading R14); Fn in the face frame
-__device__ __noinline__ void store_regs(const int32_t* face_src, const int32_t* fslot, double* R, double* FH, int blk,
-                                        int D, int side, int t, double F0, double F1, double F2, double F3, double F4,
-                                        double dt) {
-  const double Fn[5] = {F0, F1, F2, F3, F4};
-  const int f = 2 * D + side;
-  const int src = face_src[blk * 6 + f];
-  const int fs = fslot[blk * 6 + f];
+// flux registers at coarse-fine faces (a7; reading R14); Fn in the face frame.  src / fs: the face's
+// halo source and its coarse-side register slot (loaded at the start of the walk, so the walker never waits for
+// them).  Every register entry has one contributor per launch: the accumulation is a fire-and-forget reduction
+// (RED.ADD.F64) with the same result as a read-modify-write.
+__device__ __forceinline__ void store_regs(int src, int fs, double* R, double* FH, int D, int t, const double Fn[5],
+                                           double dt) {
   const int vn = 1 + D, vt1 = 1 + (D + 1) % 3, vt2 = 1 + (D + 2) % 3;
   if (src <= -2) {   // fine side of a coarse-fine face: accumulate dt * F
     double* r = R + size_t(-2 - src) * REG + t;
-    r[0] += dt * Fn[0]; r[vn * FACE] += dt * Fn[1]; r[vt1 * FACE] += dt * Fn[2]; r[vt2 * FACE] += dt * Fn[3];
-    r[4 * FACE] += dt * Fn[4];
+    atomicAdd(r, dt * Fn[0]); atomicAdd(r + vn * FACE, dt * Fn[1]); atomicAdd(r + vt1 * FACE, dt * Fn[2]);
+    atomicAdd(r + vt2 * FACE, dt * Fn[3]); atomicAdd(r + 4 * FACE, dt * Fn[4]);
   }
   if (fs >= 0) {     // coarse leaf next to a covered block: keep its own flux
     double* r = FH + size_t(fs) * REG + t;
@@ -233,12 +231,19 @@ __device__ __forceinline__ void walk_geom(int a, int b, int f0, WalkGeom& g) {
 __device__ __forceinline__ void load_cell_g(const double* __restrict__ Wl, int o, const int ov[3], double w[5]) {
   w[0] = Wl[o]; w[1] = Wl[o + ov[0]]; w[2] = Wl[o + ov[1]]; w[3] = Wl[o + ov[2]]; w[4] = Wl[o + 4 * CVS];
 }
-template <int RS>
+// REGS: the level has flux-register faces
+template <int RS, bool REGS>
 __device__ __forceinline__ void walk_corrector_generic(const double* __restrict__ Wl, double* __restrict__ dF,
                                                        const WalkGeom& g, int D, int a, int b, int f0, double gamma,
                                                        double igm1, const StageParams& p, int blk, double dt,
                                                        uint32_t bar_empty, uint32_t par_empty, bool wait_empty) {
   double wp[5], wc[5], wn[5], dp[5], dn[5], L[5], Ln[5], R[5], Fa[5], Fb[5];
+  int rsrc = 0, rfs = -1;                                     // my boundary face: halo source, coarse-side register
+  if (REGS) {
+    const int f = blk * 6 + 2 * D + (f0 != 0);
+    rsrc = p.face_src[f];
+    rfs = p.fslot[f];
+  }
   load_cell_g(Wl, g.cp[0], g.ov, wp);
   load_cell_g(Wl, g.cp[1], g.ov, wc);
   load_cell_g(Wl, g.cp[2], g.ov, wn);
@@ -257,16 +262,14 @@ __device__ __forceinline__ void walk_corrector_generic(const double* __restrict_
 #pragma unroll
     for (int v = 0; v < 5; ++v) L[v] = Ln[v];
     if (ff == 0) {
-      if (p.use_regs && f0 == 0)
-        store_regs(p.face_src, p.fslot, p.R, p.FH, blk, D, 0, b * 8 + a, Fa[0], Fa[1], Fa[2], Fa[3], Fa[4], dt);
+      if (REGS && f0 == 0 && (rsrc <= -2 || rfs >= 0)) store_regs(rsrc, rfs, p.R, p.FH, D, b * 8 + a, Fa, dt);
       if (wait_empty) mbar_wait(bar_empty, par_empty);        // the update two blocks back has read this dF buffer
     } else {
 #pragma unroll
       for (int q = 0; q < 5; ++q) dF[g.di[ff - 1] + q * NC] = (ff & 1) ? Fb[q] - Fa[q] : Fa[q] - Fb[q];
     }
   }
-  if (p.use_regs && f0 != 0)
-    store_regs(p.face_src, p.fslot, p.R, p.FH, blk, D, 1, b * 8 + a, Fa[0], Fa[1], Fa[2], Fa[3], Fa[4], dt);
+  if (REGS && f0 != 0 && (rsrc <= -2 || rfs >= 0)) store_regs(rsrc, rfs, p.R, p.FH, D, b * 8 + a, Fa, dt);
 }
 
 // ---- helpers: staging ----------------------------------------------------------------------------------
@@ -424,7 +427,7 @@ __device__ __forceinline__ void store_block(const double u[HC][NV], double gm1, 
 //   full[d]    all walkers have stored the flux differences into buffer d = it % NDF (and are done with
 //              the staging buffer, which the helpers then re-stage)
 //   empty[d]   the helpers have consumed flux-difference buffer d
-template <int STAGE, int RS>
+template <int STAGE, int RS, bool REGS>
 __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_constant__ TensorMaps tm,
                                                                   const StageParams p) {
   using C = Cfg<STAGE>;
@@ -502,7 +505,7 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
         else walk_predictor<RS, 2>(Wl, dF, a, b, f0, gm1, igm1, empty(d), pe, we);
       } else {
         const int blk = blk0 + it * stride;
-        walk_corrector_generic<RS>(Wl, dF, geom, D, a, b, f0, gamma, igm1, p, blk, dt, empty(d), pe, we);
+        walk_corrector_generic<RS, REGS>(Wl, dF, geom, D, a, b, f0, gamma, igm1, p, blk, dt, empty(d), pe, we);
       }
       __syncwarp();
       if ((tid & 31) == 0) mbar_arrive(full(d));
@@ -623,15 +626,17 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
 
 static int g_stage_ctas = 148;   // persistent grid: one CTA per SM (set by configure_kernels)
 
-template <int STAGE, int RS>
+template <int STAGE, int RS, bool REGS>
 static cudaError_t configure_one() {
-  return cudaFuncSetAttribute(stage_kernel<STAGE, RS>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<STAGE>::SMEM);
+  return cudaFuncSetAttribute(stage_kernel<STAGE, RS, REGS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              Cfg<STAGE>::SMEM);
 }
 
 cudaError_t configure_kernels() {
   cudaError_t e;
-  if ((e = configure_one<0, 0>()) != cudaSuccess || (e = configure_one<1, 0>()) != cudaSuccess ||
-      (e = configure_one<0, 1>()) != cudaSuccess || (e = configure_one<1, 1>()) != cudaSuccess)
+  if ((e = configure_one<0, 0, false>()) != cudaSuccess || (e = configure_one<0, 1, false>()) != cudaSuccess ||
+      (e = configure_one<1, 0, false>()) != cudaSuccess || (e = configure_one<1, 0, true>()) != cudaSuccess ||
+      (e = configure_one<1, 1, false>()) != cudaSuccess || (e = configure_one<1, 1, true>()) != cudaSuccess)
     return e;
   int dev = 0, sms = 0;
   if (cudaGetDevice(&dev) == cudaSuccess &&
@@ -640,15 +645,23 @@ cudaError_t configure_kernels() {
   return cudaSuccess;
 }
 
+template <int STAGE, int RS, bool REGS>
+static void launch_one(int grid, const TensorMaps& tm, const StageParams& p, cudaStream_t st) {
+  stage_kernel<STAGE, RS, REGS><<<grid, STAGE_THREADS, Cfg<STAGE>::SMEM, st>>>(tm, p);
+}
+
+// The corrector of a level with flux-register faces is its own instantiation: the register code costs the
+// uniform-grid walk a few per cent even when it never runs (measured).
 cudaError_t launch_stage(int stage, const TensorMaps& tm, const StageParams& p, cudaStream_t st) {
   if (p.count <= 0) return cudaSuccess;
   const int grid = p.count < g_stage_ctas ? p.count : g_stage_ctas;
-  if (p.riemann == 0) {
-    if (stage == 0) stage_kernel<0, 0><<<grid, STAGE_THREADS, Cfg<0>::SMEM, st>>>(tm, p);
-    else stage_kernel<1, 0><<<grid, STAGE_THREADS, Cfg<1>::SMEM, st>>>(tm, p);
+  const bool roe = p.riemann != 0;
+  if (stage == 0) {
+    if (roe) launch_one<0, 1, false>(grid, tm, p, st); else launch_one<0, 0, false>(grid, tm, p, st);
+  } else if (p.use_regs) {
+    if (roe) launch_one<1, 1, true>(grid, tm, p, st); else launch_one<1, 0, true>(grid, tm, p, st);
   } else {
-    if (stage == 0) stage_kernel<0, 1><<<grid, STAGE_THREADS, Cfg<0>::SMEM, st>>>(tm, p);
-    else stage_kernel<1, 1><<<grid, STAGE_THREADS, Cfg<1>::SMEM, st>>>(tm, p);
+    if (roe) launch_one<1, 1, false>(grid, tm, p, st); else launch_one<1, 0, false>(grid, tm, p, st);
   }
   return cudaGetLastError();
 }
