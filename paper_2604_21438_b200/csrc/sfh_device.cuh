@@ -189,13 +189,14 @@ __device__ __forceinline__ void hllc_flux(double rL, double uL, double vL, doubl
 //   F = ((F_L + F_R) - sum_k |lambda_k| alpha_k K_k) / 2,
 // with the five dissipation components summed wave by wave: b_k = |lambda_k| alpha_k,
 //   D = (b1+b2+b5, b1 (u-c) + b2 u + b5 (u+c), D0 v + b3, D0 w + b4, b1 (H - u c) + b2 q^2/2 + b3 v + b4 w + b5 (H + u c)).
+// HAVE_E (cell-centred states): the total energies EL, ER and isL, isR = 1/sqrt(rho) are known.
 template <bool HAVE_E>
-__device__ __forceinline__ void roe_flux(double rL, double uL, double vL, double wL, double PL, double EL, double rR,
-                                         double uR, double vR, double wR, double PR, double ER, double gm1, double igm1,
-                                         double Fn[5]) {
+__device__ __forceinline__ void roe_flux(double rL, double uL, double vL, double wL, double PL, double EL, double isL,
+                                         double rR, double uR, double vR, double wR, double PR, double ER, double isR,
+                                         double gm1, double igm1, double Fn[5]) {
   const double eL = HAVE_E ? EL : fma(PL, igm1, (0.5 * rL) * fma(wL, wL, fma(vL, vL, uL * uL)));
   const double eR = HAVE_E ? ER : fma(PR, igm1, (0.5 * rR) * fma(wR, wR, fma(vR, vR, uR * uR)));
-  const double iL = rsqrt_fast(rL), iR = rsqrt_fast(rR);
+  const double iL = HAVE_E ? isL : rsqrt_fast(rL), iR = HAVE_E ? isR : rsqrt_fast(rR);
   const double sL = rL * iL, sR = rR * iR;
   const double iw = rcp_fast(sL + sR);
   const double aL = sL * iw, aR = sR * iw;

@@ -143,7 +143,8 @@ __device__ __forceinline__ void cell_flux(const double w0[7], const double w1[7]
   if (RS == 0)
     hllc_flux<true>(w0[0], w0[1], w0[2], w0[3], w0[4], w0[5], w0[6], w1[0], w1[1], w1[2], w1[3], w1[4], w1[5], w1[6], igm1, F);
   else
-    roe_flux<true>(w0[0], w0[1], w0[2], w0[3], w0[4], w0[6], w1[0], w1[1], w1[2], w1[3], w1[4], w1[6], gm1, igm1, F);
+    roe_flux<true>(w0[0], w0[1], w0[2], w0[3], w0[4], w0[6], w0[5], w1[0], w1[1], w1[2], w1[3], w1[4], w1[6], w1[5], gm1,
+                   igm1, F);
 }
 
 // predictor: first-order fluxes of the cell-centred states (reading R8)
@@ -203,7 +204,7 @@ __device__ __forceinline__ void corrector_flux(const double WLs[5], const double
     hllc_flux<false>(WLs[0], WLs[1], WLs[2], WLs[3], WLs[4], cL, 0.0, WRs[0], WRs[1], WRs[2], WRs[3], WRs[4], cR, 0.0,
                      igm1, Fn);
   } else {
-    roe_flux<false>(WLs[0], WLs[1], WLs[2], WLs[3], WLs[4], 0.0, WRs[0], WRs[1], WRs[2], WRs[3], WRs[4], 0.0,
+    roe_flux<false>(WLs[0], WLs[1], WLs[2], WLs[3], WLs[4], 0.0, 0.0, WRs[0], WRs[1], WRs[2], WRs[3], WRs[4], 0.0, 0.0,
                     gamma - 1.0, igm1, Fn);
   }
 }
@@ -325,6 +326,8 @@ __device__ __forceinline__ void issue_loads(const TensorMaps& tm, const StagePar
 // next block between two walks (12 warps finish it in a fraction of the time the 4 helper warps need,
 // and the helpers' chain staging -> conversion -> ready was what the walkers waited for): walker thread
 // t converts items t, t + 384 and (t < 128) t + 768 of the list [512 interior | z | x | y halo layers].
+// Slot 5 holds what the solver needs once per cell: c_s (HLLC, RS = 0) or 1/sqrt(rho) (Roe's weights, RS = 1).
+template <int RS>
 __device__ __forceinline__ void convert_cell(double* __restrict__ c, double gamma, double gm1) {
   double u[5], w[5];
 #pragma unroll
@@ -333,12 +336,13 @@ __device__ __forceinline__ void convert_cell(double* __restrict__ c, double gamm
 #pragma unroll
   for (int v = 1; v < 5; ++v) c[v * CVS] = w[v];
   const double c2 = (gamma * w[4]) * ir;                   // c_s^2 = gamma P / rho
-  c[5 * CVS] = c2 * rsqrt_fast(c2);
+  c[5 * CVS] = RS == 0 ? c2 * rsqrt_fast(c2) : rsqrt_fast(u[0]);
   c[6 * CVS] = u[4];                                       // total energy of the cell (eq. 8)
 }
 // halo item h in [0, 384): group g = h >> 7 (z, x, y), side = bit 6, x = h & 63.
 //   z: tile 0 layer kl = 1 (positions 64..127) / tile 5 layer kl = 0;  x: tile 6 odd positions (ll = 1) /
 //   tile 7 even positions;  y: tile 8 layer ll = 1 (positions 64..127) / tile 9 layer ll = 0
+template <int RS>
 __device__ __forceinline__ void convert_halo_item(double* __restrict__ L, const int* __restrict__ fsrc, int h,
                                                   double gamma, double gm1) {
   constexpr int TS = Cfg<0>::TS;
@@ -348,17 +352,18 @@ __device__ __forceinline__ void convert_halo_item(double* __restrict__ L, const 
   const int pos = g == 0 ? (hi ? 5 * TS + x : 64 + x)
                 : g == 1 ? (T_XLO + hi) * TS + 2 * x + (hi ? 0 : 1)
                          : (T_YLO + hi) * TS + (hi ? x : 64 + x);
-  convert_cell(L + pos, gamma, gm1);
+  convert_cell<RS>(L + pos, gamma, gm1);
 }
+template <int RS>
 __device__ __forceinline__ void convert_share(double* __restrict__ L, const int* __restrict__ fsrc, double gamma,
                                               double gm1, int tid) {
   constexpr int TS = Cfg<0>::TS;
-  convert_cell(L + (1 + (tid >> 7)) * TS + (tid & 127), gamma, gm1);          // interior tiles 1..3
+  convert_cell<RS>(L + (1 + (tid >> 7)) * TS + (tid & 127), gamma, gm1);          // interior tiles 1..3
   if (tid < 128) {
-    convert_cell(L + 4 * TS + tid, gamma, gm1);                                // interior tile 4
-    convert_halo_item(L, fsrc, tid + 256, gamma, gm1);                         // y halos
+    convert_cell<RS>(L + 4 * TS + tid, gamma, gm1);                                // interior tile 4
+    convert_halo_item<RS>(L, fsrc, tid + 256, gamma, gm1);                         // y halos
   } else {
-    convert_halo_item(L, fsrc, tid - 128, gamma, gm1);                         // z and x halos
+    convert_halo_item<RS>(L, fsrc, tid - 128, gamma, gm1);                         // z and x halos
   }
 }
 
@@ -477,7 +482,7 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
     auto convert_next = [&](int it) {                  // predictor: my share of block it, then both arrivals
       const int s = it & 1;
       mbar_wait(landed(s), (it >> 1) & 1);
-      convert_share(L0 + s * C::LAND, fsrc0 + 8 * s, gamma, gm1, tid);
+      convert_share<RS>(L0 + s * C::LAND, fsrc0 + 8 * s, gamma, gm1, tid);
       fence_proxy_async();                             // my generic-proxy writes, before a later TMA overwrites them
       __syncwarp();
       if ((tid & 31) == 0) { mbar_arrive(conv(s)); mbar_arrive(ready(s)); }
