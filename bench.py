@@ -28,7 +28,7 @@ CORRECTOR_BYTES_PER_CELL = 120.0   # read U^n, U^{n+1/2}, w
 PREDICTOR_BYTES_PER_CELL = 80.0    # read U^n, write U^{n+1/2}
 # dram__bytes_read.sum + dram__bytes_write.sum of one corrector launch on C2, from the ncu --set full
 # capture summarised in profiles/ (None until captured)
-CORRECTOR_TRAFFIC_BYTES_C2 = 1.492733e9 + 0.646058e9   # profiles/r1_c2_ncu_final.md
+CORRECTOR_TRAFFIC_BYTES_C2 = 1.490592e9 + 0.649133e9   # profiles/r1_c2_ncu_final.md
 # fp64 instructions (DFMA + DMUL + DADD + DSETP) per cell-update of the two stage kernels, counted on the ncu
 # source page (profiles/r1_c2_ncu_final.md), and the measured DFMA issue rate of this B200 (profiles/r1_fp64_peak.txt)
 FP64_INST_PER_CELL_UPDATE = 236.0 + 380.0
