@@ -443,3 +443,22 @@ def test_dynamic_regrid_cycle_matches_the_oracle():
     g.advance(2, 1)
     assert np.array_equal(o.nupd, g.nupd)
     compare(o, g, p.gamma, TOL10)
+
+
+def test_calls_run_on_the_callers_stream():
+    """Every call takes the stream the caller passes (torch's current stream in the binding): the same run on
+    a side stream gives the same bits, and work queued on that stream is ordered with it."""
+    import torch
+    p = PROBLEMS["amr-small"]()
+    g = gpu_for(p)
+    g.restrict_all(0)
+    g.advance(2, 1)
+    ref = g.get_state().cpu().numpy()
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        g2 = gpu_for(p)
+        g2.restrict_all(0)
+        g2.advance(2, 1)
+        out = g2.get_state()
+    side.synchronize()
+    assert np.array_equal(out.cpu().numpy(), ref)
