@@ -22,7 +22,8 @@
 //   tile 6, 7   the x-low / x-high halo  [k][j][ll]   (ll = layer, index increasing with x)
 //   tile 8, 9   the y-low / y-high halo  [ll][k][i]
 // Every pencil read of a half-warp is bank-conflict free in this layout (x pencils read cell PAIRS with
-// 128-bit loads).  The predictor's tiles carry two more variables (c_s, E) written by the conversion.
+// 128-bit loads).  The predictor's tiles carry two more variables (P, c_s) written by the conversion; the total
+// energy stays where it landed.
 #include <cmath>
 #include <cstdio>
 
@@ -77,7 +78,8 @@ __device__ __forceinline__ int cell_pos(int c, int a, int b) {
   return c < 0 ? lo : c >= N ? hi : in;
 }
 
-// one cell in the face frame of axis D: (rho, normal v, tangential v's, P[, c_s, E])
+// one cell in the face frame of axis D: corrector (rho, normal v, tangential v's, P), predictor (rho, normal v,
+// tangential v's, E, P, c_s)
 template <int NVW, int D>
 __device__ __forceinline__ void load_cell(const double* __restrict__ Wl, int o, double w[NVW]) {
   constexpr int vn = 1 + D, vt1 = 1 + (D + 1) % 3, vt2 = 1 + (D + 2) % 3;
@@ -137,13 +139,13 @@ __device__ __forceinline__ void store_regs(int src, int fs, double* R, double* F
 // A half pencil: faces f0 .. f0+4 and cells f0 .. f0+3, f0 = 0 or 4.  Face f lies between cells f-1 and f.
 // The loops are unrolled by two so that the carried cell/face state ping-pongs between registers.
 
-// flux of the cell-centred states w0 | w1 = (rho, u, v, w, P, c_s, E) with Riemann solver RS (0 HLLC, 1 Roe)
+// flux of the cell-centred states w0 | w1 = (rho, u, v, w, E, P, c_s or 1/sqrt(rho)) with Riemann solver RS (0 HLLC, 1 Roe)
 template <int RS>
 __device__ __forceinline__ void cell_flux(const double w0[7], const double w1[7], double gm1, double igm1, double F[5]) {
   if (RS == 0)
-    hllc_flux<true>(w0[0], w0[1], w0[2], w0[3], w0[4], w0[5], w0[6], w1[0], w1[1], w1[2], w1[3], w1[4], w1[5], w1[6], igm1, F);
+    hllc_flux<true>(w0[0], w0[1], w0[2], w0[3], w0[5], w0[6], w0[4], w1[0], w1[1], w1[2], w1[3], w1[5], w1[6], w1[4], igm1, F);
   else
-    roe_flux<true>(w0[0], w0[1], w0[2], w0[3], w0[4], w0[6], w0[5], w1[0], w1[1], w1[2], w1[3], w1[4], w1[6], w1[5], gm1,
+    roe_flux<true>(w0[0], w0[1], w0[2], w0[3], w0[5], w0[4], w0[6], w1[0], w1[1], w1[2], w1[3], w1[5], w1[4], w1[6], gm1,
                    igm1, F);
 }
 
@@ -326,7 +328,8 @@ __device__ __forceinline__ void issue_loads(const TensorMaps& tm, const StagePar
 // next block between two walks (12 warps finish it in a fraction of the time the 4 helper warps need,
 // and the helpers' chain staging -> conversion -> ready was what the walkers waited for): walker thread
 // t converts items t, t + 384 and (t < 128) t + 768 of the list [512 interior | z | x | y halo layers].
-// Slot 5 holds what the solver needs once per cell: c_s (HLLC, RS = 0) or 1/sqrt(rho) (Roe's weights, RS = 1).
+// Staged cell after the conversion: (rho, vx, vy, vz, E, P, x) with x what the solver needs once per cell: c_s
+// (HLLC, RS = 0) or 1/sqrt(rho) (Roe's weights, RS = 1).
 template <int RS>
 __device__ __forceinline__ void convert_cell(double* __restrict__ c, double gamma, double gm1) {
   double u[5], w[5];
@@ -334,10 +337,11 @@ __device__ __forceinline__ void convert_cell(double* __restrict__ c, double gamm
   for (int v = 0; v < 5; ++v) u[v] = c[v * CVS];
   const double ir = cons_to_prim(u, gm1, w);
 #pragma unroll
-  for (int v = 1; v < 5; ++v) c[v * CVS] = w[v];
+  for (int v = 1; v < 4; ++v) c[v * CVS] = w[v];
+  // slot 4 keeps the total energy of the cell as it landed (eq. 8); the pressure goes to slot 5
+  c[5 * CVS] = w[4];
   const double c2 = (gamma * w[4]) * ir;                   // c_s^2 = gamma P / rho
-  c[5 * CVS] = RS == 0 ? c2 * rsqrt_fast(c2) : rsqrt_fast(u[0]);
-  c[6 * CVS] = u[4];                                       // total energy of the cell (eq. 8)
+  c[6 * CVS] = RS == 0 ? c2 * rsqrt_fast(c2) : rsqrt_fast(u[0]);
 }
 // halo item h in [0, 384): group g = h >> 7 (z, x, y), side = bit 6, x = h & 63.
 //   z: tile 0 layer kl = 1 (positions 64..127) / tile 5 layer kl = 0;  x: tile 6 odd positions (ll = 1) /
