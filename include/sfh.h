@@ -2,7 +2,7 @@
  * of arxiv/paper_2604_21438 (SFUMATO#), B200 (sm_100a) only.
  *
  * What the calls compute is defined by PAPER.md (cited per call as PAPER.md:<line>) and, where the
- * paper is silent, by the readings R1..R28 of DESIGN.md.  There is no CPU fallback: every call that
+ * paper is silent, by the readings R1..R31 of DESIGN.md.  There is no CPU fallback: every call that
  * touches field data launches CUDA kernels on the caller's stream and returns SFH_ECUDA when no
  * device is usable.
  *
@@ -20,7 +20,9 @@
  *     them from the neighbours' interiors through the neighbour map); only ghost slabs on
  *     coarse-fine faces are materialised (in the work buffer) by sfh_fill_ghosts.
  *   - Three state copies ("roles"): 0 = U^n, 1 = U^{n+1/2}, 2 = U^{n+1} (values "at
- *     the current, previous, and half timesteps" are kept for temporal interpolation).
+ *     the current, previous, and half timesteps" are kept for temporal interpolation).  The library
+ *     keeps role 1 as primitives (rho, v, P) internally; every copy crosses this interface as
+ *     conserved variables.
  *   - Pointers: "host" = ordinary host memory, "device" = CUDA device memory of the current
  *     device.  `stream` is a cudaStream_t passed as void* (NULL = default stream).  Calls are
  *     asynchronous on that stream unless they return a host scalar (noted per call).
