@@ -17,7 +17,10 @@
 // HLLC identities, conservation to round-off on periodic AMR meshes with flux correction
 // (and its failure with reflux switched off), uniform == fully refined bitwise, mirror
 // symmetry, free-stream preservation, eq. (16) closed forms, eq. (14)-(15) table,
-// prolong/restrict identities, 1-D invariance, contact advection, 2nd-order convergence.
+// prolong/restrict identities, 1-D invariance, contact advection, 2nd-order convergence; the time axis
+// (tests/test_oracle_time_pins.py): linear advection exact to round-off on a sub-cycled AMR mesh (fixes
+// the tau / tau_half schedule of advance_adaptive and the copies fill_ghosts_level reads), fill_ghosts at
+// tau in {0, 1/4, 1/2, 3/4, 1} against the expanded eq. (16), the CFL step in closed form.
 // Parity unpinned by the paper (any reasonable choice passes every pin; fixed only by
 // DESIGN.md): Davis wave speeds (R6), first-order predictor (R8), primitive-variable
 // reconstruction (R11), minmod limiter (R12), CFL speed definition (R16), the entropy-fix width of
