@@ -161,8 +161,7 @@ def whole_job_value(cu_per_rank, ms, world):
 
 def oracle_sample(config, scale_hint, riemann="hllc"):
     """The oracle on a bounded sample of the same workload: the same recipe on a smaller base grid."""
-    sys.path.insert(0, os.path.join(ROOT, "tests"))
-    from helpers import oracle_for
+    from oracle import oracle_for
     from sfh_inputs import make_config
     sample_scale = {"C1": 1, "C2": 1, "C3": 2, "C4": 2, "C5": 4}[config] * max(1, scale_hint)
     p = make_config(config, sample_scale)

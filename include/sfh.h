@@ -135,8 +135,8 @@ int sfh_get_ghosted(sfh_mesh* m, int which, double* d_G, void* stream);
  *   SFH_REFINE_JEANS      PAPER.md:641: max over the cells of h / lambda_J, lambda_J = c_s sqrt(pi / (G rho))
  *                         (the paper refines where the Jeans length spans fewer than 8 cells: > 1/8).
  * Reads one ghost layer of state copy `which`: same-level and outflow halos are gathered, coarse-fine
- * halos come from the slabs of the last sfh_fill_ghosts(which) -- call that first on refined meshes.
- * Asynchronous on `stream`.  SFH_EINVAL for an unknown criterion or G <= 0 with the Jeans criterion. */
+ * halos are prolonged from the same copy of the coarser level first (the call refills the slabs of `which`
+ * itself, as sfh_fill_ghosts(-1, which, 0, 0) would).  Asynchronous on `stream`.  SFH_EINVAL for an unknown criterion or G <= 0 with the Jeans criterion. */
 #define SFH_REFINE_CURVATURE 0
 #define SFH_REFINE_JEANS 1
 int sfh_refine_indicator(sfh_mesh* m, int which, int criterion, double G, double* d_out, void* stream);
@@ -146,7 +146,8 @@ int sfh_refine_indicator(sfh_mesh* m, int which, int criterion, double G, double
  * parent by the slope-limited conservative prolongation of reading R3 (so restricting the new children gives the
  * parent back); blocks that disappear are dropped (their parents hold the restricted data).  A new block whose
  * parent is not in the old mesh gives SFH_EMESH: refine by one level per regrid.  Only the conserved copies
- * (0 and 2).  Reads the old mesh's coarse-fine ghost slabs: call sfh_fill_ghosts(src, -1, src_which, 0, 0) first.
+ * (0 and 2).  Refills the old mesh's coarse-fine ghost slabs from src_which itself (the prolongation stencils of
+ * new blocks next to an old coarse-fine face read them).
  * The caller builds `dst` (sfh_create_mesh from the flags of sfh_refine_indicator, padded to 2:1) and binds it.
  * Synchronous (it uploads a block map and waits for the copy). */
 int sfh_transfer_state(sfh_mesh* src, int src_which, sfh_mesh* dst, int dst_which, void* stream);
@@ -154,7 +155,8 @@ int sfh_transfer_state(sfh_mesh* src, int src_which, sfh_mesh* dst, int dst_whic
 /* CFL time step (reading R16): dt = cfl * h_l / max over all cells of level l of
  * (max_d |v_d| + c_s), c_s = sqrt(gamma P / rho), from role 0; level = -1: minimum over levels
  * ("grid-level reductions").  Warp-shuffle + atomic-max reduction
- * (exact).  Returns the value in *dt_host: synchronises the stream. */
+ * (exact).  Returns the value in *dt_host: synchronises the stream.  SFH_ESTATE if the step is not finite and
+ * positive (a level without a single finite positive speed: see sfh_status). */
 int sfh_cfl_dt(sfh_mesh* m, int level, double* dt_host, void* stream);
 
 /* One predictor-corrector update of `level` (-1: every level) by dt   (R8-R14):
@@ -190,7 +192,9 @@ int sfh_end_step(sfh_mesh* m, int level);
  * round trip.  mode 1 = adaptive: Berger-Colella recursion; the step of level l+1 is
  * dt_l 2^-n with n = min{m >= 0 : dt_l 2^-m <= dt_CFL^{l+1}} (eq. 14-15); level 0 uses dt_fixed if
  * > 0 else its CFL step.  Adds the elapsed time to *t_host and the number of updates of each level
- * to nupd_host[0..max_level] (either may be NULL).  Synchronises the stream before returning. */
+ * to nupd_host[0..max_level] (either may be NULL).  Synchronises the stream before returning.  SFH_ESTATE if
+ * a CFL step is not finite and positive or a level would need more than 2^20 sub-steps of its parent (both
+ * mean the state holds bad cells, reading R28; the state is left as it was when that was detected). */
 int sfh_advance(sfh_mesh* m, int ncoarse_steps, int mode, double dt_fixed, double* t_host,
                 int64_t* nupd_host, void* stream);
 

@@ -196,3 +196,11 @@ class OracleMesh:
         if rc != 0:
             raise RuntimeError("orc_get: unresolved cell")
         return out
+
+
+def oracle_for(p, U=None):
+    """OracleMesh of a problem description `p` (fields nb0, max_level, bc, box_len, gamma, cfl, level, ijk, U:
+    sfh_inputs.Problem), holding U (default p.U) as its copy 0."""
+    m = OracleMesh(p.nb0, p.max_level, p.bc, p.box_len, p.gamma, p.cfl, p.level, p.ijk)
+    m.set_state(p.U if U is None else U)
+    return m

@@ -37,7 +37,6 @@ def build(force=False, nofma=False, verbose=False):
         cmd += ["-fmad=false"]
     if verbose:
         cmd += ["-Xptxas", "-v"]
-    cmd += os.environ.get("SFH_NVCC_EXTRA", "").split()   # e.g. -DSFH_DEBUG_TIMING (development aid)
     cmd += [os.path.join(CSRC, f) for f in SOURCES]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or res.returncode != 0:

@@ -20,6 +20,7 @@ void set_error(const std::string& s) { g_err = s; }
 struct sfh_mesh {
   HostMesh hm;
   bool bound = false;
+  int sms = 1;                          // SM count of the device (persistent grids: one CTA per SM)
   int riemann = SFH_RIEMANN_HLLC;
   char* dev_tables = nullptr;
   int32_t *d_face_src = nullptr, *d_fslot = nullptr, *d_nbr27 = nullptr, *d_parent = nullptr, *d_child0 = nullptr,
@@ -218,10 +219,11 @@ int stage_level(sfh_mesh* m, int l, int stage, Dt dt, cudaStream_t st) {
   p.use_regs = stage == 1 && (hm.cf_count[l] > 0 || hm.reflux_count[l] > 0);
   p.riemann = m->riemann;
   p.bmax = stage == 1 ? m->bmax : nullptr;
-  if (stage == 1) m->bmax_pending[l] = true;
+  // the corrector overwrites the level's cached maxima with those of U^{n+1}: they stop describing U^n now
+  if (stage == 1) { m->bmax_pending[l] = true; m->bmax_valid[l] = false; }
   {
     Timed tmr(m, stage, st);
-    CU(launch_stage(stage, m->tm[m->role[l][src_role]], p, st), "stage_kernel");
+    CU(launch_stage(stage, m->tm[m->role[l][src_role]], p, m->sms, st), "stage_kernel");
   }
   m->launches += 1;
   return SFH_OK;
@@ -247,6 +249,7 @@ int hydro_level(sfh_mesh* m, int l, Dt dt, int interp, double tau, double dtau, 
 int flux_correct_level(sfh_mesh* m, int lc, Dt dt, cudaStream_t st) {
   const HostMesh& hm = m->hm;
   if (lc + 1 >= hm.nlev || hm.lev_count[lc + 1] == 0) return SFH_OK;
+  m->bmax_valid[lc] = false;      // restriction and reflux rewrite entries with the maxima of role 2
   {
     Timed tmr(m, 3, st);
     CU(launch_restrict(role_buf(m, lc + 1, 0), role_buf(m, lc, 2), m->d_restrict_list + hm.restrict_first[lc],
@@ -273,10 +276,11 @@ int max_speed_level(sfh_mesh* m, int l, cudaStream_t st) {
   const HostMesh& hm = m->hm;
   Timed tmr(m, 5, st);
   if (m->bmax_valid[l])
-    CU(launch_max_cached(m->bmax, int(hm.lev_first[l]), int(hm.lev_count[l]), m->smax + l, st), "max_cached_kernel");
+    CU(launch_max_cached(m->bmax, int(hm.lev_first[l]), int(hm.lev_count[l]), m->smax + l, m->sms, st),
+       "max_cached_kernel");
   else
-    CU(launch_max_speed(role_buf(m, l, 0), int(hm.lev_first[l]), int(hm.lev_count[l]), hm.cfg.gamma, m->smax + l, st),
-       "max_speed_kernel");
+    CU(launch_max_speed(role_buf(m, l, 0), int(hm.lev_first[l]), int(hm.lev_count[l]), hm.cfg.gamma, m->smax + l,
+                        m->sms, st), "max_speed_kernel");
   m->launches += hm.lev_count[l] > 0;
   return SFH_OK;
 }
@@ -294,16 +298,25 @@ int cfl_host(sfh_mesh* m, int level, double* dt_out, cudaStream_t st) {
     if ((level < 0 || level == l) && hm.lev_count[l] > 0) {
       double s;
       std::memcpy(&s, &bits[l], 8);
-      dt = std::fmin(dt, hm.cfg.cfl * hm.h[l] / s);
+      const double dtl = hm.cfg.cfl * hm.h[l] / s;
+      // a NaN speed never wins the device's max (R28: bad cells are reported, not floored), so s = 0 or inf here
+      // means the level holds no finite positive speed at all
+      if (!(dtl > 0.0) || !std::isfinite(dtl)) {
+        char buf[128];
+        snprintf(buf, sizeof buf, "CFL step of level %d is not finite and positive (max speed %g): bad cells? (sfh_status)", l, s);
+        return fail(SFH_ESTATE, buf);
+      }
+      dt = std::fmin(dt, dtl);
     }
   *dt_out = dt;
   return SFH_OK;
 }
 
 // eq. (14)-(15): smallest n >= 0 with dtH 2^-n <= dt_cfl (reading R18)
+constexpr int MAX_SUBSTEP_EXPONENT = 20;   // 2^20 sub-steps of one parent step: beyond any sane hierarchy
 int substep_exponent(double dtH, double dt_cfl) {
   int n = 0;
-  while (n < 30 && std::ldexp(dtH, -n) > dt_cfl) ++n;
+  while (n <= MAX_SUBSTEP_EXPONENT && std::ldexp(dtH, -n) > dt_cfl) ++n;
   return n;
 }
 
@@ -319,6 +332,12 @@ int advance_adaptive(sfh_mesh* m, int l, double dt, double tau, double dtau, int
     double dtc;
     if ((rc = cfl_host(m, l + 1, &dtc, st))) return rc;
     const int n = substep_exponent(dt, dtc);
+    if (n > MAX_SUBSTEP_EXPONENT) {
+      char buf[160];
+      snprintf(buf, sizeof buf, "level %d would need more than 2^%d sub-steps of its parent (dt %g, CFL step %g): bad cells?",
+               l + 1, MAX_SUBSTEP_EXPONENT, dt, dtc);
+      return fail(SFH_ESTATE, buf);
+    }
     const double dtf = std::ldexp(dt, -n);
     const int nsub = 1 << n;
     for (int s = 0; s < nsub; ++s)
@@ -467,10 +486,16 @@ int sfh_bind(sfh_mesh* m, void* d_state0, void* d_state1, void* d_state2, void* 
     size_t off = 0;
     for (const Item& it : items) {
       *it.dst = m->dev_tables + off;
-      if (it.bytes) CU(cudaMemcpy(m->dev_tables + off, it.src, it.bytes, cudaMemcpyHostToDevice), "upload tables");
+      if (it.bytes) e = cudaMemcpy(m->dev_tables + off, it.src, it.bytes, cudaMemcpyHostToDevice);
+      if (e != cudaSuccess) break;
       off += up(it.bytes + 1);
     }
-    CU(configure_kernels(), "cudaFuncSetAttribute");
+    if (e == cudaSuccess) e = configure_kernels(&m->sms);
+    if (e != cudaSuccess) {          // never keep half-uploaded tables: the next sfh_bind starts over
+      cudaFree(m->dev_tables);
+      m->dev_tables = nullptr;
+      return cuda_fail(e, "upload of the mesh tables / kernel configuration");
+    }
   }
   m->state[0] = static_cast<double*>(d_state0);
   m->state[1] = static_cast<double*>(d_state1);
@@ -493,6 +518,8 @@ int sfh_bind(sfh_mesh* m, void* d_state0, void* d_state1, void* d_state2, void* 
     if (rc) return rc;
   }
   for (int l = 0; l < MAX_LEVELS; ++l) for (int r = 0; r < 3; ++r) m->role[l][r] = r;
+  // the uploads and the memset above ran on the legacy stream: the caller's (non-blocking) streams see them done
+  CU(cudaDeviceSynchronize(), "cudaDeviceSynchronize");
   m->bound = true;
   return SFH_OK;
 }
@@ -550,6 +577,9 @@ int sfh_refine_indicator(sfh_mesh* m, int which, int criterion, double G, double
   if (which < 0 || which > 2 || !d_out) return fail(SFH_EINVAL, "bad argument");
   if (criterion != SFH_REFINE_CURVATURE && criterion != SFH_REFINE_JEANS) return fail(SFH_EINVAL, "unknown criterion");
   if (criterion == SFH_REFINE_JEANS && !(G > 0.0)) return fail(SFH_EINVAL, "G must be positive");
+  // the coarse-fine slabs may hold anything (time-interpolated values of the last sub-step): refill them
+  for (int l = 1; l < m->hm.nlev; ++l)
+    if ((rc = fill_level(m, l, which, 0, 0.0, S(stream)))) return rc;
   for (int l = 0; l < m->hm.nlev; ++l) {
     CU(launch_refine_indicator(role_buf(m, l, which), which == 1 ? m->ghost1 : m->ghost, m->d_face_src, m->d_perm,
                                int(m->hm.lev_first[l]), int(m->hm.lev_count[l]), which == 1, m->hm.cfg.gamma, criterion,
@@ -594,6 +624,9 @@ int sfh_transfer_state(sfh_mesh* src, int src_which, sfh_mesh* dst, int dst_whic
     return fail(SFH_ENOMEM, "out of host memory");
   }
   cudaStream_t st = S(stream);
+  // the prolongation stencils read the old mesh's coarse-fine slabs: refill them from src_which
+  for (int l = 1; l < hs.nlev; ++l)
+    if ((rc = fill_level(src, l, src_which, 0, 0.0, st))) return rc;
   int32_t* d_tsrc = nullptr;
   if (cudaMalloc((void**)&d_tsrc, tsrc.size() * 4) != cudaSuccess) return fail(SFH_ENOMEM, "cudaMalloc of the transfer table failed");
   cudaError_t e = cudaMemcpyAsync(d_tsrc, tsrc.data(), tsrc.size() * 4, cudaMemcpyHostToDevice, st);
@@ -656,7 +689,7 @@ int sfh_restrict(sfh_mesh* m, int coarse_level, int src_role, int dst_role, void
     return fail(SFH_EINVAL, "the half-step state (role 1) is never restricted (DESIGN.md reading R10)");
   if (coarse_level + 1 >= hm.nlev || hm.restrict_count[coarse_level] == 0) return SFH_OK;
   // the cached block maxima follow a restriction into U^{n+1} (role 2); one into U^n invalidates them
-  if (dst_role == 0) m->bmax_valid[coarse_level] = false;
+  m->bmax_valid[coarse_level] = false;     // (into role 2: the entries are rewritten with role-2 maxima)
   CU(launch_restrict(role_buf(m, coarse_level + 1, src_role), role_buf(m, coarse_level, dst_role),
                      m->d_restrict_list + hm.restrict_first[coarse_level], m->d_child0,
                      int(hm.restrict_count[coarse_level]), hm.cfg.gamma, dst_role == 2 ? m->bmax : nullptr, S(stream)),
@@ -753,7 +786,7 @@ int sfh_status(sfh_mesh* m, int which, int64_t* n_bad_cells, void* stream) {
   CU(cudaMemsetAsync(m->nbad, 0, 8, st), "memset");
   for (int l = 0; l < m->hm.nlev; ++l) {
     CU(launch_count_bad(role_buf(m, l, which), int(m->hm.lev_first[l]), int(m->hm.lev_count[l]), m->hm.cfg.gamma,
-                        which == 1, m->nbad, st), "count_bad_kernel");
+                        which == 1, m->nbad, m->sms, st), "count_bad_kernel");
     m->launches += m->hm.lev_count[l] > 0;
   }
   unsigned long long n = 0;

@@ -25,7 +25,6 @@
 // 128-bit loads).  The predictor's tiles carry two more variables (P, c_s) written by the conversion; the total
 // energy stays where it landed.
 #include <cmath>
-#include <cstdio>
 
 #include "sfh_device.cuh"
 #include "sfh_kernels.cuh"
@@ -492,22 +491,13 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
       if ((tid & 31) == 0) { mbar_arrive(conv(s)); mbar_arrive(ready(s)); }
     };
     if (STAGE == 0) convert_next(0);
-#ifdef SFH_DEBUG_TIMING
-    long long tw[3] = {0, 0, 0}, t0, t1;
-#endif
     for (int it = 0; it < n; ++it) {
       const int s = it & 1, d = it % C::NDF;
-#ifdef SFH_DEBUG_TIMING
-      t0 = clock64();
-#endif
       const double* Wl = L0 + s * C::LAND;
       double* dF = dF0 + d * DF_DOUBLES;
       const bool we = it >= C::NDF;
       const uint32_t pe = ((it / C::NDF) - 1) & 1;
       mbar_wait(ready(s), (it >> 1) & 1);
-#ifdef SFH_DEBUG_TIMING
-      t1 = clock64(); tw[0] += t1 - t0;
-#endif
       if (STAGE == 0) {
         if (D == 0) walk_predictor<RS, 0>(Wl, dF, a, b, f0, gm1, igm1, empty(d), pe, we);
         else if (D == 1) walk_predictor<RS, 1>(Wl, dF, a, b, f0, gm1, igm1, empty(d), pe, we);
@@ -518,18 +508,8 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
       }
       __syncwarp();
       if ((tid & 31) == 0) mbar_arrive(full(d));
-#ifdef SFH_DEBUG_TIMING
-      tw[1] += clock64() - t1; t1 = clock64();
-#endif
       if (STAGE == 0 && it + 1 < n) convert_next(it + 1);
-#ifdef SFH_DEBUG_TIMING
-      tw[2] += clock64() - t1;
-#endif
     }
-#ifdef SFH_DEBUG_TIMING
-    if (blockIdx.x == 5 && (tid & 127) == 0)
-      printf("stage %d walker D=%d n=%d: per block wait_ready %lld  walk(+wait_empty) %lld  convert %lld\n", STAGE, D, n, tw[0] / n, tw[1] / n, tw[2] / n);
-#endif
   } else {
     // ------------------------------------------------------------------------------ helpers
     if (STAGE == 1) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(HELP_REGS));
@@ -566,15 +546,9 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
     }
     __syncwarp();
     for (int it = 0; it < 2 && it < n; ++it) prepare(it);
-#ifdef SFH_DEBUG_TIMING
-    long long th[5] = {0, 0, 0, 0, 0}, t0, t1;
-#endif
     for (int it = 0; it < n; ++it) {
       const int s = it & 1, d = it % C::NDF;
       const int blk = blk0 + it * stride;
-#ifdef SFH_DEBUG_TIMING
-      t0 = clock64();
-#endif
       // U^n of the block and the face sources of the block after next: in flight while the walkers finish
       double un[HC][NV];
       const double* Un = p.Un + size_t(blk) * BLK;
@@ -585,9 +559,6 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
       int snext[6];
       if (lane0 && it + 2 < n) load_src(it + 2, snext);
       mbar_wait(full(d), (it / C::NDF) & 1);
-#ifdef SFH_DEBUG_TIMING
-      t1 = clock64(); th[0] += t1 - t0; t0 = t1;
-#endif
       if (lane0 && it + 2 < n) {                       // the walkers are done with staging buffer s as well
         issue_loads<STAGE>(tm, p, blk + 2 * stride, snext, hw, L0 + s * C::LAND, fsrc0 + 8 * s, landed(s));
         if (hw == 3 && it + 3 < n) {
@@ -596,22 +567,11 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
         }
       }
       __syncwarp();
-#ifdef SFH_DEBUG_TIMING
-      t1 = clock64(); th[1] += t1 - t0; t0 = t1;
-#endif
       combine_fluxes(dF0 + d * DF_DOUBLES, un, lam, hid);
       __syncwarp();
       if (lane0) mbar_arrive(empty(d));                // the walkers may store the next flux differences
       store_block<STAGE == 0>(un, gm1, p.Udst + size_t(blk) * BLK, hid);
-#ifdef SFH_DEBUG_TIMING
-      t1 = clock64(); th[2] += t1 - t0; t0 = t1;
-      if (it + 2 < n) mbar_wait(landed(s), ((it + 2) >> 1) & 1);
-      t1 = clock64(); th[3] += t1 - t0; t0 = t1;
-#endif
       if (it + 2 < n) prepare(it + 2);
-#ifdef SFH_DEBUG_TIMING
-      t1 = clock64(); th[4] += t1 - t0;
-#endif
       if (STAGE == 1 && p.bmax) {
         // Off the walkers' critical path (everything they wait for has been handed over): the block's maximum
         // CFL speed for the next step's dt (reading R16) from the updated cells still in registers.
@@ -625,15 +585,8 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
         if (hid == 0) p.bmax[blk] = fmax(fmax(hm[0], hm[1]), fmax(hm[2], hm[3]));
       }
     }
-#ifdef SFH_DEBUG_TIMING
-    if (blockIdx.x == 5 && lane0)
-      printf("stage %d helper warp %d n=%d: per block wait_full %lld  issue %lld  update %lld  wait_landed %lld  prepare %lld\n",
-             STAGE, hw, n, th[0] / n, th[1] / n, th[2] / n, th[3] / n, th[4] / n);
-#endif
   }
 }
-
-static int g_stage_ctas = 148;   // persistent grid: one CTA per SM (set by configure_kernels)
 
 template <int STAGE, int RS, bool REGS>
 static cudaError_t configure_one() {
@@ -641,16 +594,19 @@ static cudaError_t configure_one() {
                               Cfg<STAGE>::SMEM);
 }
 
-cudaError_t configure_kernels() {
+// Raises the dynamic shared-memory limit of the stage kernels and returns the SM count of the current
+// device (the persistent grid is one CTA per SM).
+cudaError_t configure_kernels(int* sm_count) {
   cudaError_t e;
   if ((e = configure_one<0, 0, false>()) != cudaSuccess || (e = configure_one<0, 1, false>()) != cudaSuccess ||
       (e = configure_one<1, 0, false>()) != cudaSuccess || (e = configure_one<1, 0, true>()) != cudaSuccess ||
       (e = configure_one<1, 1, false>()) != cudaSuccess || (e = configure_one<1, 1, true>()) != cudaSuccess)
     return e;
   int dev = 0, sms = 0;
-  if (cudaGetDevice(&dev) == cudaSuccess &&
-      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
-    g_stage_ctas = sms;
+  if ((e = cudaGetDevice(&dev)) != cudaSuccess ||
+      (e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess)
+    return e;
+  *sm_count = sms > 0 ? sms : 1;
   return cudaSuccess;
 }
 
@@ -661,9 +617,9 @@ static void launch_one(int grid, const TensorMaps& tm, const StageParams& p, cud
 
 // The corrector of a level with flux-register faces is its own instantiation: the register code costs the
 // uniform-grid walk a few per cent even when it never runs (measured).
-cudaError_t launch_stage(int stage, const TensorMaps& tm, const StageParams& p, cudaStream_t st) {
+cudaError_t launch_stage(int stage, const TensorMaps& tm, const StageParams& p, int sms, cudaStream_t st) {
   if (p.count <= 0) return cudaSuccess;
-  const int grid = p.count < g_stage_ctas ? p.count : g_stage_ctas;
+  const int grid = p.count < sms ? p.count : sms;
   const bool roe = p.riemann != 0;
   if (stage == 0) {
     if (roe) launch_one<0, 1, false>(grid, tm, p, st); else launch_one<0, 0, false>(grid, tm, p, st);

@@ -67,7 +67,8 @@ struct ProlongParams {
   double tau1;
 };
 
-cudaError_t launch_stage(int stage, const TensorMaps& tm, const StageParams& p, cudaStream_t st);
+// sms: SM count of the device (configure_kernels): the persistent grid is min(count, sms) CTAs
+cudaError_t launch_stage(int stage, const TensorMaps& tm, const StageParams& p, int sms, cudaStream_t st);
 cudaError_t launch_prolong(const ProlongParams& p, cudaStream_t st);
 // bmax (nullable): per-block maximum CFL speed, rewritten for the blocks the kernel changes
 cudaError_t launch_restrict(const double* Ufine, double* Ucoarse, const int32_t* list, const int32_t* child0,
@@ -76,8 +77,8 @@ cudaError_t launch_reflux(double* U, const double* R, const double* FH, const in
                           const int32_t* fh_src, int count, double h, double dt, const double* dt_dev,
                           double gamma, double* bmax, cudaStream_t st);
 cudaError_t launch_max_speed(const double* U, int first, int count, double gamma, unsigned long long* smax_bits,
-                             cudaStream_t st);
-cudaError_t launch_max_cached(const double* bmax, int first, int count, unsigned long long* smax_bits,
+                             int sms, cudaStream_t st);
+cudaError_t launch_max_cached(const double* bmax, int first, int count, unsigned long long* smax_bits, int sms,
                               cudaStream_t st);
 struct LevelInfo {
   double h[MAX_LEVELS];
@@ -88,7 +89,7 @@ struct LevelInfo {
 cudaError_t launch_dt_finalize(const unsigned long long* smax_bits, const LevelInfo& li, double cfl, double* dt_dev,
                                double* t_dev, cudaStream_t st);
 cudaError_t launch_count_bad(const double* U, int first, int count, double gamma, int prim, unsigned long long* nbad,
-                             cudaStream_t st);
+                             int sms, cudaStream_t st);
 // dst[slot][...] = src[perm[slot]][...] (to_internal) or the inverse, for slots [first, first+count)
 // prim: the internal copy holds primitives (role 1); the caller's copy is always conserved
 cudaError_t launch_permute(const double* src, double* dst, const int64_t* perm, int first, int count, int to_internal,
@@ -103,6 +104,6 @@ cudaError_t launch_refine_indicator(const double* U, const double* ghost, const 
 // Uc / Us: the old buffers holding the block's own level (copies) and its parent level (prolongation)
 cudaError_t launch_transfer(const double* Uc, const double* Us, const double* ghost_s, const int32_t* face_src_s,
                             const int32_t* tsrc, const int32_t* coord_d, double* Ud, int count, cudaStream_t st);
-cudaError_t configure_kernels();
+cudaError_t configure_kernels(int* sm_count);
 
 }  // namespace sfh

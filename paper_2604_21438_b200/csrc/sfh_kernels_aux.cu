@@ -300,20 +300,20 @@ __global__ void __launch_bounds__(256) max_cached_kernel(const double* __restric
   if (threadIdx.x == 0) atomicMax(smax_bits, (unsigned long long)__double_as_longlong(smax));
 }
 
-cudaError_t launch_max_cached(const double* bmax, int first, int count, unsigned long long* smax_bits,
+cudaError_t launch_max_cached(const double* bmax, int first, int count, unsigned long long* smax_bits, int sms,
                               cudaStream_t st) {
   cudaError_t e = cudaMemsetAsync(smax_bits, 0, sizeof(unsigned long long), st);
   if (e != cudaSuccess || count <= 0) return e;
   const int need = (count + 2047) / 2048;
-  max_cached_kernel<<<need < 148 ? need : 148, 256, 0, st>>>(bmax, first, count, smax_bits);
+  max_cached_kernel<<<need < sms ? need : sms, 256, 0, st>>>(bmax, first, count, smax_bits);
   return cudaGetLastError();
 }
 
 cudaError_t launch_max_speed(const double* U, int first, int count, double gamma, unsigned long long* smax_bits,
-                             cudaStream_t st) {
+                             int sms, cudaStream_t st) {
   cudaError_t e = cudaMemsetAsync(smax_bits, 0, sizeof(unsigned long long), st);
   if (e != cudaSuccess || count <= 0) return e;
-  const int grid = count < 148 * 8 ? count : 148 * 8;
+  const int grid = count < sms * 8 ? count : sms * 8;
   max_speed_kernel<<<grid, 256, 0, st>>>(U, first, count, gamma, smax_bits);
   return cudaGetLastError();
 }
@@ -356,9 +356,9 @@ __global__ void __launch_bounds__(256) count_bad_kernel(const double* __restrict
 }
 
 cudaError_t launch_count_bad(const double* U, int first, int count, double gamma, int prim, unsigned long long* nbad,
-                             cudaStream_t st) {
+                             int sms, cudaStream_t st) {
   if (count <= 0) return cudaSuccess;
-  const int grid = count < 148 * 8 ? count : 148 * 8;
+  const int grid = count < sms * 8 ? count : sms * 8;
   count_bad_kernel<<<grid, 256, 0, st>>>(U, first, count, gamma, prim, nbad);
   return cudaGetLastError();
 }

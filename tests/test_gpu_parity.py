@@ -462,3 +462,93 @@ def test_calls_run_on_the_callers_stream():
         out = g2.get_state()
     side.synchronize()
     assert np.array_equal(out.cpu().numpy(), ref)
+
+
+# ------------------------------------------------------------------ the time axis (tests/test_oracle_time_pins.py on the CUDA path)
+@pytest.mark.parametrize("mode", [1, 0])
+def test_linear_advection_exact_on_subcycled_amr_mesh(mode):
+    """T1 of the oracle's time pins, on the CUDA path: against the ANALYTIC field (away from the outflow
+    boundary) and against the oracle.  A wrong tau in the level driver or in the dual ghost fill shows here
+    even if the oracle shared the mistake."""
+    from test_oracle_time_pins import advected, advection_problem, interior_mask
+    from sfh_inputs.configs import cell_centres
+    p = advection_problem(mode)
+    o, g = both(p)
+    X, Y, Z = cell_centres(p.level, p.ijk, p.nb0)
+    for step in (1, 2):
+        o.advance(1, mode)
+        g.advance(1, mode)
+        assert np.array_equal(o.nupd, g.nupd)
+        if mode == 1:
+            assert tuple(g.nupd) == (step, 2 * step, 4 * step)
+        assert abs(g.t.value - o.t.value) <= 1e-14 * o.t.value
+        Ug = g.get_state().cpu().numpy()
+        err = np.abs(Ug - advected(X, Y, Z, g.t.value))
+        sel = interior_mask(p, 3 * step + 2)
+        worst = err.transpose(1, 0, 2, 3, 4)[:, sel].max()
+        assert worst < 4e-14, (step, worst)
+        compare(o, g, p.gamma, TOL1)
+
+
+@pytest.mark.parametrize("tau", [0.0, 0.25, 0.5, 0.75, 1.0])
+def test_fill_ghosts_closed_form_on_linear_coarse_copies(tau):
+    """T2 of the oracle's time pins on the CUDA path: face ghost slabs of the fine level against the analytic
+    value (eq. 16 expanded, linear coarse data prolonged exactly)."""
+    from test_oracle_time_pins import evaluate, ghost_centres, linear_copies
+    from sfh_inputs.configs import cell_centres
+    p = problem_from_tree(small_amr_tree(4, 1, periodic=(False, False, False)), mode=1)
+    g = sfh.Mesh.from_problem(p)
+    rng = np.random.default_rng(21)
+    coarse, fine = linear_copies(rng), linear_copies(rng)
+    # positive density and pressure in every copy (role 1 is held as primitives inside the library)
+    for c in (coarse, fine):
+        c[:, 0, 0] = 4.0
+        c[:, 0, 1:] *= 0.3
+        c[:, 4, 0] = 40.0
+    X, Y, Z = cell_centres(p.level, p.ijk, p.nb0)
+    is_fine = (p.level == 1)[:, None, None, None, None]
+    for k in range(3):
+        g.set_state(np.where(is_fine, evaluate(fine[k], X, Y, Z), evaluate(coarse[k], X, Y, Z)), k)
+    w = np.array([(1 - tau) ** 2, 2 * tau * (1 - tau), tau ** 2])
+    lo, hi = 16, 48
+    fm = face_mask()
+    for which in (0, 1):
+        for interp in (1, 0):
+            g.fill_ghosts(1, which, interp, tau)
+            G = g.get_ghosted(which).cpu().numpy()
+            checked = 0
+            for b in np.nonzero(p.level == 1)[0]:
+                gx, gy, gz = ghost_centres(p, b)
+                I, J, K = (np.rint(a * 64 - 0.5).astype(int) for a in (gx, gy, gz))
+                inside = (I >= lo) & (I < hi) & (J >= lo) & (J < hi) & (K >= lo) & (K < hi)
+                if interp:
+                    from_coarse = sum(w[k] * evaluate(coarse[k], gx, gy, gz, 0) for k in range(3))
+                else:
+                    from_coarse = evaluate(coarse[which], gx, gy, gz, 0)
+                expect = np.where(inside[None], evaluate(fine[which], gx, gy, gz, 0), from_coarse)
+                sel = fm & ~inside
+                d = np.abs(G[b] - expect)[:, sel]
+                if sel.any():
+                    assert d.max() < 2e-12, (which, interp, d.max())      # |rho E| ~ 40, a few roundings of P <-> E
+                    checked += int(sel.sum())
+            assert checked == 96 * 128
+
+
+def test_cfl_dt_describes_role0_after_a_corrector_launch():
+    """the corrector rewrites the cached per-block maxima with those of U^{n+1}; sfh_cfl_dt (documented
+    as 'from role 0') must not return them before sfh_end_step."""
+    p = PROBLEMS["amr-small"]()
+    o, g = both(p)
+    o.advance(1, 1)
+    g.advance(1, 1)                      # the cache now describes role 0 of every level
+    for l in range(p.max_level + 1):
+        want = o.cfl_dt(l)
+        assert abs(g.cfl_dt(l) - want) <= TOLDT * want
+        g.fill_ghosts(l, 0, int(l > 0), 0.0)
+        g.hydro_step(l, 0.5 * want, int(l > 0), 0.0, 0.25)
+        assert abs(g.cfl_dt(l) - want) <= TOLDT * want, "cfl_dt returned the step of U^{n+1}"
+        if l < p.max_level:
+            g.flux_correct(l, 0.5 * want)
+            assert abs(g.cfl_dt(l) - want) <= TOLDT * want
+        g.restrict(l, 0, 2) if l < p.max_level else None
+        assert abs(g.cfl_dt(l) - want) <= TOLDT * want
