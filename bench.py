@@ -2,12 +2,17 @@
 """bench.py — hydro cell-updates/s of the B200 AMR hydro step (BASELINE.json metric).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C2] [--impl ours|reference]
+                    [--per-config C3,C4,C5 | --no-per-config] [--peaks]
 
 A "step" is one coarse step of the whole hot path (CFL reduction, ghost fill incl. prolongation,
 predictor, corrector, flux registers, restriction, reflux; all sub-steps of the finer levels in
 adaptive mode) over one synthetic problem; one cell-update = one predictor+corrector update of one
-cell of one block of any level (the paper's unit).  Default workload: C2 =
-BASELINE.json configs[1], uniform periodic 256^3 in 8^3 blocks (the paper's Table 5 shape).
+cell of one block of any level (the paper's unit).  Headline workload: C2 =
+BASELINE.json configs[1], uniform periodic 256^3 in 8^3 blocks (the paper's Table 5 shape); the same
+JSON line carries a `config.per_config` record for the other full-size configs (C3, C4, C5), each timed
+the same way.  K steps are timed as ceil(K / nsteps) runs of the configured length (BASELINE.json: 10 steps
+for C2-C4, 5 for C5) from the initial state, with an untimed re-initialisation between runs, so that no
+number is taken on a state older than the config describes (`bad_cells` counts non-positive rho / P).
 Prints ONE JSON line (rank 0).  N > 1 runs N independent replicas, one per GPU (DESIGN.md:
 "replicas only"; the path has no multi-GPU exchange in scope).
 """
@@ -24,15 +29,13 @@ sys.path.insert(0, ROOT)
 
 METRIC = "hydro cell-updates/sec (fp64, 1xB200)"
 UNIT = "cell-updates/s"
-CORRECTOR_BYTES_PER_CELL = 120.0   # read U^n, U^{n+1/2}, write U^{n+1}, 5 fp64 each
-PREDICTOR_BYTES_PER_CELL = 80.0    # read U^n, write U^{n+1/2}
-# dram__bytes_read.sum + dram__bytes_write.sum of one corrector launch on C2, from the ncu --set full
-# capture summarised in profiles/ (None until captured)
-CORRECTOR_TRAFFIC_BYTES_C2 = 1.490592e9 + 0.649133e9   # profiles/r1_c2_ncu_final.md
-# fp64 instructions (DFMA + DMUL + DADD + DSETP) per cell-update of the two stage kernels, counted on the ncu
-# source page (profiles/r1_c2_ncu_final.md), and the measured DFMA issue rate of this B200 (profiles/r1_fp64_peak.txt)
-FP64_INST_PER_CELL_UPDATE = 236.0 + 380.0
-FP64_PEAK_INST_PER_S = 17.069e12
+CORRECTOR_BYTES_PER_CELL = 120.0   # read U^n, W^{n+1/2}, write U^{n+1}, 5 fp64 each
+STEP_BYTES_PER_CELL_UPDATE = 200.0  # predictor 80 + corrector 120
+# Figures that come from an ncu capture, not from this run: per-launch DRAM traffic of the corrector and the
+# fp64 instructions the two stage kernels execute per cell-update.  Written by
+#   ncu -i <report> --page raw --csv | python -m paper_2604_21438_b200.ncu_summary --json
+# (the full command is in the file) and tracked under profiles/.
+NCU_FIGURES = os.path.join(ROOT, "profiles", "r2_c2_stage_figures.json")
 
 
 def parse():
@@ -45,7 +48,11 @@ def parse():
     ap.add_argument("--riemann", default="hllc", choices=["hllc", "roe"],
                     help="Riemann solver (PAPER.md:126); the paper's benchmarks and BASELINE.json use HLLC")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--threads", type=int, default=0, help="--impl reference: OpenMP threads of the oracle (0 = all cores)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--per-config", default="C3,C4,C5", help="other full-size configs reported in config.per_config")
+    ap.add_argument("--no-per-config", action="store_true")
+    ap.add_argument("--peaks", action="store_true", help="print the measured fp64 issue rates of this device and exit")
     ap.add_argument("--extras", action="store_true",
                     help="also time the regrid pieces (refinement indicators, state transfer) on this config")
     return ap.parse_args()
@@ -58,6 +65,14 @@ def peaks():
             return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json, copy bandwidth)"
     except Exception:
         return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def ncu_figures():
+    try:
+        with open(NCU_FIGURES) as f:
+            return json.load(f)
+    except Exception:
+        return {}
 
 
 class ClockSampler:
@@ -120,11 +135,12 @@ class ClockSampler:
         except Exception:
             pass
 
-    def stop(self, t0, t1):
+    def stop(self, windows):
+        """windows: [(t0, t1)] wall-clock spans of the timed runs."""
         self.stop_flag = True
         if self.th is not None:
             self.th.join(timeout=2)
-        rows = [r for r in self.rows if t0 <= r[0] <= t1]
+        rows = [r for r in self.rows if any(a <= r[0] <= b for a, b in windows)]
         where = "timed region"
         if not rows:
             rows, where = self.rows, "around the timed region"
@@ -159,6 +175,15 @@ def whole_job_value(cu_per_rank, ms, world):
     return world * cu_per_rank / (ms * 1e-3)
 
 
+def run_lengths(steps, nsteps):
+    """K steps as runs of at most the configured length: [nsteps, nsteps, ..., remainder]."""
+    nsteps = max(1, int(nsteps))
+    out = [nsteps] * (steps // nsteps)
+    if steps % nsteps:
+        out.append(steps % nsteps)
+    return out or [0]
+
+
 def oracle_sample(config, scale_hint, riemann="hllc"):
     """The oracle on a bounded sample of the same workload: the same recipe on a smaller base grid."""
     from oracle import oracle_for
@@ -177,8 +202,10 @@ def run_reference(args):
     """--impl reference: the CPU oracle as it stands, on the host cores (rank 0 only)."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
+    if args.threads > 0:
+        os.environ["OMP_NUM_THREADS"] = str(args.threads)      # before the oracle's library is loaded
     p, o, what = oracle_sample(args.config, args.scale, args.riemann)
-    cores = len(os.sched_getaffinity(0))
+    cores = args.threads if args.threads > 0 else len(os.sched_getaffinity(0))
     for _ in range(args.warmup):
         o.advance(1, p.mode)
     o.nupd[:] = 0
@@ -199,16 +226,126 @@ def run_reference(args):
         "gpu_launches": 0}))
 
 
+def measure(sfh, torch, name, args, dev, world, barrier, steps, warmup, sampler_index=None, e2e=False):
+    """One full-size config on this rank: value pass (device-resident, CUDA events around each run of the configured
+    length), kernel-span pass (same runs with events around every launch), optionally the end-to-end pass."""
+    from sfh_inputs import make_config
+    p = make_config(name, args.scale)
+    census = p.census()
+    g = sfh.Mesh.from_problem(p, device=dev)
+    g.set_riemann(args.riemann)
+    U0 = torch.from_numpy(p.U).pin_memory()
+    Ud = U0.to(dev)
+    state_bytes = int(U0.numel() * 8)
+    runs = run_lengths(steps, p.nsteps) if steps > 0 else [p.nsteps]     # steps 0: one run of the configured length
+
+    def reset():
+        g.set_state(Ud)
+        g.restrict_all(0)
+        g.nupd[:] = 0
+        torch.cuda.synchronize()
+
+    # ---- warm-up
+    reset()
+    for _ in range(max(warmup, 0)):
+        g.advance(1, p.mode)
+    bad_warm = g.status()
+
+    # ---- timed region: the runs, state resident in HBM (no per-launch events here: they cost 1.5 % on C2 and 5 %
+    # on C4, measured; the kernel spans are taken in a second pass of the same runs below)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(sampler_index) if sampler_index is not None else None
+    ms, launches, cu, bad, windows = 0.0, 0, 0.0, 0, []
+    nupd_tot = None
+    for n in runs:
+        reset()
+        l0 = g.launch_count()
+        barrier()
+        t0 = time.time()
+        e0.record()
+        g.advance(n, p.mode)
+        e1.record()
+        barrier()
+        windows.append((t0, time.time()))
+        ms += e0.elapsed_time(e1)
+        launches += g.launch_count() - l0
+        cu += cell_updates(census, g.nupd)
+        nupd_tot = g.nupd.copy() if nupd_tot is None else nupd_tot + g.nupd
+        bad = max(bad, g.status())
+    clocks = sampler.stop(windows) if sampler else None
+    ms = max_over_ranks(ms, world, dev)
+    value = whole_job_value(cu, ms, world)
+
+    # ---- the same runs again with CUDA events around every launch (sfh_profile): per-kernel spans
+    g.profile(True)
+    g.kernel_times()
+    kt = None
+    for n in runs:
+        reset()
+        g.kernel_times()              # drop the spans of the reset (none are timed) before the run
+        g.advance(n, p.mode)
+        torch.cuda.synchronize()
+        k = g.kernel_times()
+        kt = k if kt is None else {c: (kt[c][0] + k[c][0], kt[c][1] + k[c][1]) for c in k}
+    g.profile(False)
+
+    peak, peak_src = peaks()
+    c_ms, c_n = kt["corrector"]
+    corr_bytes = CORRECTOR_BYTES_PER_CELL * cu            # every cell-update passes the corrector once
+    achieved = corr_bytes / (c_ms * 1e-3) / 1e9 if c_ms > 0 else 0.0
+    figs = ncu_figures()
+    is_ref_case = name == "C2" and args.scale == 1 and args.riemann == "hllc"
+    roofline = {"bound": "hbm", "kernel": "stage_kernel<1> (corrector)", "achieved": achieved, "peak": peak,
+                "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
+                "traffic": figs.get("corrector_dram_bytes_per_launch") if is_ref_case else None,
+                "traffic_source": figs.get("source") if is_ref_case else None,
+                "algorithmic_bytes_per_launch": corr_bytes / max(c_n, 1), "launches": c_n,
+                "avg_launch_ms": c_ms / max(c_n, 1),
+                "kernel_ms": {k: round(v[0], 4) for k, v in kt.items()},
+                "kernel_launches": {k: v[1] for k, v in kt.items()},
+                "step_hbm_GBps_at_200B_per_update": STEP_BYTES_PER_CELL_UPDATE * cu / (ms * 1e-3) / 1e9,
+                "step_frac_at_200B_per_update": STEP_BYTES_PER_CELL_UPDATE * cu / (ms * 1e-3) / 1e9 / peak}
+    out = {"p": p, "g": g, "census": census, "workload": p.notes.get("workload", p.name),
+           "mode": "adaptive" if p.mode else "synchronous", "value": value, "ms": ms, "steps": sum(runs), "runs": runs,
+           "launches": launches, "nupd": nupd_tot, "bad": bad, "bad_warm": bad_warm, "clocks": clocks, "kt": kt,
+           "roofline": roofline, "cu": cu, "state_bytes": state_bytes, "reset": reset}
+
+    if e2e:
+        # ---- end to end through sfh_advance_host: pinned host buffers, H2D and D2H of the state every step
+        reset()
+        hin = g.get_state().cpu().pin_memory()    # restriction-consistent initial hierarchy, caller layout
+        hout = torch.empty_like(hin).pin_memory()
+        h0 = hin.clone().pin_memory()
+        g.advance_host(hin, hout, 1, p.mode)      # warm
+        ms_e2e, cu_e2e = 0.0, 0.0
+        for n in runs:
+            hin.copy_(h0)
+            g.nupd[:] = 0
+            a, b = hin, hout
+            barrier()
+            e0.record()
+            for _ in range(n):
+                g.advance_host(a, b, 1, p.mode)
+                a, b = b, a
+            e1.record()
+            barrier()
+            ms_e2e += e0.elapsed_time(e1)
+            cu_e2e += cell_updates(census, g.nupd)
+        ms_e2e = max_over_ranks(ms_e2e, world, dev)
+        out["e2e"] = {"value": whole_job_value(cu_e2e, ms_e2e, world), "unit": UNIT, "h2d_bytes_per_step": state_bytes,
+                      "d2h_bytes_per_step": state_bytes, "ms_per_step": ms_e2e / sum(runs)}
+        del hin, hout, h0
+    return out
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
 
-    import numpy as np
     import torch
     import torch.distributed as dist
     import paper_2604_21438_b200 as sfh
-    from sfh_inputs import make_config
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -220,103 +357,36 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device(dev))
 
-    p = make_config(args.config, args.scale)
-    census = p.census()
-    g = sfh.Mesh.from_problem(p, device=dev)
-    g.set_riemann(args.riemann)
-    U0 = torch.from_numpy(p.U).pin_memory()
-    Ud = U0.to(dev)
-
-    def reset():
-        g.set_state(Ud)
-        g.restrict_all(0)
-        g.nupd[:] = 0
-        torch.cuda.synchronize()
-
     def barrier():
         torch.cuda.synchronize()
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- warm-up
-    reset()
-    for _ in range(max(args.warmup, 0)):
-        g.advance(1, p.mode)
-    bad_warm = g.status()
+    # ---- the second ceiling's denominator, measured live: fp64 issue rate of this device
+    fp64_peak = sfh.measure_fp64_rate(8)
+    fp64_dep = sfh.measure_fp64_rate(1)
+    if args.peaks:
+        if rank == 0:
+            print(json.dumps({"fp64_dfma_per_s": fp64_peak, "fp64_tflops": 2e-12 * fp64_peak,
+                              "fp64_dfma_per_s_one_chain_per_thread": fp64_dep,
+                              "how": "sfh_measure_fp64_rate: 2 CTAs x 1024 threads per SM, 8 (1) independent DFMA chains per "
+                                     "thread, best of 3 launches, CUDA events", "hbm_gbs": peaks()[0], "hbm_source": peaks()[1]}))
+        return
 
-    # ---- timed region: K coarse steps, state resident in HBM (no per-launch events: they cost 1.5 % on C2
-    # and 5 % on C4, measured; the kernel spans are taken in a second pass of the same K steps below)
-    reset()
-    l0 = g.launch_count()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    sampler = ClockSampler(local) if rank == 0 else None
-    t0 = time.time()
-    e0.record()
-    g.advance(args.steps, p.mode)
-    e1.record()
-    barrier()
-    t1 = time.time()
-    clocks = sampler.stop(t0, t1) if sampler else None
-    ms = e0.elapsed_time(e1)
-    launches = g.launch_count() - l0
-    nupd = g.nupd.copy()
-    cu = cell_updates(census, nupd)
-    bad = g.status()
-    ms = max_over_ranks(ms, world, dev)
-    value = whole_job_value(cu, ms, world)
-
-    # ---- the same K steps again with CUDA events around every launch (sfh_profile): per-kernel spans
-    reset()
-    g.profile(True)
-    g.kernel_times()
-    g.advance(args.steps, p.mode)
-    torch.cuda.synchronize()
-    kt = g.kernel_times()
-    g.profile(False)
-
-    # ---- end to end through sfh_advance_host: pinned host buffers, H2D and D2H every step
-    reset()
-    hin = g.get_state().cpu().pin_memory()    # restriction-consistent initial hierarchy, caller layout
-    hout = torch.empty_like(hin).pin_memory()
-    g.advance_host(hin, hout, 1, p.mode)      # warm
-    g.nupd[:] = 0
-    barrier()
-    e0.record()
-    for _ in range(args.steps):
-        g.advance_host(hin, hout, 1, p.mode)
-        hin, hout = hout, hin
-    e1.record()
-    barrier()
-    ms_e2e = e0.elapsed_time(e1)
-    cu_e2e = cell_updates(census, g.nupd)
-    ms_e2e = max_over_ranks(ms_e2e, world, dev)
-    state_bytes = int(U0.numel() * 8)
-
-    # ---- roofline of the dominant kernel (the corrector stage), CUDA events around each launch
-    peak, peak_src = peaks()
-    c_ms, c_n = kt["corrector"]
-    corr_bytes = CORRECTOR_BYTES_PER_CELL * cu            # every cell-update passes the corrector once
-    achieved = corr_bytes / (c_ms * 1e-3) / 1e9 if c_ms > 0 else 0.0
-    roofline = {"bound": "hbm", "kernel": "stage_kernel<1> (corrector)", "achieved": achieved, "peak": peak,
-                "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
-                "traffic": CORRECTOR_TRAFFIC_BYTES_C2 if (args.config == "C2" and args.scale == 1 and
-                                                          args.riemann == "hllc") else None,
-                "algorithmic_bytes_per_launch": corr_bytes / max(c_n, 1), "launches": c_n,
-                "avg_launch_ms": c_ms / max(c_n, 1),
-                "kernel_ms": {k: round(v[0], 4) for k, v in kt.items()},
-                "kernel_launches": {k: v[1] for k, v in kt.items()},
-                "step_hbm_GBps_at_200B_per_update": 200.0 * cu / (ms * 1e-3) / 1e9}
-    # the second ceiling: the stage kernels are bound by fp64 instruction issue, not by HBM
-    stage_ms = kt["predictor"][0] + kt["corrector"][0]
-    f64 = FP64_INST_PER_CELL_UPDATE * cu / (stage_ms * 1e-3) if stage_ms > 0 else 0.0
-    roofline_fp64 = {"bound": "alu", "kernel": "stage_kernel<0> + stage_kernel<1>", "achieved": f64,
-                     "peak": FP64_PEAK_INST_PER_S, "unit": "fp64 inst/s", "frac": f64 / FP64_PEAK_INST_PER_S,
-                     "inst_per_cell_update": FP64_INST_PER_CELL_UPDATE,
-                     "peak_source": "measured DFMA issue rate (profiles/r1_fp64_peak.txt)"}
-    if args.riemann != "hllc":
-        roofline_fp64 = None          # the instruction count was taken with the HLLC kernels
+    m = measure(sfh, torch, args.config, args, dev, world, barrier, args.steps, args.warmup,
+                sampler_index=local if rank == 0 else None, e2e=True)
+    p, g = m["p"], m["g"]
+    figs = ncu_figures()
+    roofline_fp64 = None
+    ipc = figs.get("fp64_thread_inst_per_cell_update")
+    if ipc and args.riemann == "hllc":        # the instruction count was taken with the HLLC kernels
+        stage_ms = m["kt"]["predictor"][0] + m["kt"]["corrector"][0]
+        f64 = ipc * m["cu"] / (stage_ms * 1e-3) if stage_ms > 0 else 0.0
+        roofline_fp64 = {"bound": "alu", "kernel": "stage_kernel<0> + stage_kernel<1>", "achieved": f64,
+                         "peak": fp64_peak, "unit": "fp64 inst/s", "frac": f64 / fp64_peak, "inst_per_cell_update": ipc,
+                         "inst_source": figs.get("source"),
+                         "peak_source": "measured in this run (sfh_measure_fp64_rate, 8 chains per thread)"}
 
     if rank != 0:
         if world > 1:
@@ -327,9 +397,8 @@ def main():
     if args.extras and world == 1:
         # the indicator kernel reads the state once (40 B/cell + halos through L2); the
         # transfer onto an identical mesh copies it (80 B/cell)
-        reset()
-        g.fill_ghosts(-1, 0, 0, 0.0)
-        ncell = 512.0 * sum(census)
+        m["reset"]()
+        ncell = 512.0 * sum(m["census"])
         ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
 
         def timed(fn, reps=5):
@@ -352,6 +421,26 @@ def main():
                                               "note": "includes building and uploading the block map on the host"}}
         del g2
 
+    per_config = {}
+    if world == 1 and not args.no_per_config and args.scale == 1:
+        del m["g"], m["p"], m["reset"], g, p
+        torch.cuda.empty_cache()
+        for name in [c for c in args.per_config.split(",") if c and c != args.config]:
+            t0 = time.time()
+            q = measure(sfh, torch, name, args, dev, world, barrier, 0, args.warmup)
+            per_config[name] = {
+                "workload": q["workload"], "value": q["value"], "ms_per_step": q["ms"] / q["steps"],
+                "steps": q["steps"], "mode": q["mode"],
+                "blocks_per_level": q["census"], "updates_per_level": [int(x) for x in q["nupd"]],
+                "bad_cells": int(q["bad"]), "bad_cells_after_warmup": int(q["bad_warm"]), "gpu_launches": int(q["launches"]),
+                "roofline_frac": q["roofline"]["frac"],
+                "step_hbm_GBps_at_200B_per_update": q["roofline"]["step_hbm_GBps_at_200B_per_update"],
+                "step_frac_at_200B_per_update": q["roofline"]["step_frac_at_200B_per_update"],
+                "kernel_ms": q["roofline"]["kernel_ms"], "kernel_launches": q["roofline"]["kernel_launches"],
+                "wall_s_incl_input_generation": round(time.time() - t0, 1)}
+            del q
+            torch.cuda.empty_cache()
+
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         # the oracle as it stands on this box's host cores, on a bounded sample: whole coarse steps of
@@ -366,22 +455,23 @@ def main():
                "kind": "oracle", "sample": what + ", %d coarse step(s), %.1f s" % (nst, tt)}
 
     out = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "metric": METRIC, "value": m["value"], "unit": UNIT, "n_gpus": world, "steps": m["steps"], "warmup": args.warmup,
+        "ms_per_step": m["ms"] / m["steps"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": p.notes.get("workload", p.name), "config": args.config, "scale": args.scale,
-                   "riemann": args.riemann,
-                   "blocks_per_level": census, "updates_per_level": [int(x) for x in nupd],
-                   "mode": "adaptive" if p.mode else "synchronous",
-                   "l2": "inputs larger than L2 (one state copy %.0f MB vs 126 MB L2)" % (state_bytes / 1e6),
-                   "kernel_spans": "second pass of the same K steps with CUDA events around every launch",
-                   "parallelism": "replicas x%d" % world, "bad_cells": int(bad), "bad_cells_after_warmup": int(bad_warm)},
-        "clocks": clocks,
-        "e2e": {"value": whole_job_value(cu_e2e, ms_e2e, world), "unit": UNIT, "h2d_bytes_per_step": state_bytes,
-                "d2h_bytes_per_step": state_bytes, "ms_per_step": ms_e2e / args.steps},
-        "gpu_launches": int(launches),
-        "roofline": roofline,
+        "config": {"workload": m["workload"], "config": args.config, "scale": args.scale, "riemann": args.riemann,
+                   "blocks_per_level": m["census"], "updates_per_level": [int(x) for x in m["nupd"]],
+                   "mode": m["mode"],
+                   "timed_runs": m["runs"],
+                   "l2": "inputs larger than L2 (one state copy %.0f MB vs 126 MB L2)" % (m["state_bytes"] / 1e6),
+                   "kernel_spans": "second pass of the same runs with CUDA events around every launch",
+                   "parallelism": "replicas x%d" % world, "bad_cells": int(m["bad"]),
+                   "bad_cells_after_warmup": int(m["bad_warm"]), "per_config": per_config},
+        "clocks": m["clocks"],
+        "e2e": m["e2e"],
+        "gpu_launches": int(m["launches"]),
+        "roofline": m["roofline"],
         "roofline_fp64": roofline_fp64,
+        "fp64_rates": {"dfma_per_s_8_chains": fp64_peak, "dfma_per_s_1_chain": fp64_dep},
         "extras": extras,
         "cpu_baseline": cpu,
     }

@@ -220,6 +220,13 @@ int64_t sfh_launch_count(const sfh_mesh* m);
 int sfh_profile(sfh_mesh* m, int enable);
 int sfh_kernel_times(sfh_mesh* m, double* ms, int64_t* count);
 
+/* Measurement support (bench.py's "alu" roofline denominator; SURVEY.md 8(d) "verify by microbenchmark"): the
+ * rate at which this device issues fp64 fused multiply-adds, in thread-level DFMA instructions per second
+ * (x2 = FLOP/s).  `chains` (1, 2, 4 or 8) independent dependent chains per thread, 2 CTAs of 1024 threads per
+ * SM: 8 measures the pipe's peak, 1 the rate a fully dependent instruction stream reaches at full occupancy.
+ * Best of three timed launches (CUDA events on `stream`).  Synchronous.  Needs no mesh. */
+int sfh_measure_fp64_rate(int chains, double* dfma_per_second, void* stream);
+
 const char* sfh_last_error(void);
 
 #ifdef __cplusplus

@@ -79,6 +79,7 @@ def load_library(path=None):
         "sfh_launch_count": (i64, [vp]),
         "sfh_profile": (i32, [vp, i32]),
         "sfh_kernel_times": (i32, [vp, vp, vp]),
+        "sfh_measure_fp64_rate": (i32, [i32, C.POINTER(dbl), vp]),
         "sfh_last_error": (C.c_char_p, []),
     }
     for name, (res, args) in sig.items():
@@ -93,6 +94,16 @@ def load_library(path=None):
 def _stream():
     import torch
     return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def measure_fp64_rate(chains=8):
+    """Thread-level DFMA instructions per second of the current device (sfh_measure_fp64_rate)."""
+    L = load_library()
+    r = C.c_double()
+    rc = L.sfh_measure_fp64_rate(int(chains), C.byref(r), _stream())
+    if rc != 0:
+        raise SfhError(rc, L.sfh_last_error().decode())
+    return r.value
 
 
 class Mesh:

@@ -778,6 +778,38 @@ int sfh_kernel_times(sfh_mesh* m, double* ms, int64_t* count) {
   return SFH_OK;
 }
 
+int sfh_measure_fp64_rate(int chains, double* dfma_per_second, void* stream) {
+  if (!dfma_per_second || (chains != 1 && chains != 2 && chains != 4 && chains != 8))
+    return fail(SFH_EINVAL, "chains must be 1, 2, 4 or 8");
+  int dev = 0, sms = 0;
+  CU(cudaGetDevice(&dev), "cudaGetDevice");
+  CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev), "cudaDeviceGetAttribute");
+  cudaStream_t st = S(stream);
+  double* sink = nullptr;
+  if (cudaMalloc((void**)&sink, 8) != cudaSuccess) return fail(SFH_ENOMEM, "cudaMalloc failed");
+  cudaEvent_t a = nullptr, b = nullptr;
+  cudaError_t e = cudaEventCreate(&a);
+  if (e == cudaSuccess) e = cudaEventCreate(&b);
+  const int ctas = 2 * sms, iters = 4096;
+  double best = 0.0;
+  for (int rep = 0; rep < 4 && e == cudaSuccess; ++rep) {        // the first launch warms up
+    cudaEventRecord(a, st);
+    e = launch_dfma_rate(chains, ctas, iters, sink, st);
+    cudaEventRecord(b, st);
+    if (e == cudaSuccess) e = cudaEventSynchronize(b);
+    float ms = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, a, b);
+    const double rate = double(ctas) * 1024.0 * iters * 16.0 * chains / (double(ms) * 1e-3);
+    if (rep > 0 && rate > best) best = rate;
+  }
+  if (a) cudaEventDestroy(a);
+  if (b) cudaEventDestroy(b);
+  cudaFree(sink);
+  if (e != cudaSuccess) return cuda_fail(e, "dfma_rate_kernel");
+  *dfma_per_second = best;
+  return SFH_OK;
+}
+
 int sfh_status(sfh_mesh* m, int which, int64_t* n_bad_cells, void* stream) {
   int rc = check_bound(m);
   if (rc) return rc;

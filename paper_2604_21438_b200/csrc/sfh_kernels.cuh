@@ -105,5 +105,7 @@ cudaError_t launch_refine_indicator(const double* U, const double* ghost, const 
 cudaError_t launch_transfer(const double* Uc, const double* Us, const double* ghost_s, const int32_t* face_src_s,
                             const int32_t* tsrc, const int32_t* coord_d, double* Ud, int count, cudaStream_t st);
 cudaError_t configure_kernels(int* sm_count);
+// fp64 issue-rate microbenchmark: `ctas` CTAs of 1024 threads, each thread `iters` x 16 x `chains` DFMAs
+cudaError_t launch_dfma_rate(int chains, int ctas, int iters, double* sink, cudaStream_t st);
 
 }  // namespace sfh

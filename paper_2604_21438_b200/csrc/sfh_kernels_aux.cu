@@ -621,4 +621,36 @@ cudaError_t launch_transfer(const double* Uc, const double* Us, const double* gh
   return cudaGetLastError();
 }
 
+// =====================================================================================================
+// fp64 issue-rate microbenchmark (the "alu" roofline denominator of bench.py): every thread runs CHAINS
+// independent DFMA chains; with 1024 threads per SM the fp64 pipe is saturated whatever the dependent
+// latency.  Returns nothing useful in `sink` (it only keeps the compiler from dropping the loop).
+// =====================================================================================================
+template <int CHAINS>
+__global__ void __launch_bounds__(1024) dfma_rate_kernel(int iters, double seed, double* __restrict__ sink) {
+  double x[CHAINS];
+#pragma unroll
+  for (int c = 0; c < CHAINS; ++c) x[c] = seed + 1e-3 * (threadIdx.x + c);
+  const double a = 1.0 - 1e-9, b = 1e-9;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int r = 0; r < 16; ++r)
+#pragma unroll
+      for (int c = 0; c < CHAINS; ++c) x[c] = fma(x[c], a, b);
+  }
+  double t = 0.0;
+#pragma unroll
+  for (int c = 0; c < CHAINS; ++c) t += x[c];
+  if (t == 123.456) sink[0] = t;
+}
+
+// thread-level DFMA instructions per launch = ctas * 1024 * iters * 16 * chains
+cudaError_t launch_dfma_rate(int chains, int ctas, int iters, double* sink, cudaStream_t st) {
+  if (chains == 1) dfma_rate_kernel<1><<<ctas, 1024, 0, st>>>(iters, 0.5, sink);
+  else if (chains == 2) dfma_rate_kernel<2><<<ctas, 1024, 0, st>>>(iters, 0.5, sink);
+  else if (chains == 4) dfma_rate_kernel<4><<<ctas, 1024, 0, st>>>(iters, 0.5, sink);
+  else dfma_rate_kernel<8><<<ctas, 1024, 0, st>>>(iters, 0.5, sink);
+  return cudaGetLastError();
+}
+
 }  // namespace sfh

@@ -4,6 +4,8 @@
 by parity cases the oracle finishes in seconds); scale=1 is the size BASELINE.json names.
 Recipes and the readings they rest on: DESIGN.md "Synthetic inputs".
 """
+import os
+from concurrent.futures import ThreadPoolExecutor
 from dataclasses import dataclass, field
 
 import numpy as np
@@ -22,6 +24,17 @@ CONFIG_NAMES = ("C1", "C2", "C3", "C4", "C5")
 # refinement levels populated.
 RHO_C5 = 8.0
 RHO_C5_SMALL = 1.30
+
+
+def _pmap(fn, items):
+    """fn over items on the host cores (numpy releases the GIL in the gathers and ufuncs that dominate here);
+    results in order, bit-identical to the serial loop."""
+    items = list(items)
+    workers = min(len(items), len(os.sched_getaffinity(0)))
+    if workers <= 1:
+        return [fn(x) for x in items]
+    with ThreadPoolExecutor(workers) as ex:
+        return list(ex.map(fn, items))
 
 
 @dataclass
@@ -96,8 +109,7 @@ def sod(nb=4, gamma=1.4, axis=0, x0=0.5, nsteps=20, slab=False):
 def turbulent_box(name, n, mach, seed, nsteps=10, gamma=5.0 / 3.0, sigma=1.0):
     """C2/C3: periodic uniform n^3, lognormal density, k^-4 velocity at rms Mach `mach`, P = 1/gamma."""
     nb = n // N
-    rho = lognormal_density(n, sigma, seed)
-    v = velocity_field(n, mach, seed + 1)
+    rho, v = _pmap(lambda k: lognormal_density(n, sigma, seed) if k == 0 else velocity_field(n, mach, seed + 1), (0, 1))
     t = uniform_tree((nb, nb, nb), 0)
     level, ijk = t.block_list()
     b = [blockify(a, (nb, nb, nb)) for a in (rho, v[0], v[1], v[2])]
@@ -120,22 +132,26 @@ def amr_sphere(nb=16, nsteps=10, seed=SEED + 20, noise=0.01, max_level=3, mode=1
     def flag(l, idx):
         lev = np.full(len(idx), l, dtype=np.int32)
         out = np.zeros(len(idx), dtype=bool)
-        for s in range(0, len(idx), 4096):
-            X, Y, Z = cell_centres(lev[s:s + 4096], idx[s:s + 4096], nb0)
-            out[s:s + 4096] = (rho_fn(X, Y, Z) > 4.0 ** (l - 3)).reshape(len(X), -1).any(axis=1)
+
+        def chunk(s):
+            X, Y, Z = cell_centres(lev[s:s + 2048], idx[s:s + 2048], nb0)
+            out[s:s + 2048] = (rho_fn(X, Y, Z) > 4.0 ** (l - 3)).reshape(len(X), -1).any(axis=1)
+        _pmap(chunk, range(0, len(idx), 2048))
         return out
 
     t = tree_from_criterion(nb0, max_level, (True, True, True), flag)
     level, ijk = t.block_list()
     U = np.empty((len(level), 5, N, N, N))
-    for s in range(0, len(level), 4096):
-        sl = slice(s, s + 4096)
+
+    def fill(s):
+        sl = slice(s, s + 2048)
         X, Y, Z = cell_centres(level[sl], ijk[sl], nb0)
         I, J, K = global_indices(level[sl], ijk[sl])
         rho = rho_fn(X, Y, Z)
         lv = level[sl][:, None, None, None]
         v = [noise * hash_normal(seed, lv, I, J, K, d) if noise else np.zeros_like(rho) for d in range(3)]
         U[sl] = prim_to_cons(rho, v[0], v[1], v[2], np.full_like(rho, 0.1), gamma)
+    _pmap(fill, range(0, len(level), 2048))
     return Problem("C4", nb0, max_level, ((0, 0),) * 3, (1.0, 1.0, 1.0), gamma, 0.4, mode, nsteps, level, ijk, U,
                    {"workload": "AMR sphere base %d^3 + %d levels" % (nb * N, max_level), "census": t.census()})
 
@@ -147,8 +163,7 @@ def gmc(n=256, nsteps=5, seed=SEED + 30, mach=10.0, sigma=1.5, max_level=4, rho_
     gamma = 1.0001
     nb = n // N
     nb0 = (nb, nb, nb)
-    rho_hat = lognormal_density(n, sigma, seed)
-    v = velocity_field(n, mach, seed + 1)
+    rho_hat, v = _pmap(lambda k: lognormal_density(n, sigma, seed) if k == 0 else velocity_field(n, mach, seed + 1), (0, 1))
     A = np.pi * n * n / (64.0 * rho_c)
 
     def sample(fld, lev, idx):
@@ -158,19 +173,23 @@ def gmc(n=256, nsteps=5, seed=SEED + 30, mach=10.0, sigma=1.5, max_level=4, rho_
     def flag(l, idx):
         lev = np.full(len(idx), l, dtype=np.int32)
         out = np.zeros(len(idx), dtype=bool)
-        for s in range(0, len(idx), 2048):
-            r = sample(rho_hat, lev[s:s + 2048], idx[s:s + 2048])
-            out[s:s + 2048] = (r > rho_c * 4.0 ** l).reshape(len(r), -1).any(axis=1)
+
+        def chunk(s):
+            r = sample(rho_hat, lev[s:s + 1024], idx[s:s + 1024])
+            out[s:s + 1024] = (r > rho_c * 4.0 ** l).reshape(len(r), -1).any(axis=1)
+        _pmap(chunk, range(0, len(idx), 1024))
         return out
 
     t = tree_from_criterion(nb0, max_level, (True, True, True), flag)
     level, ijk = t.block_list()
     U = np.empty((len(level), 5, N, N, N))
-    for s in range(0, len(level), 2048):
-        sl = slice(s, s + 2048)
+
+    def fill(s):
+        sl = slice(s, s + 1024)
         rho = A * sample(rho_hat, level[sl], ijk[sl])
         vv = [sample(c, level[sl], ijk[sl]) for c in v]
         U[sl] = prim_to_cons(rho, vv[0], vv[1], vv[2], rho / gamma, gamma)
+    _pmap(fill, range(0, len(level), 1024))
     return Problem("C5", nb0, max_level, ((0, 0),) * 3, (1.0, 1.0, 1.0), gamma, 0.4, mode, nsteps, level, ijk, U,
                    {"workload": "GMC-like AMR base %d^3 + %d levels" % (n, max_level), "census": t.census(),
                     "amplitude": A, "rho_c": rho_c})
