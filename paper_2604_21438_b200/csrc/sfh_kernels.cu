@@ -33,9 +33,7 @@ namespace sfh {
 
 constexpr int WALK_WARPS = 12, HELP_WARPS = 4;
 constexpr int WALK_THREADS = 32 * WALK_WARPS, HELP_THREADS = 32 * HELP_WARPS;
-constexpr int STAGE_THREADS = WALK_THREADS + HELP_THREADS;   // 512, launched with 128 registers each
-constexpr int WALK_REGS = 136, HELP_REGS = 104;              // corrector, after setmaxnreg
-static_assert(WALK_THREADS * WALK_REGS + HELP_THREADS * HELP_REGS <= 65536, "register file of one SM");
+constexpr int STAGE_THREADS = WALK_THREADS + HELP_THREADS;   // 512 threads of 128 registers: the register file of one SM
 constexpr int CVS = NG * FACE;                // variable stride of every tile (128 cells)
 constexpr int NTILE = 10;
 constexpr int T_XLO = 6, T_XHI = 7, T_YLO = 8, T_YHI = 9;
@@ -472,8 +470,7 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
 
   if (tid < WALK_THREADS) {
     // ------------------------------------------------------------------------------ walkers
-    // corrector: the helpers' update needs few registers; the walkers take what they release
-    if (STAGE == 1) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(WALK_REGS));
+
     const double igm1 = 1.0 / gm1;
     const int D = tid >> 7, f0 = ((tid >> 6) & 1) * 4, pen = tid & 63, a = pen & 7, b = pen >> 3;
     WalkGeom geom;
@@ -512,7 +509,6 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
     }
   } else {
     // ------------------------------------------------------------------------------ helpers
-    if (STAGE == 1) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(HELP_REGS));
     const int hid = tid - WALK_THREADS, hw = hid >> 5;
     const bool lane0 = (tid & 31) == 0;
     const double lam = (STAGE == 0 ? 0.5 : 1.0) * dt / p.h;
@@ -573,8 +569,10 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
       store_block<STAGE == 0>(un, gm1, p.Udst + size_t(blk) * BLK, hid);
       if (it + 2 < n) prepare(it + 2);
       if (STAGE == 1 && p.bmax) {
-        // Off the walkers' critical path (everything they wait for has been handed over): the block's maximum
-        // CFL speed for the next step's dt (reading R16) from the updated cells still in registers.
+        // The block's maximum CFL speed for the next step's dt (reading R16) from the updated cells still in
+        // registers, after everything the walkers wait for has been handed over.  (Measured: these 26 fp64
+        // instructions per cell cost the corrector 10 %: the stage kernels are bound by the instructions the SM
+        // sub-partitions can dispatch, whichever warp they come from.)
         double sp[HC];
 #pragma unroll
         for (int r = 0; r < HC; ++r) sp[r] = cell_speed(un[r], gamma, gm1);   // four independent chains
