@@ -14,7 +14,8 @@ N, G, M, NV = 8, 2, 12, 5
 
 class Config(C.Structure):
     _fields_ = [("nb0", C.c_int32 * 3), ("ncell", C.c_int32), ("nghost", C.c_int32), ("max_level", C.c_int32),
-                ("bc", (C.c_int32 * 2) * 3), ("box_len", C.c_double * 3), ("gamma", C.c_double), ("cfl", C.c_double)]
+                ("bc", (C.c_int32 * 2) * 3), ("box_len", C.c_double * 3), ("gamma", C.c_double), ("cfl", C.c_double),
+                ("nscalar", C.c_int32)]
 
 
 _lib = None
@@ -65,8 +66,9 @@ def lib():
     return _lib
 
 
-def make_config(nb0, max_level, bc, box_len, gamma, cfl):
+def make_config(nb0, max_level, bc, box_len, gamma, cfl, nscalar=0):
     cfg = Config()
+    cfg.nscalar = int(nscalar)
     for d in range(3):
         cfg.nb0[d] = int(nb0[d])
         cfg.box_len[d] = float(box_len[d])
@@ -96,18 +98,19 @@ def roe(WL, WR, d, gamma):
 class OracleMesh:
     """Oracle mesh + three ghosted state copies (0: U^n, 1: U^{n+1/2}, 2: U^{n+1})."""
 
-    def __init__(self, nb0, max_level, bc, box_len, gamma, cfl, level, ijk):
+    def __init__(self, nb0, max_level, bc, box_len, gamma, cfl, level, ijk, nscalar=0):
         self.L = lib()
         self.level = np.ascontiguousarray(level, dtype=np.int32)
         self.ijk = np.ascontiguousarray(ijk, dtype=np.int32).reshape(-1, 3)
         self.nb = len(self.level)
-        self.cfg = make_config(nb0, max_level, bc, box_len, gamma, cfl)
+        self.nv = NV + int(nscalar)          # 5 hydro variables + passive scalars rho*s
+        self.cfg = make_config(nb0, max_level, bc, box_len, gamma, cfl, nscalar)
         self.h = C.c_void_p()
         rc = self.L.orc_create_mesh(C.byref(self.cfg), self.nb, self.level.ctypes.data, self.ijk.ctypes.data,
                                     C.byref(self.h))
         if rc != 0:
             raise ValueError("orc_create_mesh failed: %d" % rc)
-        self.U = [np.zeros((self.nb, NV, M, M, M)) for _ in range(3)]
+        self.U = [np.zeros((self.nb, self.nv, M, M, M)) for _ in range(3)]
         self.L.orc_bind(self.h, *[u.ctypes.data for u in self.U])
         self.max_level = int(max_level)
         self.t = C.c_double(0.0)
@@ -191,7 +194,7 @@ class OracleMesh:
         return out
 
     def get(self, level, I, J, K, which=0):
-        out = np.zeros(NV)
+        out = np.zeros(self.nv)
         rc = self.L.orc_get(self.h, level, I, J, K, which, out.ctypes.data)
         if rc != 0:
             raise RuntimeError("orc_get: unresolved cell")
@@ -201,6 +204,7 @@ class OracleMesh:
 def oracle_for(p, U=None):
     """OracleMesh of a problem description `p` (fields nb0, max_level, bc, box_len, gamma, cfl, level, ijk, U:
     sfh_inputs.Problem), holding U (default p.U) as its copy 0."""
-    m = OracleMesh(p.nb0, p.max_level, p.bc, p.box_len, p.gamma, p.cfl, p.level, p.ijk)
-    m.set_state(p.U if U is None else U)
+    U = p.U if U is None else U
+    m = OracleMesh(p.nb0, p.max_level, p.bc, p.box_len, p.gamma, p.cfl, p.level, p.ijk, nscalar=U.shape[1] - NV)
+    m.set_state(U)
     return m

@@ -26,6 +26,10 @@
 // reconstruction (R11), minmod limiter (R12), CFL speed definition (R16), the entropy-fix width of
 // the Roe solver (R30; the Roe flux itself is pinned by tests/test_oracle_roe_pins.py).
 //
+// Passive scalars (eq. 12-13; reading R32): up to 8 extra conserved densities
+// rho*s per cell, carried by the Riemann solver's mass flux, reconstructed, prolonged, restricted and refluxed like
+// the hydro variables; pins in tests/test_oracle_scalar_pins.py.
+//
 // Passages followed: PAPER.md:39-44,58 (Euler equations, E of eq. 8); :96 (blocks, levels);
 // :108-120 (time marching, eq. 14-15); :126 (MUSCL, predictor-corrector, HLLC);
 // :128 (ghost interpolation in space and time, reflux); :142-148 (three stored time levels,
@@ -45,8 +49,9 @@ constexpr int N = 8;    // cells per block edge
 constexpr int G = 2;    // ghost layers                    BASELINE.json configs
 constexpr int M = N + 2 * G;
 constexpr int NV = 5;   // rho, rho vx, rho vy, rho vz, rho E
+constexpr int NSMAX = 8;          // passive scalars rho*s advected with the gas (eq. 12-13; reading R32)
+constexpr int NVMAX = NV + NSMAX; // a mesh carries nv = NV + nscalar conserved variables per cell
 constexpr int M3 = M * M * M;
-constexpr int BLK = NV * M3;  // doubles per ghosted block
 
 struct Config {            // binary layout mirrored by the ctypes Structure in oracle/binding.py
   int32_t nb0[3];
@@ -55,6 +60,7 @@ struct Config {            // binary layout mirrored by the ctypes Structure in 
   int32_t bc[3][2];        // 0 periodic, 1 outflow (zero gradient)
   double box_len[3];
   double gamma, cfl;
+  int32_t nscalar;         // passive scalars carried besides the 5 hydro variables (0..NSMAX)
 };
 
 struct Src {               // how a block cell is read
@@ -67,6 +73,8 @@ struct Mesh {
   Config cfg;
   int64_t nb = 0;
   int nlev = 0;
+  int nv = NV;             // conserved variables per cell: NV + cfg.nscalar
+  int64_t blk = NV * M3;   // doubles per ghosted block: nv * 12^3
   std::vector<int> lev, bx, by, bz;
   std::vector<char> leaf;
   std::unordered_map<uint64_t, int> map;
@@ -104,9 +112,9 @@ inline double time_interp(double U0, double Uh, double U1, double tau) {
   return (U1 - U1st) * (tau * tau) + ((1.0 - tau) * U0 + tau * U1st);   // eq. (16), tau=(t-t^n)/(t^{n+1}-t^n)
 }
 
-inline void cell_value(const Mesh& m, int b, int i, int j, int k, const Src& s, double out[NV]) {
-  for (int v = 0; v < NV; ++v) {
-    const int64_t o = int64_t(b) * BLK + gidx(v, i, j, k);
+inline void cell_value(const Mesh& m, int b, int i, int j, int k, const Src& s, double out[NVMAX]) {
+  for (int v = 0; v < m.nv; ++v) {
+    const int64_t o = int64_t(b) * m.blk + gidx(v, i, j, k);
     if (s.mode == 0) out[v] = m.U[s.which][o];
     else out[v] = time_interp(m.U[0][o], m.U[1][o], m.U[2][o], s.tau);
   }
@@ -133,7 +141,7 @@ inline bool apply_bc(const Mesh& m, int l, int idx[3]) {
 
 // Accessor: value of global cell (I,J,K) of level l (readings R1, R3).  srcs[lv] says how
 // level lv's stored data are read.  Returns false on a nesting violation.
-bool get(const Mesh& m, int l, int I, int J, int K, const Src* srcs, double out[NV]) {
+bool get(const Mesh& m, int l, int I, int J, int K, const Src* srcs, double out[NVMAX]) {
   int idx[3] = {I, J, K};
   apply_bc(m, l, idx);
   const int b = find(m, l, idx[0] >> 3, idx[1] >> 3, idx[2] >> 3);
@@ -146,16 +154,16 @@ bool get(const Mesh& m, int l, int I, int J, int K, const Src* srcs, double out[
   // slope-limited linear prolongation from level l-1 (reading R3; PAPER.md:128 defers the
   // formula to a paper that is not available)
   const int c[3] = {idx[0] >> 1, idx[1] >> 1, idx[2] >> 1};
-  double Q[NV], Qp[NV], Qm[NV];
+  double Q[NVMAX], Qp[NVMAX], Qm[NVMAX];
   if (!get(m, l - 1, c[0], c[1], c[2], srcs, Q)) return false;
-  for (int v = 0; v < NV; ++v) out[v] = Q[v];
+  for (int v = 0; v < m.nv; ++v) out[v] = Q[v];
   for (int d = 0; d < 3; ++d) {
     int cp[3] = {c[0], c[1], c[2]}, cm[3] = {c[0], c[1], c[2]};
     cp[d] += 1; cm[d] -= 1;
     if (!get(m, l - 1, cp[0], cp[1], cp[2], srcs, Qp)) return false;
     if (!get(m, l - 1, cm[0], cm[1], cm[2], srcs, Qm)) return false;
     const double sigma = (idx[d] & 1) ? 1.0 : -1.0;
-    for (int v = 0; v < NV; ++v) {
+    for (int v = 0; v < m.nv; ++v) {
       const double slope = minmod(Qp[v] - Q[v], Q[v] - Qm[v]);
       out[v] = out[v] + sigma * 0.25 * slope;
     }
@@ -177,14 +185,14 @@ int fill_ghosts_level(Mesh& m, int l, int which, int interp, double tau) {
 #pragma omp parallel for schedule(dynamic, 8) reduction(+ : bad)
   for (int64_t t = 0; t < (int64_t)blocks.size(); ++t) {
     const int b = blocks[t];
-    double* dst = m.U[which] + int64_t(b) * BLK;
-    double val[NV];
+    double* dst = m.U[which] + int64_t(b) * m.blk;
+    double val[NVMAX];
     for (int k = -G; k < N + G; ++k)
       for (int j = -G; j < N + G; ++j)
         for (int i = -G; i < N + G; ++i) {
           if (i >= 0 && i < N && j >= 0 && j < N && k >= 0 && k < N) continue;
           if (!get(m, l, m.bx[b] * N + i, m.by[b] * N + j, m.bz[b] * N + k, srcs.data(), val)) { bad++; continue; }
-          for (int v = 0; v < NV; ++v) dst[gidx(v, i, j, k)] = val[v];
+          for (int v = 0; v < m.nv; ++v) dst[gidx(v, i, j, k)] = val[v];
         }
   }
   if (bad) { snprintf(m.err, sizeof m.err, "fill_ghosts: %d cells could not be resolved (nesting)", bad); return -2; }
@@ -298,59 +306,77 @@ inline void cell_of(int d, int c, int a, int b, int& i, int& j, int& k) {
   else { i = a; j = b; k = c; }
 }
 
+// ------------------------------------------------------------------ passive scalars (eq. 12-13; reading R32)
+// A scalar is carried as the conserved density q = rho * s (y_i n_H of eq. 12, rho C_d T_d of eq. 13; source terms are
+// not part of this path).  Its primitive is s = q / rho; its interface flux is the Riemann solver's mass flux times
+// the interface value of s on the side the mass comes from:  F_q = F_rho * (F_rho >= 0 ? s_L : s_R).
+inline void scalar_fluxes(int nv, const double WL[NVMAX], const double WR[NVMAX], double F[NVMAX]) {
+  for (int v = NV; v < nv; ++v) F[v] = F[0] * (F[0] >= 0.0 ? WL[v] : WR[v]);
+}
+inline void all_prims(const Mesh& m, const double* U, int i, int j, int k, double w[NVMAX]) {
+  double u[NV];
+  for (int v = 0; v < NV; ++v) u[v] = U[gidx(v, i, j, k)];
+  cons_to_prim(u, m.cfg.gamma, w);
+  for (int v = NV; v < m.nv; ++v) w[v] = U[gidx(v, i, j, k)] / u[0];
+}
+
+// U_out = U^n - lam * ((dFx + dFy) + dFz) on the interior cells, all nv variables; F = [3][nv][9][8][8]
+void flux_update(const Mesh& m, const double* Un, double* Uout, const std::vector<double>& F, double lam) {
+  const int fs = m.nv * 9 * N * N;
+  const double* Fx = F.data(); const double* Fy = Fx + fs; const double* Fz = Fy + fs;
+  for (int k = 0; k < N; ++k) for (int j = 0; j < N; ++j) for (int i = 0; i < N; ++i)
+    for (int v = 0; v < m.nv; ++v) {
+      const double sum = ((Fx[fidx(v, i + 1, j, k)] - Fx[fidx(v, i, j, k)]) +
+                          (Fy[fidx(v, j + 1, i, k)] - Fy[fidx(v, j, i, k)])) +
+                         (Fz[fidx(v, k + 1, i, j)] - Fz[fidx(v, k, i, j)]);
+      Uout[gidx(v, i, j, k)] = Un[gidx(v, i, j, k)] - lam * sum;
+    }
+}
+
 // ------------------------------------------------------------------ predictor (a4; reading R8)
 void predictor_block(Mesh& m, int b, double dt) {
-  const double gamma = m.cfg.gamma;
+  const int nv = m.nv, fs = nv * 9 * N * N;
   const double h = h_of(m, m.lev[b]);
-  const double* Un = m.U[0] + int64_t(b) * BLK;
-  double* Uh = m.U[1] + int64_t(b) * BLK;
-  std::vector<double> W(BLK), F(3 * NV * 9 * N * N);
+  const double* Un = m.U[0] + int64_t(b) * m.blk;
+  double* Uh = m.U[1] + int64_t(b) * m.blk;
+  std::vector<double> W(m.blk), F(3 * fs);
   for (int k = -1; k <= N; ++k) for (int j = -1; j <= N; ++j) for (int i = -1; i <= N; ++i) {
     // only face-adjacent ghost cells are read below, but converting the whole 10^3 box is harmless
-    double u[NV], w[NV];
-    for (int v = 0; v < NV; ++v) u[v] = Un[gidx(v, i, j, k)];
-    cons_to_prim(u, gamma, w);
-    for (int v = 0; v < NV; ++v) W[gidx(v, i, j, k)] = w[v];
+    double w[NVMAX];
+    all_prims(m, Un, i, j, k, w);
+    for (int v = 0; v < nv; ++v) W[gidx(v, i, j, k)] = w[v];
   }
   for (int d = 0; d < 3; ++d)
     for (int tb = 0; tb < N; ++tb) for (int ta = 0; ta < N; ++ta) for (int f = 0; f <= N; ++f) {
       int i0, j0, k0, i1, j1, k1;
       cell_of(d, f - 1, ta, tb, i0, j0, k0);
       cell_of(d, f, ta, tb, i1, j1, k1);
-      double WL[NV], WR[NV], Ff[NV];
-      for (int v = 0; v < NV; ++v) { WL[v] = W[gidx(v, i0, j0, k0)]; WR[v] = W[gidx(v, i1, j1, k1)]; }
+      double WL[NVMAX], WR[NVMAX], Ff[NVMAX];
+      for (int v = 0; v < nv; ++v) { WL[v] = W[gidx(v, i0, j0, k0)]; WR[v] = W[gidx(v, i1, j1, k1)]; }
       riemann_flux(m, WL, WR, d, Ff);
-      for (int v = 0; v < NV; ++v) F[d * NV * 9 * N * N + fidx(v, f, ta, tb)] = Ff[v];
+      scalar_fluxes(nv, WL, WR, Ff);
+      for (int v = 0; v < nv; ++v) F[d * fs + fidx(v, f, ta, tb)] = Ff[v];
     }
-  const double lam = 0.5 * dt / h;
-  const double* Fx = F.data(); const double* Fy = Fx + NV * 9 * N * N; const double* Fz = Fy + NV * 9 * N * N;
-  for (int k = 0; k < N; ++k) for (int j = 0; j < N; ++j) for (int i = 0; i < N; ++i)
-    for (int v = 0; v < NV; ++v) {
-      const double sum = ((Fx[fidx(v, i + 1, j, k)] - Fx[fidx(v, i, j, k)]) +
-                          (Fy[fidx(v, j + 1, i, k)] - Fy[fidx(v, j, i, k)])) +
-                         (Fz[fidx(v, k + 1, i, j)] - Fz[fidx(v, k, i, j)]);
-      Uh[gidx(v, i, j, k)] = Un[gidx(v, i, j, k)] - lam * sum;
-    }
+  flux_update(m, Un, Uh, F, 0.5 * dt / h);
 }
 
 // ------------------------------------------------------------------ corrector (a6, a7; readings R11-R14)
 void corrector_block(Mesh& m, int b, double dt) {
-  const double gamma = m.cfg.gamma;
+  const int nv = m.nv, fs = nv * 9 * N * N;
   const double h = h_of(m, m.lev[b]);
-  const double* Un = m.U[0] + int64_t(b) * BLK;
-  const double* Uh = m.U[1] + int64_t(b) * BLK;
-  double* Unew = m.U[2] + int64_t(b) * BLK;
-  std::vector<double> W(BLK), F(3 * NV * 9 * N * N);
+  const double* Un = m.U[0] + int64_t(b) * m.blk;
+  const double* Uh = m.U[1] + int64_t(b) * m.blk;
+  double* Unew = m.U[2] + int64_t(b) * m.blk;
+  std::vector<double> W(m.blk), F(3 * fs);
   for (int k = -G; k < N + G; ++k) for (int j = -G; j < N + G; ++j) for (int i = -G; i < N + G; ++i) {
-    double u[NV], w[NV];
-    for (int v = 0; v < NV; ++v) u[v] = Uh[gidx(v, i, j, k)];
-    cons_to_prim(u, gamma, w);
-    for (int v = 0; v < NV; ++v) W[gidx(v, i, j, k)] = w[v];
+    double w[NVMAX];
+    all_prims(m, Uh, i, j, k, w);
+    for (int v = 0; v < nv; ++v) W[gidx(v, i, j, k)] = w[v];
   }
   for (int d = 0; d < 3; ++d)
     for (int tb = 0; tb < N; ++tb) for (int ta = 0; ta < N; ++ta) for (int f = 0; f <= N; ++f) {
-      double WL[NV], WR[NV], Ff[NV];
-      for (int v = 0; v < NV; ++v) {
+      double WL[NVMAX], WR[NVMAX], Ff[NVMAX];
+      for (int v = 0; v < nv; ++v) {
         double w[4];  // cells f-2, f-1, f, f+1 along d
         for (int s = 0; s < 4; ++s) { int i, j, k; cell_of(d, f - 2 + s, ta, tb, i, j, k); w[s] = W[gidx(v, i, j, k)]; }
         const double dl = minmod(w[2] - w[1], w[1] - w[0]);   // slope of the left cell  (f-1)
@@ -359,28 +385,21 @@ void corrector_block(Mesh& m, int b, double dt) {
         WR[v] = w[2] - 0.5 * dr;
       }
       riemann_flux(m, WL, WR, d, Ff);
-      for (int v = 0; v < NV; ++v) F[d * NV * 9 * N * N + fidx(v, f, ta, tb)] = Ff[v];
+      scalar_fluxes(nv, WL, WR, Ff);
+      for (int v = 0; v < nv; ++v) F[d * fs + fidx(v, f, ta, tb)] = Ff[v];
     }
-  const double lam = dt / h;
-  const double* Fx = F.data(); const double* Fy = Fx + NV * 9 * N * N; const double* Fz = Fy + NV * 9 * N * N;
-  for (int k = 0; k < N; ++k) for (int j = 0; j < N; ++j) for (int i = 0; i < N; ++i)
-    for (int v = 0; v < NV; ++v) {
-      const double sum = ((Fx[fidx(v, i + 1, j, k)] - Fx[fidx(v, i, j, k)]) +
-                          (Fy[fidx(v, j + 1, i, k)] - Fy[fidx(v, j, i, k)])) +
-                         (Fz[fidx(v, k + 1, i, j)] - Fz[fidx(v, k, i, j)]);
-      Unew[gidx(v, i, j, k)] = Un[gidx(v, i, j, k)] - lam * sum;
-    }
+  flux_update(m, Un, Unew, F, dt / h);
   // flux bookkeeping at coarse-fine faces (reading R14): fine side accumulates dt*F, the
   // coarse leaf stores its own flux.
   for (int d = 0; d < 3; ++d) for (int side = 0; side < 2; ++side) {
     const int face = 2 * d + side;
-    const double* Fd = F.data() + d * NV * 9 * N * N;
+    const double* Fd = F.data() + d * fs;
     const int f = side ? N : 0;
-    const int rs = m.rslot[int64_t(b) * 6 + face], fs = m.fslot[int64_t(b) * 6 + face];
-    for (int v = 0; v < NV; ++v) for (int tb = 0; tb < N; ++tb) for (int ta = 0; ta < N; ++ta) {
+    const int rs = m.rslot[int64_t(b) * 6 + face], fsl = m.fslot[int64_t(b) * 6 + face];
+    for (int v = 0; v < nv; ++v) for (int tb = 0; tb < N; ++tb) for (int ta = 0; ta < N; ++ta) {
       const double val = Fd[fidx(v, f, ta, tb)];
-      if (rs >= 0) m.R[(int64_t(rs) * NV + v) * 64 + tb * N + ta] += dt * val;
-      if (fs >= 0) m.FH[(int64_t(fs) * NV + v) * 64 + tb * N + ta] = val;
+      if (rs >= 0) m.R[(int64_t(rs) * nv + v) * 64 + tb * N + ta] += dt * val;
+      if (fsl >= 0) m.FH[(int64_t(fsl) * nv + v) * 64 + tb * N + ta] = val;
     }
   }
 }
@@ -393,15 +412,15 @@ void restrict_level(Mesh& m, int lc, int src_copy, int dst_copy) {   // level lc
   for (int64_t t = 0; t < (int64_t)blocks.size(); ++t) {
     const int b = blocks[t];
     if (m.leaf[b]) continue;
-    double* dst = m.U[dst_copy] + int64_t(b) * BLK;
+    double* dst = m.U[dst_copy] + int64_t(b) * m.blk;
     for (int k = 0; k < N; ++k) for (int j = 0; j < N; ++j) for (int i = 0; i < N; ++i) {
       const int I = 2 * (m.bx[b] * N + i), J = 2 * (m.by[b] * N + j), K = 2 * (m.bz[b] * N + k);
-      for (int v = 0; v < NV; ++v) {
+      for (int v = 0; v < m.nv; ++v) {
         double sum = 0.0;
         for (int c = 0; c < 8; ++c) {   // fixed child-cell order c = cx + 2 cy + 4 cz
           const int fi = I + (c & 1), fj = J + ((c >> 1) & 1), fk = K + ((c >> 2) & 1);
           const int fb = find(m, lc + 1, fi >> 3, fj >> 3, fk >> 3);
-          sum += m.U[src_copy][int64_t(fb) * BLK + gidx(v, fi & 7, fj & 7, fk & 7)];
+          sum += m.U[src_copy][int64_t(fb) * m.blk + gidx(v, fi & 7, fj & 7, fk & 7)];
         }
         dst[gidx(v, i, j, k)] = 0.125 * sum;
       }
@@ -419,7 +438,7 @@ void reflux_level(Mesh& m, int lc, int copy, double dt_coarse) {
 #pragma omp parallel for schedule(dynamic, 8)
   for (int64_t t = 0; t < (int64_t)blocks.size(); ++t) {
     const int b = blocks[t];
-    double* U = m.U[copy] + int64_t(b) * BLK;
+    double* U = m.U[copy] + int64_t(b) * m.blk;
     for (int face = 0; face < 6; ++face) {   // fixed order x-, x+, y-, y+, z-, z+
       const int fs = m.fslot[int64_t(b) * 6 + face];
       if (fs < 0) continue;
@@ -429,7 +448,7 @@ void reflux_level(Mesh& m, int lc, int copy, double dt_coarse) {
         int i, j, k;
         cell_of(d, side ? N - 1 : 0, ta, tb, i, j, k);
         const int gc[3] = {m.bx[b] * N + i, m.by[b] * N + j, m.bz[b] * N + k};
-        for (int v = 0; v < NV; ++v) {
+        for (int v = 0; v < m.nv; ++v) {
           double sumR = 0.0;
           for (int q = 0; q < 4; ++q) {   // 2x2 fine faces, first tangential index fastest
             int ff[3];
@@ -446,9 +465,9 @@ void reflux_level(Mesh& m, int lc, int copy, double dt_coarse) {
             if (d == 0) { fa = ff[1] & 7; fbb = ff[2] & 7; }
             else if (d == 1) { fa = ff[0] & 7; fbb = ff[2] & 7; }
             else { fa = ff[0] & 7; fbb = ff[1] & 7; }
-            sumR += m.R[(int64_t(rs) * NV + v) * 64 + fbb * N + fa];
+            sumR += m.R[(int64_t(rs) * m.nv + v) * 64 + fbb * N + fa];
           }
-          const double FHv = m.FH[(int64_t(fs) * NV + v) * 64 + tb * N + ta];
+          const double FHv = m.FH[(int64_t(fs) * m.nv + v) * 64 + tb * N + ta];
           U[gidx(v, i, j, k)] = U[gidx(v, i, j, k)] - (s / h) * (0.25 * sumR - dt_coarse * FHv);
         }
       }
@@ -462,7 +481,7 @@ double max_speed_level(const Mesh& m, int l, int copy) {
   double smax = 0.0;
 #pragma omp parallel for schedule(static) reduction(max : smax)
   for (int64_t t = 0; t < (int64_t)blocks.size(); ++t) {
-    const double* U = m.U[copy] + int64_t(blocks[t]) * BLK;
+    const double* U = m.U[copy] + int64_t(blocks[t]) * m.blk;
     for (int k = 0; k < N; ++k) for (int j = 0; j < N; ++j) for (int i = 0; i < N; ++i) {
       double u[NV], w[NV];
       for (int v = 0; v < NV; ++v) u[v] = U[gidx(v, i, j, k)];
@@ -483,16 +502,16 @@ double cfl_dt_level(const Mesh& m, int l, int copy) {
 void zero_registers(Mesh& m, int lc) {   // registers of the (lc, lc+1) interface
   for (int b : m.of_level[lc + 1]) for (int f = 0; f < 6; ++f) {
     const int rs = m.rslot[int64_t(b) * 6 + f];
-    if (rs >= 0) std::fill_n(&m.R[int64_t(rs) * NV * 64], NV * 64, 0.0);
+    if (rs >= 0) std::fill_n(&m.R[int64_t(rs) * m.nv * 64], m.nv * 64, 0.0);
   }
   for (int b : m.of_level[lc]) for (int f = 0; f < 6; ++f) {
     const int fs = m.fslot[int64_t(b) * 6 + f];
-    if (fs >= 0) std::fill_n(&m.FH[int64_t(fs) * NV * 64], NV * 64, 0.0);
+    if (fs >= 0) std::fill_n(&m.FH[int64_t(fs) * m.nv * 64], m.nv * 64, 0.0);
   }
 }
 
 void copy_level(Mesh& m, int l, int src, int dst) {
-  for (int b : m.of_level[l]) std::memcpy(m.U[dst] + int64_t(b) * BLK, m.U[src] + int64_t(b) * BLK, sizeof(double) * BLK);
+  for (int b : m.of_level[l]) std::memcpy(m.U[dst] + int64_t(b) * m.blk, m.U[src] + int64_t(b) * m.blk, sizeof(double) * m.blk);
 }
 
 void for_blocks(Mesh& m, int l, double dt, void (*fn)(Mesh&, int, double)) {
@@ -548,9 +567,11 @@ int advance_adaptive(Mesh& m, int l, double dt, double tau, double dt_parent, in
 extern "C" {
 
 int orc_create_mesh(const Config* cfg, int64_t nblocks, const int32_t* level, const int32_t* ijk, Mesh** out) {
-  if (!cfg || !out || cfg->ncell != N || cfg->nghost != G) return -1;
+  if (!cfg || !out || cfg->ncell != N || cfg->nghost != G || cfg->nscalar < 0 || cfg->nscalar > NSMAX) return -1;
   Mesh* m = new Mesh;
   m->cfg = *cfg;
+  m->nv = NV + cfg->nscalar;
+  m->blk = int64_t(m->nv) * M3;
   m->nb = nblocks;
   m->nlev = cfg->max_level + 1;
   m->lev.resize(nblocks); m->bx.resize(nblocks); m->by.resize(nblocks); m->bz.resize(nblocks);
@@ -579,15 +600,15 @@ int orc_create_mesh(const Config* cfg, int64_t nblocks, const int32_t* level, co
     if (nbk < 0) { if (l > 0) m->rslot[b * 6 + face] = nr++; }
     else if (m->leaf[b] && !m->leaf[nbk]) m->fslot[b * 6 + face] = nf++;
   }
-  m->R.assign(int64_t(nr) * NV * 64, 0.0);
-  m->FH.assign(int64_t(nf) * NV * 64, 0.0);
+  m->R.assign(int64_t(nr) * m->nv * 64, 0.0);
+  m->FH.assign(int64_t(nf) * m->nv * 64, 0.0);
   *out = m;
   return 0;
 }
 
 void orc_destroy_mesh(Mesh* m) { delete m; }
 const char* orc_last_error(Mesh* m) { return m->err; }
-int64_t orc_state_doubles(const Mesh* m) { return m->nb * BLK; }
+int64_t orc_state_doubles(const Mesh* m) { return m->nb * m->blk; }
 
 int orc_bind(Mesh* m, double* U0, double* U1, double* U2) { m->U[0] = U0; m->U[1] = U1; m->U[2] = U2; return 0; }
 void orc_set_reflux(Mesh* m, int on) { m->reflux_on = on; }
@@ -636,7 +657,10 @@ void orc_roe(const double* WL, const double* WR, int d, double gamma, double* F)
 double orc_minmod(double a, double b) { return minmod(a, b); }
 int orc_get(Mesh* m, int level, int I, int J, int K, int which, double* out) {   // sync-mode accessor
   std::vector<Src> srcs(m->nlev, Src{0, which, 0.0});
-  return get(*m, level, I, J, K, srcs.data(), out) ? 0 : -2;
+  double val[NVMAX];
+  if (!get(*m, level, I, J, K, srcs.data(), val)) return -2;
+  for (int v = 0; v < m->nv; ++v) out[v] = val[v];      // out: nv = 5 + nscalar doubles
+  return 0;
 }
 
 // mode 0: synchronous, dt_fixed>0 overrides the CFL step; mode 1: adaptive
@@ -661,7 +685,7 @@ int orc_advance(Mesh* m, int nsteps, int mode, double dt_fixed, double* t, int64
 int64_t orc_status(Mesh* m, int copy) {   // cells with rho<=0 or P<=0 (or NaN), interior, all blocks
   int64_t bad = 0;
   for (int64_t b = 0; b < m->nb; ++b) {
-    const double* U = m->U[copy] + b * BLK;
+    const double* U = m->U[copy] + b * m->blk;
     for (int k = 0; k < N; ++k) for (int j = 0; j < N; ++j) for (int i = 0; i < N; ++i) {
       double u[NV], w[NV];
       for (int v = 0; v < NV; ++v) u[v] = U[gidx(v, i, j, k)];
@@ -685,7 +709,7 @@ int orc_refine_indicator(Mesh* m, int which, int criterion, double G, double* ou
   const double gamma = m->cfg.gamma;
   const double pi = 3.14159265358979323846;
   for (int64_t b = 0; b < m->nb; ++b) {
-    const double* U = m->U[which] + b * BLK;
+    const double* U = m->U[which] + b * m->blk;
     const double h = h_of(*m, m->lev[b]);
     auto prim = [&](int i, int j, int k, double& rho, double& P) {
       double u[NV], w[NV];
@@ -730,16 +754,17 @@ int orc_transfer_state(const Mesh* src, int src_which, Mesh* dst, int dst_which)
   for (int d = 0; d < 3; ++d)
     if (src->cfg.nb0[d] != dst->cfg.nb0[d] || src->cfg.bc[d][0] != dst->cfg.bc[d][0] ||
         src->cfg.bc[d][1] != dst->cfg.bc[d][1]) return -1;
+  if (src->nv != dst->nv) return -1;
   std::vector<Src> srcs(std::max(src->nlev, dst->nlev), Src{0, src_which, 0.0});
   int bad = 0;
 #pragma omp parallel for schedule(dynamic, 8) reduction(+ : bad)
   for (int64_t b = 0; b < dst->nb; ++b) {
     const int l = dst->lev[b];
-    double* out = dst->U[dst_which] + b * BLK;
-    double val[NV];
+    double* out = dst->U[dst_which] + b * dst->blk;
+    double val[NVMAX];
     for (int k = 0; k < N; ++k) for (int j = 0; j < N; ++j) for (int i = 0; i < N; ++i) {
       if (!get(*src, l, dst->bx[b] * N + i, dst->by[b] * N + j, dst->bz[b] * N + k, srcs.data(), val)) { bad++; continue; }
-      for (int v = 0; v < NV; ++v) out[gidx(v, i, j, k)] = val[v];
+      for (int v = 0; v < dst->nv; ++v) out[gidx(v, i, j, k)] = val[v];
     }
   }
   if (bad) { snprintf(dst->err, sizeof dst->err, "transfer_state: %d cells could not be resolved", bad); return -2; }

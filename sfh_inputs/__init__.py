@@ -10,4 +10,4 @@ from .mesh import Tree, uniform_tree, tree_from_criterion, blockify, unblockify 
 from .fields import (gaussian_random_field, lognormal_density, velocity_field, hash_normal,  # noqa: F401
                      prim_to_cons)
 from .configs import make_config, CONFIG_NAMES, Problem  # noqa: F401
-from .small import small_amr_tree, smooth_fields, problem_from_tree  # noqa: F401
+from .small import small_amr_tree, smooth_fields, problem_from_tree, add_scalars  # noqa: F401

@@ -42,3 +42,14 @@ def problem_from_tree(t, gamma=5.0 / 3.0, cfl=0.4, mode=0, nsteps=1, fields=smoo
         bc = tuple((0, 0) if per else (1, 1) for per in t.periodic)
     box = tuple(n / t.nb0[0] for n in t.nb0)
     return Problem(name, t.nb0, t.max_level, bc, box, gamma, cfl, mode, nsteps, level, ijk, U)
+
+
+def add_scalars(p, s_fields):
+    """The problem p with passive scalars appended: s_fields is a list of functions s(X, Y, Z) (concentration per
+    unit mass, evaluated at the cell centres); the conserved densities rho*s become variables 5, 6, ... of p.U."""
+    import dataclasses
+    X, Y, Z = cell_centres(p.level, p.ijk, p.nb0)
+    rho = p.U[:, 0]
+    q = [rho * np.broadcast_to(np.asarray(f(X, Y, Z), dtype=np.float64), rho.shape) for f in s_fields]
+    U = np.concatenate([p.U, np.stack(q, axis=1)], axis=1) if q else p.U
+    return dataclasses.replace(p, U=np.ascontiguousarray(U), name=p.name + "+%ds" % len(q))
