@@ -13,7 +13,13 @@
  *     EVERY block of every level holds data and is updated, covered (non-leaf) blocks too.
  *   - Conserved variables, in this order: rho, rho*vx, rho*vy, rho*vz, rho*E with
  *     rho*E = P/(gamma-1) + rho |v|^2 / 2 (eq. 1-3; eq. 8).  fp64.
- *   - "Caller layout" of a state: double U[nblocks][5][8][8][8], indexed [block][var][k][j][i]
+ *   - Passive scalars (sfh_config.nscalar = NS > 0): conserved densities q = rho*s
+ *     (y_i n_H of eq. 12, rho C_d T_d of eq. 13; source terms are not part of this
+ *     path) follow the 5 hydro variables of every cell.  Their interface flux is the Riemann solver's
+ *     mass flux times the interface value of s = q/rho on the side the mass comes from (cell-centred
+ *     in the predictor, minmod-limited linear in the corrector; reading R32); ghost fill,
+ *     eq. (16), restriction, flux registers and reflux treat them like the hydro variables.
+ *   - "Caller layout" of a state: double U[nblocks][5 + NS][8][8][8], indexed [block][var][k][j][i]
  *     (i = x fastest), blocks in the order given to sfh_create_mesh, INTERIOR cells only.
  *   - Internal layout: interior-only blocks in the library's own order (level-major, Morton within
  *     a level); ghost values are never stored for same-level neighbours (the stage kernels gather
@@ -59,7 +65,9 @@ typedef struct {
   double box_len[3];  /* physical size; cells are cubes of h_0 = box_len[0]/(nb0[0]*8)           */
   double gamma;       /* ideal-gas exponent of eq. (8)      */
   double cfl;         /* CFL number used by sfh_cfl_dt / sfh_advance                             */
+  int32_t nscalar;    /* passive scalars advected with the gas, 0..SFH_MAX_SCALARS   PAPER.md:80-88 (eq. 12-13) */
 } sfh_config;
+#define SFH_MAX_SCALARS 8
 
 /* ---- mesh: octree block table and neighbour map -------------------------- */
 
@@ -94,8 +102,9 @@ int sfh_num_faces(const sfh_mesh* m, int64_t* n_fine_faces, int64_t* n_coarse_fa
 /* Cell width of a level. */
 double sfh_cell_width(const sfh_mesh* m, int level);
 
-/* Bytes of ONE state copy in the internal layout, and of the work buffer (coarse-fine ghost
- * slabs, flux registers, per-block maximum speeds, reduction scratch). */
+/* Bytes of ONE state copy in the internal layout (hydro blocks, then the scalars' blocks), and of the
+ * work buffer (coarse-fine ghost slabs, flux registers, per-block maximum speeds, reduction scratch;
+ * with scalars also their slabs and registers and the mass fluxes of one stage). */
 int64_t sfh_state_bytes(const sfh_mesh* m);
 int64_t sfh_work_bytes(const sfh_mesh* m);
 
@@ -121,8 +130,8 @@ int sfh_get_state(sfh_mesh* m, int which, double* d_U, void* stream);
  * Asynchronous. */
 int sfh_fill_ghosts(sfh_mesh* m, int level, int which, int interp, double tau, void* stream);
 
-/* Writes ghosted blocks double G[nblocks][5][12][12][12] (caller block order, DEVICE) of role
- * `which`: interiors, and the 6 face halos exactly as the stage kernels see them (same-level
+/* Writes ghosted blocks double G[nblocks][5][12][12][12] (caller block order, DEVICE; the 5 hydro
+ * variables only) of role `which`: interiors, and the 6 face halos exactly as the stage kernels see them (same-level
  * gather, outflow copy, or the coarse-fine slabs last written by sfh_fill_ghosts); edge and
  * corner ghost cells, which no stage reads, are set to NaN.  For parity tests of the ghost fill. */
 int sfh_get_ghosted(sfh_mesh* m, int which, double* d_G, void* stream);
@@ -213,10 +222,10 @@ int64_t sfh_launch_count(const sfh_mesh* m);
 /* Per-kernel device timing for roofline reports.  While enabled, every launch of a hot-path kernel
  * is bracketed by two CUDA events on the caller's stream.  Kernel classes: 0 predictor stage (a4),
  * 1 corrector stage (a6+a7), 2 coarse-fine ghost prolongation (a3), 3 restriction (a8), 4 reflux
- * (a9), 5 CFL reduction (a10).  sfh_kernel_times synchronises on the recorded events, ADDS the
- * elapsed milliseconds and launch counts since the last call to ms[6] / count[6] (host arrays)
- * and forgets them. */
-#define SFH_NUM_KERNEL_CLASSES 6
+ * (a9), 5 CFL reduction (a10), 6 the passive-scalar kernels (stage, prolongation, restriction,
+ * reflux).  sfh_kernel_times synchronises on the recorded events, ADDS the elapsed milliseconds and
+ * launch counts since the last call to ms[7] / count[7] (host arrays) and forgets them. */
+#define SFH_NUM_KERNEL_CLASSES 7
 int sfh_profile(sfh_mesh* m, int enable);
 int sfh_kernel_times(sfh_mesh* m, double* ms, int64_t* count);
 

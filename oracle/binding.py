@@ -62,6 +62,10 @@ def lib():
         L.orc_refine_indicator.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_void_p]
         L.orc_transfer_state.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int]
         L.orc_status.restype = C.c_int64
+        L.orc_regrid.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_double, C.POINTER(C.c_void_p)]
+        L.orc_num_blocks.argtypes = [C.c_void_p]
+        L.orc_num_blocks.restype = C.c_int64
+        L.orc_block_list.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         _lib = L
     return _lib
 
@@ -98,18 +102,25 @@ def roe(WL, WR, d, gamma):
 class OracleMesh:
     """Oracle mesh + three ghosted state copies (0: U^n, 1: U^{n+1/2}, 2: U^{n+1})."""
 
-    def __init__(self, nb0, max_level, bc, box_len, gamma, cfl, level, ijk, nscalar=0):
+    def __init__(self, nb0, max_level, bc, box_len, gamma, cfl, level, ijk, nscalar=0, handle=None):
         self.L = lib()
-        self.level = np.ascontiguousarray(level, dtype=np.int32)
-        self.ijk = np.ascontiguousarray(ijk, dtype=np.int32).reshape(-1, 3)
-        self.nb = len(self.level)
         self.nv = NV + int(nscalar)          # 5 hydro variables + passive scalars rho*s
         self.cfg = make_config(nb0, max_level, bc, box_len, gamma, cfl, nscalar)
-        self.h = C.c_void_p()
-        rc = self.L.orc_create_mesh(C.byref(self.cfg), self.nb, self.level.ctypes.data, self.ijk.ctypes.data,
-                                    C.byref(self.h))
-        if rc != 0:
-            raise ValueError("orc_create_mesh failed: %d" % rc)
+        if handle is None:
+            self.level = np.ascontiguousarray(level, dtype=np.int32)
+            self.ijk = np.ascontiguousarray(ijk, dtype=np.int32).reshape(-1, 3)
+            self.nb = len(self.level)
+            self.h = C.c_void_p()
+            rc = self.L.orc_create_mesh(C.byref(self.cfg), self.nb, self.level.ctypes.data, self.ijk.ctypes.data,
+                                        C.byref(self.h))
+            if rc != 0:
+                raise ValueError("orc_create_mesh failed: %d" % rc)
+        else:                                # a mesh the oracle built itself (orc_regrid): read its block list back
+            self.h = handle
+            self.nb = int(self.L.orc_num_blocks(self.h))
+            self.level = np.zeros(self.nb, dtype=np.int32)
+            self.ijk = np.zeros((self.nb, 3), dtype=np.int32)
+            self.L.orc_block_list(self.h, self.level.ctypes.data, self.ijk.ctypes.data)
         self.U = [np.zeros((self.nb, self.nv, M, M, M)) for _ in range(3)]
         self.L.orc_bind(self.h, *[u.ctypes.data for u in self.U])
         self.max_level = int(max_level)
@@ -186,6 +197,17 @@ class OracleMesh:
     def transfer_from(self, src, which=0):
         """State copy `which` of this (new) mesh from the old mesh `src` after a regrid: copies and prolongations."""
         self._chk(self.L.orc_transfer_state(src.h, which, self.h, which))
+
+    def regrid(self, criterion, threshold, which=0, G=1.0):
+        """The regridded mesh (blocks flagged where the indicator >= threshold get children, 2:1 padded) holding the
+        state of copy `which` moved onto it (orc_regrid + orc_transfer_state)."""
+        h = C.c_void_p()
+        self._chk(self.L.orc_regrid(self.h, which, criterion, float(G), float(threshold), C.byref(h)))
+        c = self.cfg
+        new = OracleMesh(tuple(c.nb0), c.max_level, [tuple(b) for b in c.bc], tuple(c.box_len), c.gamma, c.cfl, None, None,
+                         nscalar=c.nscalar, handle=h)
+        new.transfer_from(self, which)
+        return new
 
     def refine_indicator(self, criterion=0, which=0, G=1.0):
         """Per-block refinement indicator (0: eq. 33-34 curvature, 1: h / Jeans length); ghosts must be filled."""

@@ -36,10 +36,13 @@
 // eq. 16-17); :599 (correction between coarse and fine cells = restriction).
 
 #include <algorithm>
+#include <array>
 #include <cmath>
 #include <cstdint>
 #include <cstdio>
 #include <cstring>
+#include <functional>
+#include <set>
 #include <unordered_map>
 #include <vector>
 
@@ -769,6 +772,74 @@ int orc_transfer_state(const Mesh* src, int src_which, Mesh* dst, int dst_which)
   }
   if (bad) { snprintf(dst->err, sizeof dst->err, "transfer_state: %d cells could not be resolved", bad); return -2; }
   return 0;
+}
+
+// ------------------------------------------------------------------ regrid: the new block list
+// PAPER.md:96 ("a block is refined ... subdivided into eight child blocks"), :277-285 (eq. 33-34), :641 (Jeans), :100
+// (lists built on the host).  The new tree, from the indicator of copy `which` (ghosts filled here):
+//   * every root block;
+//   * the 8 children of every block B of level < max_level that is in the OLD mesh, is in the NEW tree, and whose
+//     indicator is >= threshold (eq. 33 is written with >=) -- so a regrid deepens the tree by at most one level
+//     anywhere and drops the children of blocks that are no longer flagged;
+//   * closed under proper nesting (reading R25): every one of the 26 neighbour positions of a level-l block that lies
+//     inside the domain (periodic wrap applied; positions beyond an outflow face are skipped) is covered at level
+//     l-1; missing blocks are created with their 7 siblings and, recursively, their ancestors.
+// The new mesh lists its blocks level by level, (bx, by, bz) lexicographic within a level, and carries the same
+// configuration.  The state is then moved with orc_transfer_state.
+int orc_regrid(Mesh* m, int which, int criterion, double Gc, double threshold, Mesh** out) {
+  if (!out) return -1;
+  *out = nullptr;
+  for (int l = 0; l < m->nlev; ++l) if (int rc = fill_ghosts_level(*m, l, which, 0, 0.0)) return rc;
+  std::vector<double> ind(m->nb);
+  if (int rc = orc_refine_indicator(m, which, criterion, Gc, ind.data())) return rc;
+  typedef std::array<int, 3> C3;
+  std::vector<std::set<C3>> tree(m->nlev);
+  for (int64_t b = 0; b < m->nb; ++b) if (m->lev[b] == 0) tree[0].insert(C3{m->bx[b], m->by[b], m->bz[b]});
+  for (int l = 0; l + 1 < m->nlev; ++l)
+    for (int b : m->of_level[l]) {
+      const C3 c{m->bx[b], m->by[b], m->bz[b]};
+      if (!tree[l].count(c) || !(ind[b] >= threshold)) continue;
+      for (int q = 0; q < 8; ++q) tree[l + 1].insert(C3{2 * c[0] + (q & 1), 2 * c[1] + ((q >> 1) & 1), 2 * c[2] + ((q >> 2) & 1)});
+    }
+  // make the octet that holds block c of level l exist (and its ancestors)
+  std::function<void(int, C3)> ensure = [&](int l, C3 c) {
+    if (l == 0 || tree[l].count(c)) return;
+    const C3 par{c[0] >> 1, c[1] >> 1, c[2] >> 1};
+    ensure(l - 1, par);
+    for (int q = 0; q < 8; ++q) tree[l].insert(C3{2 * par[0] + (q & 1), 2 * par[1] + ((q >> 1) & 1), 2 * par[2] + ((q >> 2) & 1)});
+  };
+  bool changed = true;
+  while (changed) {
+    changed = false;
+    for (int l = m->nlev - 1; l >= 2; --l) {
+      const std::vector<C3> blocks(tree[l].begin(), tree[l].end());
+      for (const C3& x : blocks)
+        for (int dz = -1; dz <= 1; ++dz) for (int dy = -1; dy <= 1; ++dy) for (int dx = -1; dx <= 1; ++dx) {
+          int pos[3] = {x[0] + dx, x[1] + dy, x[2] + dz};
+          bool outside = false;
+          for (int d = 0; d < 3; ++d) {
+            const int n = m->cfg.nb0[d] << l;
+            if (pos[d] < 0) { if (m->cfg.bc[d][0] != 0) outside = true; else pos[d] += n; }
+            else if (pos[d] >= n) { if (m->cfg.bc[d][1] != 0) outside = true; else pos[d] -= n; }
+          }
+          if (outside) continue;
+          const C3 c{pos[0] >> 1, pos[1] >> 1, pos[2] >> 1};
+          if (!tree[l - 1].count(c)) { ensure(l - 1, c); changed = true; }
+        }
+    }
+  }
+  std::vector<int32_t> level, ijk;
+  for (int l = 0; l < m->nlev; ++l)
+    for (const C3& c : tree[l]) { level.push_back(l); ijk.push_back(c[0]); ijk.push_back(c[1]); ijk.push_back(c[2]); }
+  return orc_create_mesh(&m->cfg, int64_t(level.size()), level.data(), ijk.data(), out);
+}
+
+int64_t orc_num_blocks(const Mesh* m) { return m->nb; }
+void orc_block_list(const Mesh* m, int32_t* level, int32_t* ijk) {
+  for (int64_t b = 0; b < m->nb; ++b) {
+    level[b] = m->lev[b];
+    ijk[3 * b] = m->bx[b]; ijk[3 * b + 1] = m->by[b]; ijk[3 * b + 2] = m->bz[b];
+  }
 }
 
 }  // extern "C"

@@ -23,7 +23,8 @@ class SfhError(RuntimeError):
 
 class SfhConfig(C.Structure):
     _fields_ = [("nb0", C.c_int32 * 3), ("ncell", C.c_int32), ("nghost", C.c_int32), ("max_level", C.c_int32),
-                ("bc", (C.c_int32 * 2) * 3), ("box_len", C.c_double * 3), ("gamma", C.c_double), ("cfl", C.c_double)]
+                ("bc", (C.c_int32 * 2) * 3), ("box_len", C.c_double * 3), ("gamma", C.c_double), ("cfl", C.c_double),
+                ("nscalar", C.c_int32)]
 
 
 def library_path():
@@ -112,7 +113,8 @@ class Mesh:
     level[nb], ijk[nb,3]: the caller's block list; states cross this interface in caller layout
     double [nb][5][8][8][8] (interior cells, [block][var][k][j][i])."""
 
-    def __init__(self, nb0, max_level, bc, box_len, gamma, cfl, level, ijk, device="cuda:0", bind=True, lib=None):
+    def __init__(self, nb0, max_level, bc, box_len, gamma, cfl, level, ijk, device="cuda:0", bind=True, lib=None,
+                 nscalar=0):
         self.L = lib or load_library()
         self.level = np.ascontiguousarray(level, dtype=np.int32)
         self.ijk = np.ascontiguousarray(ijk, dtype=np.int32).reshape(-1, 3)
@@ -125,6 +127,8 @@ class Mesh:
                 cfg.bc[d][s] = int(bc[d][s])
         cfg.ncell, cfg.nghost, cfg.max_level = N, 2, int(max_level)
         cfg.gamma, cfg.cfl = float(gamma), float(cfl)
+        cfg.nscalar = int(nscalar)
+        self.nv = NV + int(nscalar)          # variables per cell in the caller layout
         self.cfg = cfg
         self.max_level = int(max_level)
         self.h = C.c_void_p()
@@ -139,6 +143,7 @@ class Mesh:
 
     @classmethod
     def from_problem(cls, p, **kw):
+        kw.setdefault("nscalar", p.U.shape[1] - NV)
         return cls(p.nb0, p.max_level, p.bc, p.box_len, p.gamma, p.cfl, p.level, p.ijk, **kw)
 
     def __del__(self):
@@ -201,7 +206,7 @@ class Mesh:
         if isinstance(U, np.ndarray):
             U = torch.from_numpy(np.ascontiguousarray(U, dtype=np.float64))
         U = U.to(device=self.device, dtype=torch.float64).contiguous()
-        assert U.numel() == self.nb * BLK, "state must be [nb][5][8][8][8]"
+        assert U.numel() == self.nb * self.nv * N ** 3, "state must be [nb][5 + nscalar][8][8][8]"
         return U
 
     def set_state(self, U, which=0):
@@ -213,7 +218,7 @@ class Mesh:
     def get_state(self, which=0):
         """torch tensor [nb][5][8][8][8] on the device."""
         import torch
-        out = torch.empty((self.nb, NV, N, N, N), dtype=torch.float64, device=self.device)
+        out = torch.empty((self.nb, self.nv, N, N, N), dtype=torch.float64, device=self.device)
         self._chk(self.L.sfh_get_state(self.h, which, out.data_ptr(), _stream()))
         return out
 
@@ -260,15 +265,15 @@ class Mesh:
                                           self.nupd.ctypes.data, _stream()))
         return self.t.value
 
-    KERNEL_CLASSES = ("predictor", "corrector", "prolong", "restrict", "reflux", "max_speed")
+    KERNEL_CLASSES = ("predictor", "corrector", "prolong", "restrict", "reflux", "max_speed", "scalars")
 
     def profile(self, enable=True):
         self._chk(self.L.sfh_profile(self.h, int(enable)))
 
     def kernel_times(self):
         """{class: (total ms, launches)} since the last call (synchronises)."""
-        ms = np.zeros(6, dtype=np.float64)
-        cnt = np.zeros(6, dtype=np.int64)
+        ms = np.zeros(len(self.KERNEL_CLASSES), dtype=np.float64)
+        cnt = np.zeros(len(self.KERNEL_CLASSES), dtype=np.int64)
         self._chk(self.L.sfh_kernel_times(self.h, ms.ctypes.data, cnt.ctypes.data))
         return {k: (float(ms[i]), int(cnt[i])) for i, k in enumerate(self.KERNEL_CLASSES)}
 

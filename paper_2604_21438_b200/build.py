@@ -11,8 +11,8 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = ["sfh_mesh.cpp", "sfh_kernels.cu", "sfh_kernels_aux.cu", "sfh_api.cu"]
-HEADERS = ["sfh_internal.h", "sfh_device.cuh", "sfh_kernels.cuh", os.path.join("..", "..", "include", "sfh.h")]
+SOURCES = ["sfh_mesh.cpp", "sfh_kernels.cu", "sfh_kernels_mf.cu", "sfh_kernels_aux.cu", "sfh_kernels_scalar.cu", "sfh_api.cu"]
+HEADERS = ["sfh_internal.h", "sfh_device.cuh", "sfh_kernels.cuh", "sfh_stage.cuh", os.path.join("..", "..", "include", "sfh.h")]
 
 
 def lib_path(nofma=False):
@@ -32,7 +32,7 @@ def build(force=False, nofma=False, verbose=False):
     if not force and os.path.exists(out) and all(os.path.getmtime(out) >= os.path.getmtime(d) for d in deps):
         return out
     cmd = [_nvcc(), "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-           "-Xcompiler", "-fPIC", "-shared", "-cudart", "static", "-o", out]
+           "-Xcompiler", "-fPIC", "-shared", "-cudart", "static", "--threads", "0", "-o", out]
     if nofma:
         cmd += ["-fmad=false"]
     if verbose:

@@ -29,6 +29,9 @@ struct sfh_mesh {
   int64_t* d_perm = nullptr;
   double* state[3] = {nullptr, nullptr, nullptr};
   double *ghost = nullptr, *ghost1 = nullptr, *R = nullptr, *FH = nullptr;   // ghost: slabs of U^n, ghost1: of U^{n+1/2}
+  // passive scalars (ns = cfg.nscalar > 0): slabs of q^n / q^{n+1/2}, flux registers, the stage kernels' mass fluxes
+  int ns = 0;
+  double *ghostS = nullptr, *ghostS1 = nullptr, *RS = nullptr, *FHS = nullptr, *MF = nullptr;
   unsigned long long* smax = nullptr;   // [MAX_LEVELS] bit patterns of the per-level maximum speed
   double *dt_dev = nullptr, *t_dev = nullptr;
   unsigned long long* nbad = nullptr;
@@ -53,16 +56,20 @@ constexpr size_t ALIGN = 256;
 inline size_t up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct WorkLayout {
-  size_t ghost, R, FH, bmax, scalars, total;
+  size_t ghost, R, FH, bmax, ghostS, RS, FHS, MF, scalars, total;
 };
 WorkLayout work_layout(const HostMesh& hm) {
   WorkLayout w;
-  const size_t ncf = hm.cf_block.size();
+  const size_t ncf = hm.cf_block.size(), ns = size_t(hm.cfg.nscalar);
   w.ghost = 0;
   w.R = up(w.ghost + 2 * ncf * SLAB * 8);      // two slab sets: the fill of U^n and of the half-step state
   w.FH = up(w.R + ncf * REG * 8);
   w.bmax = up(w.FH + size_t(hm.nfh) * REG * 8);
-  w.scalars = up(w.bmax + size_t(hm.nb) * 8);
+  w.ghostS = up(w.bmax + size_t(hm.nb) * 8);   // passive scalars: two slab sets, registers, mass fluxes
+  w.RS = up(w.ghostS + 2 * ncf * ns * NG * FACE * 8);
+  w.FHS = up(w.RS + ncf * ns * FACE * 8);
+  w.MF = up(w.FHS + size_t(hm.nfh) * ns * FACE * 8);
+  w.scalars = up(w.MF + (ns ? size_t(hm.nb) * 3 * 9 * FACE * 8 : 0));
   w.total = w.scalars + 4096;
   return w;
 }
@@ -159,6 +166,8 @@ struct Timed {
   }
 };
 inline double* role_buf(const sfh_mesh* m, int l, int r) { return m->state[m->role[l][r]]; }
+// scalar part of the same copy: Q[nb][ns][512] behind the hydro blocks
+inline double* role_q(const sfh_mesh* m, int l, int r) { return m->state[m->role[l][r]] + size_t(m->hm.nb) * BLK; }
 
 int check_bound(const sfh_mesh* m) {
   if (!m) return fail(SFH_EINVAL, "null mesh");
@@ -201,6 +210,19 @@ int fill_level(sfh_mesh* m, int l, int which, int interp, double tau, cudaStream
     CU(launch_prolong(p, st), "prolong_kernel");
   }
   m->launches += 1;
+  if (m->ns > 0) {      // the scalars' slabs: same gather, conserved values in every copy
+    ProlongScalarParams q;
+    if (interp) { q.C0 = role_q(m, l - 1, 0); q.C1 = role_q(m, l - 1, 1); q.C2 = role_q(m, l - 1, 2); }
+    else { q.C0 = q.C1 = q.C2 = role_q(m, l - 1, which); }
+    q.ghost = which == 1 ? m->ghostS1 : m->ghostS;
+    q.ghost1 = dual ? m->ghostS1 : nullptr;
+    q.cf_block = m->d_cf_block; q.cf_face = m->d_cf_face; q.parent = m->d_parent; q.coord = m->d_coord;
+    q.nbr27 = m->d_nbr27;
+    q.first = p.first; q.count = p.count; q.ns = m->ns; q.interp = interp; q.tau = tau; q.tau1 = tau1;
+    Timed tmr(m, 6, st);
+    CU(launch_prolong_scalar(q, st), "prolong_scalar_kernel");
+    m->launches += 1;
+  }
   return SFH_OK;
 }
 
@@ -219,6 +241,7 @@ int stage_level(sfh_mesh* m, int l, int stage, Dt dt, cudaStream_t st) {
   p.use_regs = stage == 1 && (hm.cf_count[l] > 0 || hm.reflux_count[l] > 0);
   p.riemann = m->riemann;
   p.bmax = stage == 1 ? m->bmax : nullptr;
+  p.mf = m->ns > 0 ? m->MF : nullptr;
   // the corrector overwrites the level's cached maxima with those of U^{n+1}: they stop describing U^n now
   if (stage == 1) { m->bmax_pending[l] = true; m->bmax_valid[l] = false; }
   {
@@ -226,6 +249,16 @@ int stage_level(sfh_mesh* m, int l, int stage, Dt dt, cudaStream_t st) {
     CU(launch_stage(stage, m->tm[m->role[l][src_role]], p, m->sms, st), "stage_kernel");
   }
   m->launches += 1;
+  if (m->ns > 0) {      // the scalars ride on the mass fluxes the stage has just exported
+    ScalarStageParams q;
+    q.Qsrc = role_q(m, l, src_role); q.Qn = role_q(m, l, 0); q.Qdst = role_q(m, l, stage == 0 ? 1 : 2);
+    q.Hsrc = p.Usrc; q.ghostH = p.ghost; q.ghostS = stage == 0 ? m->ghostS : m->ghostS1; q.mf = m->MF;
+    q.RS = m->RS; q.FHS = m->FHS; q.face_src = m->d_face_src; q.fslot = m->d_fslot;
+    q.dt_dev = dt.dev; q.dt = dt.host; q.h = hm.h[l]; q.first = p.first; q.count = p.count; q.ns = m->ns;
+    Timed tmr(m, 6, st);
+    CU(launch_scalar_stage(stage, q, st), "scalar_stage_kernel");
+    m->launches += 1;
+  }
   return SFH_OK;
 }
 
@@ -234,6 +267,9 @@ int zero_fine_registers(sfh_mesh* m, int coarse_level, cudaStream_t st) {   // r
   const int lf = coarse_level + 1;
   if (lf >= hm.nlev || hm.cf_count[lf] == 0) return SFH_OK;
   CU(cudaMemsetAsync(m->R + size_t(hm.cf_first[lf]) * REG, 0, size_t(hm.cf_count[lf]) * REG * 8, st), "memset R");
+  if (m->ns > 0)
+    CU(cudaMemsetAsync(m->RS + size_t(hm.cf_first[lf]) * m->ns * FACE, 0, size_t(hm.cf_count[lf]) * m->ns * FACE * 8, st),
+       "memset RS");
   return SFH_OK;
 }
 
@@ -263,6 +299,15 @@ int flux_correct_level(sfh_mesh* m, int lc, Dt dt, cudaStream_t st) {
        "reflux_kernel");
   }
   m->launches += hm.reflux_count[lc] > 0;
+  if (m->ns > 0) {
+    Timed tmr(m, 6, st);
+    CU(launch_restrict_scalar(role_q(m, lc + 1, 0), role_q(m, lc, 2), m->d_restrict_list + hm.restrict_first[lc],
+                              m->d_child0, int(hm.restrict_count[lc]), m->ns, st), "restrict_scalar_kernel");
+    CU(launch_reflux_scalar(role_q(m, lc, 2), m->RS, m->FHS, m->d_reflux_list + hm.reflux_first[lc], m->d_fslot,
+                            m->d_fh_src, int(hm.reflux_count[lc]), m->ns, hm.h[lc], dt.host, dt.dev, st),
+       "reflux_scalar_kernel");
+    m->launches += (hm.restrict_count[lc] > 0) + (hm.reflux_count[lc] > 0);
+  }
   return SFH_OK;
 }
 
@@ -402,6 +447,7 @@ int sfh_create_mesh(const sfh_config* cfg, int64_t nblocks, const int32_t* level
     return fail(rc, err);
   }
   for (int l = 0; l < MAX_LEVELS; ++l) for (int r = 0; r < 3; ++r) m->role[l][r] = r;
+  m->ns = cfg->nscalar;
   *out = m;
   return SFH_OK;
 }
@@ -449,7 +495,7 @@ double sfh_cell_width(const sfh_mesh* m, int level) {
   return m->hm.h[level];
 }
 
-int64_t sfh_state_bytes(const sfh_mesh* m) { return m ? int64_t(up(size_t(m->hm.nb) * BLK * 8)) : 0; }
+int64_t sfh_state_bytes(const sfh_mesh* m) { return m ? int64_t(up(size_t(m->hm.nb) * (NV + m->ns) * NC * 8)) : 0; }
 int64_t sfh_work_bytes(const sfh_mesh* m) { return m ? int64_t(work_layout(m->hm).total) : 0; }
 int64_t sfh_launch_count(const sfh_mesh* m) { return m ? m->launches : 0; }
 
@@ -508,6 +554,11 @@ int sfh_bind(sfh_mesh* m, void* d_state0, void* d_state1, void* d_state2, void* 
   m->R = reinterpret_cast<double*>(wb + w.R);
   m->FH = reinterpret_cast<double*>(wb + w.FH);
   m->bmax = reinterpret_cast<double*>(wb + w.bmax);
+  m->ghostS = reinterpret_cast<double*>(wb + w.ghostS);
+  m->ghostS1 = m->ghostS + hm.cf_block.size() * size_t(m->ns) * NG * FACE;
+  m->RS = reinterpret_cast<double*>(wb + w.RS);
+  m->FHS = reinterpret_cast<double*>(wb + w.FHS);
+  m->MF = reinterpret_cast<double*>(wb + w.MF);
   for (int l = 0; l < MAX_LEVELS; ++l) m->bmax_pending[l] = m->bmax_valid[l] = false;
   m->smax = reinterpret_cast<unsigned long long*>(wb + w.scalars);
   m->dt_dev = reinterpret_cast<double*>(wb + w.scalars + 256);
@@ -532,8 +583,10 @@ int sfh_set_state(sfh_mesh* m, int which, const double* d_U, void* stream) {
     if (which == 0) m->bmax_valid[l] = false;
     if (which == 2) m->bmax_pending[l] = false;
     CU(launch_permute(d_U, role_buf(m, l, which), m->d_perm, int(m->hm.lev_first[l]), int(m->hm.lev_count[l]), 1,
-                      which == 1, m->hm.cfg.gamma, S(stream)), "permute_kernel");
-    m->launches += m->hm.lev_count[l] > 0;
+                      which == 1, m->hm.cfg.gamma, m->ns, S(stream)), "permute_kernel");
+    CU(launch_permute_scalar(d_U, role_q(m, l, which), m->d_perm, int(m->hm.lev_first[l]), int(m->hm.lev_count[l]),
+                             m->ns, 1, S(stream)), "permute_scalar_kernel");
+    m->launches += (m->hm.lev_count[l] > 0) * (1 + (m->ns > 0));
   }
   return SFH_OK;
 }
@@ -544,8 +597,10 @@ int sfh_get_state(sfh_mesh* m, int which, double* d_U, void* stream) {
   if (which < 0 || which > 2 || !d_U) return fail(SFH_EINVAL, "bad argument");
   for (int l = 0; l < m->hm.nlev; ++l) {
     CU(launch_permute(role_buf(m, l, which), d_U, m->d_perm, int(m->hm.lev_first[l]), int(m->hm.lev_count[l]), 0,
-                      which == 1, m->hm.cfg.gamma, S(stream)), "permute_kernel");
-    m->launches += m->hm.lev_count[l] > 0;
+                      which == 1, m->hm.cfg.gamma, m->ns, S(stream)), "permute_kernel");
+    CU(launch_permute_scalar(role_q(m, l, which), d_U, m->d_perm, int(m->hm.lev_first[l]), int(m->hm.lev_count[l]),
+                             m->ns, 0, S(stream)), "permute_scalar_kernel");
+    m->launches += (m->hm.lev_count[l] > 0) * (1 + (m->ns > 0));
   }
   return SFH_OK;
 }
@@ -599,6 +654,7 @@ int sfh_transfer_state(sfh_mesh* src, int src_which, sfh_mesh* dst, int dst_whic
     if (hs.cfg.nb0[d] != hd.cfg.nb0[d] || hs.cfg.bc[d][0] != hd.cfg.bc[d][0] || hs.cfg.bc[d][1] != hd.cfg.bc[d][1] ||
         hs.cfg.box_len[d] != hd.cfg.box_len[d])
       return fail(SFH_EINVAL, "the two meshes describe different domains");
+  if (src->ns != dst->ns) return fail(SFH_EINVAL, "the two meshes carry different numbers of passive scalars");
   auto key = [](int l, const int32_t* c) {
     return (uint64_t(l) << 60) | (uint64_t(uint32_t(c[0]) & 0xFFFFF) << 40) | (uint64_t(uint32_t(c[1]) & 0xFFFFF) << 20) |
            uint64_t(uint32_t(c[2]) & 0xFFFFF);
@@ -638,7 +694,11 @@ int sfh_transfer_state(sfh_mesh* src, int src_which, sfh_mesh* dst, int dst_whic
     e = launch_transfer(role_buf(src, lc, src_which), role_buf(src, lp, src_which), src->ghost, src->d_face_src,
                         d_tsrc + first, dst->d_coord + 3 * first, role_buf(dst, l, dst_which) + size_t(first) * BLK,
                         int(count), st);
-    dst->launches += count > 0;
+    if (e == cudaSuccess)
+      e = launch_transfer_scalar(role_q(src, lc, src_which), role_q(src, lp, src_which), src->ghostS, src->d_face_src,
+                                 d_tsrc + first, dst->d_coord + 3 * first,
+                                 role_q(dst, l, dst_which) + size_t(first) * dst->ns * NC, int(count), dst->ns, st);
+    dst->launches += (count > 0) * (1 + (dst->ns > 0));
   }
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);
   cudaFree(d_tsrc);
@@ -694,7 +754,10 @@ int sfh_restrict(sfh_mesh* m, int coarse_level, int src_role, int dst_role, void
                      m->d_restrict_list + hm.restrict_first[coarse_level], m->d_child0,
                      int(hm.restrict_count[coarse_level]), hm.cfg.gamma, dst_role == 2 ? m->bmax : nullptr, S(stream)),
      "restrict_kernel");
-  m->launches += 1;
+  CU(launch_restrict_scalar(role_q(m, coarse_level + 1, src_role), role_q(m, coarse_level, dst_role),
+                            m->d_restrict_list + hm.restrict_first[coarse_level], m->d_child0,
+                            int(hm.restrict_count[coarse_level]), m->ns, S(stream)), "restrict_scalar_kernel");
+  m->launches += 1 + (m->ns > 0);
   return SFH_OK;
 }
 
@@ -743,7 +806,7 @@ int sfh_advance_host(sfh_mesh* m, const double* h_in, double* h_out, int ncoarse
   if (rc) return rc;
   if (!h_in || !h_out) return fail(SFH_EINVAL, "null host buffer");
   cudaStream_t st = S(stream);
-  const size_t bytes = size_t(m->hm.nb) * BLK * 8;
+  const size_t bytes = size_t(m->hm.nb) * (NV + m->ns) * NC * 8;
   // role 1 (U^{n+1/2}) of level 0 is scratch between steps: use its buffer for staging in caller order
   double* stage = m->state[m->role[0][1]];
   for (int l = 1; l < m->hm.nlev; ++l)

@@ -25,6 +25,7 @@ struct StageParams {
   int use_regs;          // corrector: the level has flux-register faces
   int riemann;           // 0 HLLC, 1 Roe
   double* bmax;          // corrector: per-block maximum CFL speed of U^{n+1} (or null)
+  double* mf;            // if non-null: mass flux of every face, [nb][3 axes][9 faces][64 pencils] (passive scalars)
 };
 
 struct TensorMaps {      // tensor maps of ONE state buffer seen as [5 nb][8][8][8]
@@ -92,8 +93,9 @@ cudaError_t launch_count_bad(const double* U, int first, int count, double gamma
                              int sms, cudaStream_t st);
 // dst[slot][...] = src[perm[slot]][...] (to_internal) or the inverse, for slots [first, first+count)
 // prim: the internal copy holds primitives (role 1); the caller's copy is always conserved
+// ns: passive scalars per cell: the caller's blocks are [5 + ns][512], the internal hydro blocks [5][512]
 cudaError_t launch_permute(const double* src, double* dst, const int64_t* perm, int first, int count, int to_internal,
-                           int prim, double gamma, cudaStream_t st);
+                           int prim, double gamma, int ns, cudaStream_t st);
 cudaError_t launch_ghosted(const double* U, const double* ghost, const int32_t* face_src, const int64_t* perm,
                            int first, int count, int prim, double gamma, double* G, cudaStream_t st);
 // per-block refinement indicator (criterion 0: eq. 33-34, 1: h / Jeans length) of slots [first, first+count), caller order
@@ -105,6 +107,44 @@ cudaError_t launch_refine_indicator(const double* U, const double* ghost, const 
 cudaError_t launch_transfer(const double* Uc, const double* Us, const double* ghost_s, const int32_t* face_src_s,
                             const int32_t* tsrc, const int32_t* coord_d, double* Ud, int count, cudaStream_t st);
 cudaError_t configure_kernels(int* sm_count);
+
+// ---- passive scalars (sfh_kernels_scalar.cu): Q[nb][ns][512] behind the hydro part of every state buffer ----------
+struct ScalarStageParams {
+  const double* Qsrc;    // scalars the stage differentiates: q^n (predictor) or q^{n+1/2} (corrector), conserved
+  const double* Qn;      // q^n
+  double* Qdst;          // q^{n+1/2} or q^{n+1}
+  const double* Hsrc;    // hydro copy of the same state as Qsrc (variable 0 = rho in both its forms)
+  const double* ghostH;  // its coarse-fine slabs
+  const double* ghostS;  // coarse-fine slabs of Qsrc  [ncf][ns][128]
+  const double* mf;      // mass fluxes written by the hydro stage  [nb][3][9][64]
+  double* RS;            // fine-side scalar flux registers [ncf][ns][64]
+  double* FHS;           // coarse-side                     [nfh][ns][64]
+  const int32_t* face_src;
+  const int32_t* fslot;
+  const double* dt_dev;
+  double dt, h;
+  int first, count, ns;
+};
+struct ProlongScalarParams {
+  const double *C0, *C1, *C2;   // scalar parts of the coarse level's copies (interp = 0: C0 only)
+  double* ghost;
+  double* ghost1;               // dual fill (interp only), or null
+  const int32_t *cf_block, *cf_face, *parent, *coord, *nbr27;
+  int first, count, ns, interp;
+  double tau, tau1;
+};
+cudaError_t launch_scalar_stage(int stage, const ScalarStageParams& p, cudaStream_t st);
+cudaError_t launch_prolong_scalar(const ProlongScalarParams& p, cudaStream_t st);
+cudaError_t launch_restrict_scalar(const double* Qfine, double* Qcoarse, const int32_t* list, const int32_t* child0,
+                                   int count, int ns, cudaStream_t st);
+cudaError_t launch_reflux_scalar(double* Q, const double* RS, const double* FHS, const int32_t* list,
+                                 const int32_t* fslot, const int32_t* fh_src, int count, int ns, double h, double dt,
+                                 const double* dt_dev, cudaStream_t st);
+cudaError_t launch_permute_scalar(const double* src, double* dst, const int64_t* perm, int first, int count, int ns,
+                                  int to_internal, cudaStream_t st);
+cudaError_t launch_transfer_scalar(const double* Qc, const double* Qs, const double* ghost_s, const int32_t* face_src_s,
+                                   const int32_t* tsrc, const int32_t* coord_d, double* Qd, int count, int ns,
+                                   cudaStream_t st);
 // fp64 issue-rate microbenchmark: `ctas` CTAs of 1024 threads, each thread `iters` x 16 x `chains` DFMAs
 cudaError_t launch_dfma_rate(int chains, int ctas, int iters, double* sink, cudaStream_t st);
 

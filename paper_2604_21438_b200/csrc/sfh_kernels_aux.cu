@@ -368,9 +368,10 @@ cudaError_t launch_count_bad(const double* U, int first, int count, double gamma
 // held as primitives internally, so its copies convert on the way in and out.
 // =====================================================================================================
 __global__ void __launch_bounds__(256) permute_kernel(const double2* __restrict__ src, double2* __restrict__ dst,
-                                                      const int64_t* __restrict__ perm, int first, int to_internal) {
+                                                      const int64_t* __restrict__ perm, int first, int to_internal,
+                                                      int ns) {
   const int s = first + blockIdx.x;
-  const size_t a = size_t(s) * (BLK / 2), b = size_t(perm[s]) * (BLK / 2);
+  const size_t a = size_t(s) * (BLK / 2), b = size_t(perm[s]) * ((NV + ns) * NC / 2);
   const double2* from = src + (to_internal ? b : a);
   double2* to = dst + (to_internal ? a : b);
   for (int t = threadIdx.x; t < BLK / 2; t += 256) to[t] = from[t];
@@ -378,9 +379,9 @@ __global__ void __launch_bounds__(256) permute_kernel(const double2* __restrict_
 
 __global__ void __launch_bounds__(256) permute_prim_kernel(const double* __restrict__ src, double* __restrict__ dst,
                                                            const int64_t* __restrict__ perm, int first, int to_internal,
-                                                           double gamma) {
+                                                           double gamma, int ns) {
   const int s = first + blockIdx.x;
-  const size_t a = size_t(s) * BLK, b = size_t(perm[s]) * BLK;
+  const size_t a = size_t(s) * BLK, b = size_t(perm[s]) * (NV + ns) * NC;
   const double* from = src + (to_internal ? b : a);
   double* to = dst + (to_internal ? a : b);
   const double gm1 = gamma - 1.0, igm1 = 1.0 / gm1;
@@ -396,11 +397,11 @@ __global__ void __launch_bounds__(256) permute_prim_kernel(const double* __restr
 }
 
 cudaError_t launch_permute(const double* src, double* dst, const int64_t* perm, int first, int count, int to_internal,
-                           int prim, double gamma, cudaStream_t st) {
+                           int prim, double gamma, int ns, cudaStream_t st) {
   if (count <= 0) return cudaSuccess;
-  if (prim) permute_prim_kernel<<<count, 256, 0, st>>>(src, dst, perm, first, to_internal, gamma);
+  if (prim) permute_prim_kernel<<<count, 256, 0, st>>>(src, dst, perm, first, to_internal, gamma, ns);
   else permute_kernel<<<count, 256, 0, st>>>(reinterpret_cast<const double2*>(src), reinterpret_cast<double2*>(dst), perm,
-                                             first, to_internal);
+                                             first, to_internal, ns);
   return cudaGetLastError();
 }
 

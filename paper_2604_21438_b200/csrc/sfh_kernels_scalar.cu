@@ -1,0 +1,360 @@
+// sfh_kernels_scalar.cu — passive scalars on the hydro sweep (eq. 12-13, PAPER.md:80-88;
+// DESIGN.md reading R32).  A scalar is carried as the conserved density q = rho * s; its interface flux is the
+// Riemann solver's mass flux (exported by the stage kernels, StageParams::mf) times the interface value of s on the
+// side the mass comes from, F_q = F_rho * (F_rho >= 0 ? s_L : s_R); s is cell-centred in the predictor and
+// minmod-limited linear in the corrector, like the other primitives (R11, R12).  The scalars live behind the hydro
+// part of every state buffer, Q[nb][ns][8][8][8] (conserved in all three roles), with their own coarse-fine ghost
+// slabs and flux registers; prolongation, eq. (16), restriction and reflux act on them exactly as on the hydro
+// variables.  These kernels move 40 B per scalar and cell-update and do a handful of flops: plain gather kernels.
+#include <cmath>
+
+#include "sfh_device.cuh"
+#include "sfh_kernels.cuh"
+
+namespace sfh {
+
+constexpr int M12 = N + 2 * NG;      // ghosted edge
+constexpr int G3 = M12 * M12 * M12;
+__device__ __forceinline__ int gpos(int i, int j, int k) { return ((k + NG) * M12 + (j + NG)) * M12 + (i + NG); }
+
+// Source of one variable of ghosted cell (i, j, k) of block s: the block itself, the same-level neighbour, the block's
+// own edge layer (outflow) or the coarse-fine slab.  Edge / corner ghosts (no stage reads them): returns null.
+// U: array [nb][nvar][512] (+ v * NC selects the variable); slab: [ncf][nslabvar][128] (+ v * 128).
+__device__ __forceinline__ const double* ghost_src(const double* __restrict__ U, int nvar, const double* __restrict__ slab,
+                                                   int nslabvar, const int32_t* __restrict__ face_src, int s, int i, int j,
+                                                   int k, int* vstride) {
+  const int o[3] = {i < 0 ? -1 : i >= N ? 1 : 0, j < 0 ? -1 : j >= N ? 1 : 0, k < 0 ? -1 : k >= N ? 1 : 0};
+  const int nout = (o[0] != 0) + (o[1] != 0) + (o[2] != 0);
+  *vstride = NC;
+  if (nout == 0) return U + size_t(s) * nvar * NC + (k * 8 + j) * 8 + i;
+  if (nout > 1) return nullptr;
+  const int axis = o[0] ? 0 : o[1] ? 1 : 2, side = o[axis] > 0;
+  const int src = face_src[s * 6 + 2 * axis + side];
+  int q[3] = {i, j, k};
+  if (src == SRC_OUTFLOW) {
+    q[axis] = side ? N - 1 : 0;
+    return U + size_t(s) * nvar * NC + (q[2] * 8 + q[1]) * 8 + q[0];
+  }
+  if (src >= 0) {
+    q[axis] += side ? -N : N;
+    return U + size_t(src) * nvar * NC + (q[2] * 8 + q[1]) * 8 + q[0];
+  }
+  const int ll = side ? q[axis] - N : q[axis] + NG;
+  *vstride = NG * FACE;
+  return slab + size_t(-2 - src) * nslabvar * (NG * FACE) + slab_pos(axis, ll, axis == 0 ? j : i, axis == 2 ? j : k);
+}
+
+// =====================================================================================================
+// Scalar stage: one CTA of 256 threads per block.  rho and s = q / rho of the block and its two-layer face halos go
+// to shared memory (gathered like the stage kernels gather: neighbour interiors, outflow copies, coarse-fine slabs);
+// every thread then updates two cells: the six face fluxes of a cell (each face is evaluated by both its cells,
+// a few flops), dF in the order (x + y) + z, q_out = q^n - lambda dF.  STAGE 1 also feeds the scalar flux registers
+// of coarse-fine faces (fine side += dt F, coarse leaf side = F; one contributor per entry: no atomics needed).
+// =====================================================================================================
+template <int STAGE>
+__global__ void __launch_bounds__(256) scalar_stage_kernel(const ScalarStageParams p) {
+  __shared__ double rho[G3];
+  __shared__ double sv[G3];
+  const int s = p.first + blockIdx.x;
+  const int t = threadIdx.x;
+  const double dt = p.dt_dev ? *p.dt_dev : p.dt;
+  const double lam = (STAGE == 0 ? 0.5 : 1.0) * dt / p.h;
+  for (int c = t; c < G3; c += 256) {
+    const int i = c % M12 - NG, j = (c / M12) % M12 - NG, k = c / (M12 * M12) - NG;
+    int vs;
+    const double* from = ghost_src(p.Hsrc, NV, p.ghostH, NV, p.face_src, s, i, j, k, &vs);
+    rho[c] = from ? from[0] : 1.0;          // variable 0 of both the conserved and the primitive copies is rho
+  }
+  const double* mf = p.mf + size_t(s) * 3 * 9 * FACE;
+  for (int v = 0; v < p.ns; ++v) {
+    __syncthreads();                         // rho is complete / the previous scalar's sv is no longer read
+    for (int c = t; c < G3; c += 256) {
+      const int i = c % M12 - NG, j = (c / M12) % M12 - NG, k = c / (M12 * M12) - NG;
+      int vs;
+      const double* from = ghost_src(p.Qsrc, p.ns, p.ghostS, p.ns, p.face_src, s, i, j, k, &vs);
+      sv[c] = from ? from[v * vs] / rho[c] : 0.0;
+    }
+    __syncthreads();
+#pragma unroll 1
+    for (int cell = t; cell < NC; cell += 256) {
+      const int ijk[3] = {cell & 7, (cell >> 3) & 7, cell >> 6};
+      const int st[3] = {1, M12, M12 * M12};
+      const int m0 = gpos(ijk[0], ijk[1], ijk[2]);
+      double dF[3];
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {
+        const int ta = d == 0 ? ijk[1] : ijk[0], tb = d == 2 ? ijk[1] : ijk[2], c = ijk[d];
+        double F[2];
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {        // the cell's lower (e = 0) and upper face: face index c + e
+          const int ml = m0 + (e - 1) * st[d], mr = ml + st[d];     // cells left and right of the face
+          double sL = sv[ml], sR = sv[mr];
+          if (STAGE == 1) {
+            sL = sL + 0.5 * minmod(sv[mr] - sv[ml], sv[ml] - sv[ml - st[d]]);
+            sR = sR - 0.5 * minmod(sv[mr + st[d]] - sv[mr], sv[mr] - sv[ml]);
+          }
+          const double fm = mf[(d * 9 + c + e) * FACE + tb * 8 + ta];
+          F[e] = fm * (fm >= 0.0 ? sL : sR);
+        }
+        dF[d] = F[1] - F[0];
+        if (STAGE == 1 && (c == 0 || c == N - 1)) {        // flux registers (a7 for the scalars)
+          const int e = c == 0 ? 0 : 1, f = s * 6 + 2 * d + e;
+          const int src = p.face_src[f], fs = p.fslot[f];
+          if (src <= -2) {
+            double* r = p.RS + (size_t(-2 - src) * p.ns + v) * FACE + tb * 8 + ta;
+            *r = *r + dt * F[e];
+          }
+          if (fs >= 0) p.FHS[(size_t(fs) * p.ns + v) * FACE + tb * 8 + ta] = F[e];
+        }
+      }
+      const size_t o = (size_t(s) * p.ns + v) * NC + cell;
+      p.Qdst[o] = p.Qn[o] - lam * ((dF[0] + dF[1]) + dF[2]);
+    }
+  }
+}
+
+cudaError_t launch_scalar_stage(int stage, const ScalarStageParams& p, cudaStream_t st) {
+  if (p.count <= 0 || p.ns <= 0) return cudaSuccess;
+  if (stage == 0) scalar_stage_kernel<0><<<p.count, 256, 0, st>>>(p);
+  else scalar_stage_kernel<1><<<p.count, 256, 0, st>>>(p);
+  return cudaGetLastError();
+}
+
+// =====================================================================================================
+// Coarse-fine ghost slabs of the scalars: the geometry of prolong_kernel (sfh_kernels_aux.cu), one variable at a
+// time, conserved values throughout (no primitive copies).  interp: eq. (16) at tau (and at tau1 into ghost1).
+// =====================================================================================================
+constexpr int PR_RIM = 36, PR_CELLS = PR_RIM + 2 * 16;
+
+__global__ void __launch_bounds__(128) prolong_scalar_kernel(const ProlongScalarParams p) {
+  __shared__ double q[PR_CELLS], q1[PR_CELLS];
+  __shared__ int missing;
+  const int slot = p.first + blockIdx.x;
+  const int F = p.cf_block[slot], f = p.cf_face[slot], axis = f >> 1, side = f & 1;
+  const int P = p.parent[F];
+  const int t1ax = axis == 0 ? 1 : 0, t2ax = axis == 2 ? 1 : 2;
+  int oct[3];
+#pragma unroll
+  for (int d = 0; d < 3; ++d) oct[d] = p.coord[3 * F + d] & 1;
+  const int r = threadIdx.x;
+  if (r == 0) missing = 0;
+  // ---- which coarse cell thread r < 68 gathers (the same for every variable)
+  size_t src_off = 0;
+  bool gather = false;
+  if (r < PR_CELLS) {
+    int ca, c1, c2;
+    bool needed = true;
+    if (r < PR_RIM) {
+      ca = 0; c1 = r % 6 - 1; c2 = r / 6 - 1;
+      needed = !((c1 < 0 || c1 > 3) && (c2 < 0 || c2 > 3));
+    } else {
+      const int e = (r - PR_RIM) & 15;
+      ca = r < PR_RIM + 16 ? -1 : 1; c1 = e & 3; c2 = e >> 2;
+    }
+    if (needed) {
+      int c[3], rg[3];
+      c[axis] = (side ? oct[axis] * 4 + 4 : oct[axis] * 4 - 1) + ca;
+      c[t1ax] = oct[t1ax] * 4 + c1;
+      c[t2ax] = oct[t2ax] * 4 + c2;
+      const int32_t* nb = p.nbr27 + size_t(P) * 27;
+      const bool out_lo[3] = {nb[12] == NBR_OUTSIDE, nb[10] == NBR_OUTSIDE, nb[4] == NBR_OUTSIDE};
+      const bool out_hi[3] = {nb[14] == NBR_OUTSIDE, nb[16] == NBR_OUTSIDE, nb[22] == NBR_OUTSIDE};
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {
+        rg[d] = 0;
+        if (c[d] < 0) { if (out_lo[d]) c[d] = 0; else { rg[d] = -1; c[d] += N; } }
+        else if (c[d] >= N) { if (out_hi[d]) c[d] = N - 1; else { rg[d] = 1; c[d] -= N; } }
+      }
+      const int Q = nb[(rg[2] + 1) * 9 + (rg[1] + 1) * 3 + (rg[0] + 1)];
+      if (Q < 0) missing = 1;
+      else { gather = true; src_off = size_t(Q) * p.ns * NC + (c[2] * 8 + c[1]) * 8 + c[0]; }
+    }
+  }
+  // ---- which fine ghost cell thread r computes
+  int fc[3];
+  if (axis == 0) { const int ll = r & 1; fc[0] = side ? N + ll : ll - NG; fc[1] = (r >> 1) & 7; fc[2] = r >> 4; }
+  else if (axis == 1) { const int ll = (r >> 3) & 1; fc[0] = r & 7; fc[1] = side ? N + ll : ll - NG; fc[2] = r >> 4; }
+  else { const int ll = r >> 6; fc[0] = r & 7; fc[1] = (r >> 3) & 7; fc[2] = side ? N + ll : ll - NG; }
+  const int c1 = fc[t1ax] >> 1, c2 = fc[t2ax] >> 1;
+  const int ctr = (c2 + 1) * 6 + (c1 + 1);
+  int nbp[3], nbm[3];
+  nbp[axis] = PR_RIM + 16 + c2 * 4 + c1; nbm[axis] = PR_RIM + c2 * 4 + c1;
+  nbp[t1ax] = ctr + 1; nbm[t1ax] = ctr - 1;
+  nbp[t2ax] = ctr + 6; nbm[t2ax] = ctr - 6;
+  const int ll = fc[axis] < 0 ? fc[axis] + NG : fc[axis] - N;
+  const int rout = slab_pos(axis, ll, fc[axis == 0 ? 1 : 0], fc[axis == 2 ? 1 : 2]);
+  for (int v = 0; v < p.ns; ++v) {
+    __syncthreads();
+    if (gather) {
+      const size_t o = src_off + size_t(v) * NC;
+      const double u0 = p.C0[o];
+      if (p.interp) {
+        const double u1 = p.C1[o], u2 = p.C2[o];
+        q[r] = time_interp(u0, u1, u2, p.tau);
+        if (p.ghost1) q1[r] = time_interp(u0, u1, u2, p.tau1);
+      } else {
+        q[r] = u0;
+      }
+    }
+    __syncthreads();
+    auto fine_value = [&](const double* qq, double* __restrict__ ghost) {
+      const double q0 = qq[ctr];
+      double val = q0;
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {
+        const double sig = (fc[d] & 1) ? 0.25 : -0.25;
+        val = val + sig * minmod(qq[nbp[d]] - q0, q0 - qq[nbm[d]]);
+      }
+      if (missing) val = nan("");
+      ghost[(size_t(slot) * p.ns + v) * (NG * FACE) + rout] = val;
+    };
+    fine_value(q, p.ghost);
+    if (p.ghost1) fine_value(q1, p.ghost1);
+  }
+}
+
+cudaError_t launch_prolong_scalar(const ProlongScalarParams& p, cudaStream_t st) {
+  if (p.count <= 0 || p.ns <= 0) return cudaSuccess;
+  prolong_scalar_kernel<<<p.count, 128, 0, st>>>(p);
+  return cudaGetLastError();
+}
+
+// =====================================================================================================
+// Restriction and reflux of the scalars: restrict_kernel / reflux_kernel (sfh_kernels_aux.cu) on Q, RS, FHS.
+// =====================================================================================================
+__global__ void __launch_bounds__(NC) restrict_scalar_kernel(const double* __restrict__ Qf, double* __restrict__ Qc,
+                                                             const int32_t* __restrict__ list,
+                                                             const int32_t* __restrict__ child0, int ns) {
+  const int b = list[blockIdx.x];
+  const int t = threadIdx.x, i = t & 7, j = (t >> 3) & 7, k = t >> 6;
+  const int child = child0[b] + (i >> 2) + 2 * (j >> 2) + 4 * (k >> 2);
+  const int fi = 2 * (i & 3), fj = 2 * (j & 3), fk = 2 * (k & 3);
+  for (int v = 0; v < ns; ++v) {
+    const double* src = Qf + (size_t(child) * ns + v) * NC;
+    double sum = 0.0;
+#pragma unroll
+    for (int c = 0; c < 8; ++c) sum += src[((fk + ((c >> 2) & 1)) * 8 + fj + ((c >> 1) & 1)) * 8 + fi + (c & 1)];
+    Qc[(size_t(b) * ns + v) * NC + t] = 0.125 * sum;
+  }
+}
+
+cudaError_t launch_restrict_scalar(const double* Qfine, double* Qcoarse, const int32_t* list, const int32_t* child0,
+                                   int count, int ns, cudaStream_t st) {
+  if (count <= 0 || ns <= 0) return cudaSuccess;
+  restrict_scalar_kernel<<<count, NC, 0, st>>>(Qfine, Qcoarse, list, child0, ns);
+  return cudaGetLastError();
+}
+
+__global__ void __launch_bounds__(FACE) reflux_scalar_kernel(double* __restrict__ Q, const double* __restrict__ RS,
+                                                             const double* __restrict__ FHS,
+                                                             const int32_t* __restrict__ list,
+                                                             const int32_t* __restrict__ fslot,
+                                                             const int32_t* __restrict__ fh_src, int ns, double h,
+                                                             double dt_host, const double* __restrict__ dt_dev) {
+  const int b = list[blockIdx.x];
+  const int t = threadIdx.x, ta = t & 7, tb = t >> 3;
+  const double dt = dt_dev ? *dt_dev : dt_host;
+  for (int f = 0; f < 6; ++f) {
+    const int fs = fslot[b * 6 + f];
+    if (fs >= 0) {
+      const int d = f >> 1, side = f & 1, c = side ? N - 1 : 0;
+      const double s = side ? 1.0 : -1.0;
+      const int cell = d == 0 ? (tb * 8 + ta) * 8 + c : d == 1 ? (tb * 8 + c) * 8 + ta : (c * 8 + tb) * 8 + ta;
+      const int slot = fh_src[fs * 4 + (ta >> 2) + 2 * (tb >> 2)];
+      const int fa = 2 * (ta & 3), fb = 2 * (tb & 3);
+      for (int v = 0; v < ns; ++v) {
+        const double* r = RS + (size_t(slot) * ns + v) * FACE;
+        double sumR = 0.0;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) sumR += r[(fb + (q >> 1)) * 8 + fa + (q & 1)];
+        const double FHv = FHS[(size_t(fs) * ns + v) * FACE + t];
+        double* u = Q + (size_t(b) * ns + v) * NC + cell;
+        *u = *u - (s / h) * (0.25 * sumR - dt * FHv);
+      }
+    }
+    __syncthreads();
+  }
+}
+
+cudaError_t launch_reflux_scalar(double* Q, const double* RS, const double* FHS, const int32_t* list,
+                                 const int32_t* fslot, const int32_t* fh_src, int count, int ns, double h, double dt,
+                                 const double* dt_dev, cudaStream_t st) {
+  if (count <= 0 || ns <= 0) return cudaSuccess;
+  reflux_scalar_kernel<<<count, FACE, 0, st>>>(Q, RS, FHS, list, fslot, fh_src, ns, h, dt, dt_dev);
+  return cudaGetLastError();
+}
+
+// =====================================================================================================
+// caller layout [nb][5 + ns][512] <-> internal scalar part [slot][ns][512]
+// =====================================================================================================
+__global__ void __launch_bounds__(256) permute_scalar_kernel(const double2* __restrict__ src, double2* __restrict__ dst,
+                                                             const int64_t* __restrict__ perm, int first, int ns,
+                                                             int to_internal) {
+  const int s = first + blockIdx.x;
+  const size_t in = size_t(s) * ns * (NC / 2);                               // internal: scalars only
+  const size_t ca = (size_t(perm[s]) * (NV + ns) + NV) * (NC / 2);           // caller: behind the 5 hydro variables
+  const double2* from = src + (to_internal ? ca : in);
+  double2* to = dst + (to_internal ? in : ca);
+  for (int t = threadIdx.x; t < ns * (NC / 2); t += 256) to[t] = from[t];
+}
+
+cudaError_t launch_permute_scalar(const double* src, double* dst, const int64_t* perm, int first, int count, int ns,
+                                  int to_internal, cudaStream_t st) {
+  if (count <= 0 || ns <= 0) return cudaSuccess;
+  permute_scalar_kernel<<<count, 256, 0, st>>>(reinterpret_cast<const double2*>(src), reinterpret_cast<double2*>(dst),
+                                               perm, first, ns, to_internal);
+  return cudaGetLastError();
+}
+
+// =====================================================================================================
+// Regrid: scalars of a new mesh from an old one (transfer_kernel of sfh_kernels_aux.cu on Q and the scalar slabs)
+// =====================================================================================================
+__global__ void __launch_bounds__(256) transfer_scalar_kernel(const double* __restrict__ Qc, const double* __restrict__ Qs,
+                                                              const double* __restrict__ ghost_s,
+                                                              const int32_t* __restrict__ face_src_s,
+                                                              const int32_t* __restrict__ tsrc,
+                                                              const int32_t* __restrict__ coord_d, double* __restrict__ Qd,
+                                                              int ns) {
+  const int d = blockIdx.x;
+  const int t = tsrc[d];
+  double* out = Qd + size_t(d) * ns * NC;
+  if (t >= 0) {
+    const double2* from = reinterpret_cast<const double2*>(Qc + size_t(t) * ns * NC);
+    double2* to = reinterpret_cast<double2*>(out);
+    for (int q = threadIdx.x; q < ns * NC / 2; q += 256) to[q] = from[q];
+    return;
+  }
+  const int P = -2 - t;
+  const int oct[3] = {coord_d[3 * d] & 1, coord_d[3 * d + 1] & 1, coord_d[3 * d + 2] & 1};
+  for (int v = 0; v < ns; ++v)
+    for (int cell = threadIdx.x; cell < NC; cell += 256) {
+      const int f[3] = {cell & 7, (cell >> 3) & 7, cell >> 6};
+      const int c[3] = {oct[0] * 4 + (f[0] >> 1), oct[1] * 4 + (f[1] >> 1), oct[2] * 4 + (f[2] >> 1)};
+      auto fetch = [&](int c0, int c1, int c2) {
+        int vs;
+        const double* from = ghost_src(Qs, ns, ghost_s, ns, face_src_s, P, c0, c1, c2, &vs);
+        // one ghost layer only: layer index next to the face (ghost_src addresses layer c - N / c + NG of the slab)
+        return from[v * vs];
+      };
+      const double Q = fetch(c[0], c[1], c[2]);
+      double val = Q;
+#pragma unroll
+      for (int a = 0; a < 3; ++a) {
+        const double Qp = fetch(c[0] + (a == 0), c[1] + (a == 1), c[2] + (a == 2));
+        const double Qm = fetch(c[0] - (a == 0), c[1] - (a == 1), c[2] - (a == 2));
+        const double sig = (f[a] & 1) ? 0.25 : -0.25;
+        val = val + sig * minmod(Qp - Q, Q - Qm);
+      }
+      out[size_t(v) * NC + cell] = val;
+    }
+}
+
+cudaError_t launch_transfer_scalar(const double* Qc, const double* Qs, const double* ghost_s, const int32_t* face_src_s,
+                                   const int32_t* tsrc, const int32_t* coord_d, double* Qd, int count, int ns,
+                                   cudaStream_t st) {
+  if (count <= 0 || ns <= 0) return cudaSuccess;
+  transfer_scalar_kernel<<<count, 256, 0, st>>>(Qc, Qs, ghost_s, face_src_s, tsrc, coord_d, Qd, ns);
+  return cudaGetLastError();
+}
+
+}  // namespace sfh

@@ -65,6 +65,7 @@ int build_host_mesh(const sfh_config& cfg, int64_t nblocks, const int32_t* level
     if ((cfg.bc[d][0] == 0) != (cfg.bc[d][1] == 0)) { err = "periodic bc must be set on both faces of an axis"; return SFH_EINVAL; }
   }
   if (!(cfg.gamma > 1.0) || !(cfg.cfl > 0.0)) { err = "gamma must be > 1 and cfl > 0"; return SFH_EINVAL; }
+  if (cfg.nscalar < 0 || cfg.nscalar > SFH_MAX_SCALARS) { err = "nscalar out of range"; return SFH_EINVAL; }
 
   m = HostMesh();
   m.cfg = cfg;

@@ -552,3 +552,139 @@ def test_cfl_dt_describes_role0_after_a_corrector_launch():
             assert abs(g.cfl_dt(l) - want) <= TOLDT * want
         g.restrict(l, 0, 2) if l < p.max_level else None
         assert abs(g.cfl_dt(l) - want) <= TOLDT * want
+
+
+# ------------------------------------------------------------------ passive scalars (R32)
+def scalar_fields():
+    from test_oracle_scalar_pins import blob, wavy
+    return [wavy, blob, lambda X, Y, Z: 0.37 + 0 * X]
+
+
+def compare_all(o, g, gamma, tol):
+    """Hydro variables in the parity norm, every scalar normalised by its largest conserved density."""
+    Uo = o.get_state()
+    Ug = g.get_state().cpu().numpy()
+    assert np.isfinite(Ug).all() and Ug.shape == Uo.shape
+    err = parity_errors(Ug, Uo, gamma)
+    assert (err <= tol).all(), err
+    for v in range(5, Uo.shape[1]):
+        e = np.abs(Ug[:, v] - Uo[:, v]).max() / np.abs(Uo[:, v]).max()
+        assert e <= tol, (v, e)
+
+
+@pytest.mark.parametrize("name", ["C1", "C2/4", "C4/4", "C5/8", "amr-small", "amr-outflow", "ragged", "one-block"])
+def test_scalar_parity(name):
+    from sfh_inputs import add_scalars
+    p = add_scalars(PROBLEMS[name](), scalar_fields())
+    assert p.U.shape[1] == 8
+    o, g = both(p)
+    o.advance(1, p.mode)
+    g.advance(1, p.mode)
+    assert abs(g.t.value - o.t.value) <= TOLDT * o.t.value
+    compare_all(o, g, p.gamma, TOL1)
+    n = max(p.nsteps, 10) - 1
+    o.advance(n, p.mode)
+    g.advance(n, p.mode)
+    assert np.array_equal(o.nupd, g.nupd), (o.nupd, g.nupd)
+    compare_all(o, g, p.gamma, TOL10)
+    # a uniform concentration stays uniform on the CUDA path as well
+    U = g.get_state().cpu().numpy()
+    assert np.abs(U[:, 7] / U[:, 0] - 0.37).max() < 1e-13
+
+
+@pytest.mark.parametrize("roe", [False, True])
+def test_scalars_do_not_change_the_hydro_variables(roe):
+    from sfh_inputs import add_scalars
+    p0 = PROBLEMS["amr-small"]()
+    p3 = add_scalars(p0, scalar_fields())
+    a, b = gpu_for(p0), gpu_for(p3)
+    for g in (a, b):
+        g.set_riemann("roe" if roe else "hllc")
+        g.restrict_all(0)
+        g.advance(3, 1)
+    assert np.array_equal(a.nupd, b.nupd)
+    assert np.array_equal(a.get_state().cpu().numpy(), b.get_state().cpu().numpy()[:, :5])
+    if roe:        # and the Roe mass flux carries them like the HLLC one: parity with the oracle
+        o = oracle_for(p3)
+        o.set_riemann("roe")
+        o.restrict_all(0)
+        o.advance(3, 1)
+        compare_all(o, b, p3.gamma, TOL10)
+
+
+@pytest.mark.parametrize("mode", [1, 0])
+def test_linear_scalar_advection_exact_and_conserved(mode):
+    from test_oracle_scalar_pins import advected_s, advection_problem as scalar_advection_problem
+    from sfh_inputs.configs import cell_centres
+    p = scalar_advection_problem(mode)
+    o, g = both(p)
+    X, Y, Z = cell_centres(p.level, p.ijk, p.nb0)
+    d = np.minimum.reduce([X, Y, Z, 1 - X, 1 - Y, 1 - Z]) * (p.nb0[0] * 8)
+    for step in (1, 2):
+        o.advance(1, mode)
+        g.advance(1, mode)
+        U = g.get_state().cpu().numpy()
+        err = np.abs(U[:, 5] / U[:, 0] - advected_s(X, Y, Z, g.t.value))
+        assert err[d > 3 * step + 2].max() < 4e-14, err[d > 3 * step + 2].max()
+        compare_all(o, g, p.gamma, TOL1)
+
+
+def test_scalar_mass_conserved_across_refinement_boundaries():
+    from helpers import leaf_totals
+    from sfh_inputs import add_scalars
+    p = add_scalars(PROBLEMS["amr-small"](), scalar_fields())
+    o, g = both(p)
+    leaf, h0 = o.is_leaf(), o.cell_width(0)
+
+    def totals():
+        U = g.get_state().cpu().numpy()
+        out = []
+        for v in range(5, 8):
+            W = np.zeros((len(U), 5, 8, 8, 8))
+            W[:, 0] = U[:, v]
+            out.append(leaf_totals(leaf, W, p.level, h0)[0])
+        return np.array(out)
+    t0 = totals()
+    g.advance(3, 1)
+    t1 = totals()
+    assert (np.abs(t1 - t0) <= 1e-14 * np.abs(t0)).all(), (t1 - t0) / t0
+
+
+def test_regrid_transfer_with_scalars():
+    from sfh_inputs import add_scalars
+    told, tnew = regrid_pair()
+    p = add_scalars(problem_from_tree(told, mode=1), scalar_fields())
+    q = add_scalars(problem_from_tree(tnew, mode=1), scalar_fields())
+    o, g = both(p)
+    o.advance(2, 1)
+    g.advance(2, 1)
+    o.fill_ghosts(-1, 0, 0, 0.0)
+    o2 = oracle_for(q)
+    g2 = sfh.Mesh.from_problem(q)
+    o2.transfer_from(o)
+    g2.transfer_from(g)
+    compare_all(o2, g2, p.gamma, TOL10)
+    o2.restrict_all(0)
+    g2.restrict_all(0)
+    o2.advance(2, 1)
+    g2.advance(2, 1)
+    compare_all(o2, g2, p.gamma, TOL10)
+    with pytest.raises(sfh.SfhError):         # different numbers of scalars
+        sfh.Mesh.from_problem(problem_from_tree(tnew, mode=1)).transfer_from(g)
+
+
+def test_scalar_count_is_validated_and_host_path_carries_scalars():
+    import torch
+    from sfh_inputs import add_scalars
+    p = PROBLEMS["one-block"]()
+    with pytest.raises(sfh.SfhError) as e:
+        sfh.Mesh.from_problem(p, nscalar=9, bind=False)
+    assert e.value.code == -1
+    p = add_scalars(PROBLEMS["C2/4"](), scalar_fields()[:2])
+    g = gpu_for(p)
+    g.advance(2, 0)
+    ref = g.get_state().cpu()
+    hin = torch.from_numpy(p.U).pin_memory()
+    hout = torch.empty_like(hin).pin_memory()
+    g.advance_host(hin, hout, 2, 0)
+    assert torch.equal(hout, ref.reshape(hout.shape))
