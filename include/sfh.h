@@ -137,7 +137,7 @@ int sfh_fill_ghosts(sfh_mesh* m, int level, int which, int interp, double tau, v
 int sfh_get_ghosted(sfh_mesh* m, int which, double* d_G, void* stream);
 
 /* Refinement indicators, one double per block in CALLER order to d_out (device,
- * [nblocks]); the caller compares with its threshold and rebuilds the mesh (no regrid inside the library).
+ * [nblocks]); sfh_regrid thresholds them and builds the new mesh.
  *   SFH_REFINE_CURVATURE  eq. (33)-(34): max over the block's interior cells of
  *                         max(E(rho), E(P)), E(q) = |d2x q + d2y q + d2z q| h^2 / q with centred second
  *                         differences (the paper refines where this is >= 1e-2);
@@ -150,15 +150,39 @@ int sfh_get_ghosted(sfh_mesh* m, int which, double* d_G, void* stream);
 #define SFH_REFINE_JEANS 1
 int sfh_refine_indicator(sfh_mesh* m, int which, int criterion, double G, double* d_out, void* stream);
 
-/* Regrid: fills state copy dst_which of the NEW mesh `dst` from copy src_which of the OLD
- * mesh `src` (both bound, same domain): a block present in both is copied; a new block is created from its old
- * parent by the slope-limited conservative prolongation of reading R3 (so restricting the new children gives the
- * parent back); blocks that disappear are dropped (their parents hold the restricted data).  A new block whose
- * parent is not in the old mesh gives SFH_EMESH: refine by one level per regrid.  Only the conserved copies
+/* Regrid, step 1: builds the NEW mesh of a regrid from the
+ * state of `m` (bound).  The refinement indicator of copy `which` (sfh_refine_indicator: criterion, G) is evaluated
+ * on the device and brought to the host, where the library builds the new block list (the lists are
+ * managed on the hosts):
+ *   - every root block;
+ *   - the 8 children of every block of level < max_level that is in `m`, is in the new tree, and whose indicator is
+ *     >= threshold (eq. 33 is written with >=): a regrid deepens the tree by at most one level anywhere and drops
+ *     the children of blocks that are no longer flagged;
+ *   - closed under proper nesting over the 26 neighbours (reading R25): missing blocks are added with their 7
+ *     siblings and, recursively, their ancestors.
+ * *out is a new, UNBOUND mesh with the same configuration and Riemann solver (destroy it with sfh_destroy_mesh); its
+ * caller order is level-major, (bx, by, bz) lexicographic within a level (sfh_block_list).  The caller allocates its
+ * buffers (sfh_state_bytes / sfh_work_bytes), binds it and moves the state with sfh_transfer_state.  Synchronises
+ * `stream`. */
+int sfh_regrid(sfh_mesh* m, int which, int criterion, double G, double threshold, sfh_mesh** out, void* stream);
+
+/* The host half of sfh_regrid: the new mesh from an indicator the caller supplies (host array [nblocks], caller
+ * order; any criterion of the caller's own), same rules.  Needs no GPU and no binding. */
+int sfh_regrid_from_indicator(const sfh_mesh* m, const double* h_indicator, double threshold, sfh_mesh** out);
+
+/* The block list of a mesh in caller order: level[nblocks], ijk[nblocks][3] (host arrays). */
+int sfh_block_list(const sfh_mesh* m, int32_t* level, int32_t* ijk);
+
+/* Regrid, step 2: fills state copy dst_which of the NEW mesh `dst` from copy src_which of the OLD
+ * mesh `src` (both bound, same domain, same number of scalars): a block present in both is copied; a new block is
+ * created from its parent by the slope-limited conservative prolongation of reading R3 (so restricting the new
+ * children gives the parent back) -- from its parent in the old mesh where that exists, else from its parent in the
+ * new mesh, which the same call created one level earlier (any number of new levels); blocks that disappear are
+ * dropped (their parents hold the restricted data).  A new root block gives SFH_EMESH.  Only the conserved copies
  * (0 and 2).  Refills the old mesh's coarse-fine ghost slabs from src_which itself (the prolongation stencils of
  * new blocks next to an old coarse-fine face read them).
- * The caller builds `dst` (sfh_create_mesh from the flags of sfh_refine_indicator, padded to 2:1) and binds it.
- * Synchronous (it uploads a block map and waits for the copy). */
+ * `dst` comes from sfh_regrid or from sfh_create_mesh.  Synchronous (it uploads a block map built on the host
+ * into a table allocated at sfh_bind, and waits for the copy). */
 int sfh_transfer_state(sfh_mesh* src, int src_which, sfh_mesh* dst, int dst_which, void* stream);
 
 /* CFL time step (reading R16): dt = cfl * h_l / max over all cells of level l of

@@ -70,6 +70,9 @@ def load_library(path=None):
         "sfh_cfl_dt": (i32, [vp, i32, C.POINTER(dbl), vp]),
         "sfh_refine_indicator": (i32, [vp, i32, i32, dbl, vp, vp]),
         "sfh_transfer_state": (i32, [vp, i32, vp, i32, vp]),
+        "sfh_regrid": (i32, [vp, i32, i32, dbl, dbl, C.POINTER(vp), vp]),
+        "sfh_regrid_from_indicator": (i32, [vp, vp, dbl, C.POINTER(vp)]),
+        "sfh_block_list": (i32, [vp, vp, vp]),
         "sfh_hydro_step": (i32, [vp, i32, dbl, i32, dbl, dbl, vp]),
         "sfh_flux_correct": (i32, [vp, i32, dbl, vp]),
         "sfh_restrict": (i32, [vp, i32, i32, i32, vp]),
@@ -114,11 +117,8 @@ class Mesh:
     double [nb][5][8][8][8] (interior cells, [block][var][k][j][i])."""
 
     def __init__(self, nb0, max_level, bc, box_len, gamma, cfl, level, ijk, device="cuda:0", bind=True, lib=None,
-                 nscalar=0):
+                 nscalar=0, handle=None):
         self.L = lib or load_library()
-        self.level = np.ascontiguousarray(level, dtype=np.int32)
-        self.ijk = np.ascontiguousarray(ijk, dtype=np.int32).reshape(-1, 3)
-        self.nb = len(self.level)
         cfg = SfhConfig()
         for d in range(3):
             cfg.nb0[d] = int(nb0[d])
@@ -131,9 +131,19 @@ class Mesh:
         self.nv = NV + int(nscalar)          # variables per cell in the caller layout
         self.cfg = cfg
         self.max_level = int(max_level)
-        self.h = C.c_void_p()
-        self._chk(self.L.sfh_create_mesh(C.byref(cfg), self.nb, self.level.ctypes.data, self.ijk.ctypes.data,
-                                         C.byref(self.h)))
+        if handle is None:
+            self.level = np.ascontiguousarray(level, dtype=np.int32)
+            self.ijk = np.ascontiguousarray(ijk, dtype=np.int32).reshape(-1, 3)
+            self.nb = len(self.level)
+            self.h = C.c_void_p()
+            self._chk(self.L.sfh_create_mesh(C.byref(cfg), self.nb, self.level.ctypes.data, self.ijk.ctypes.data,
+                                             C.byref(self.h)))
+        else:                                # a mesh the library built itself (sfh_regrid): read its block list back
+            self.h = handle
+            self.nb = int(self.L.sfh_num_blocks(self.h))
+            self.level = np.zeros(self.nb, dtype=np.int32)
+            self.ijk = np.zeros((self.nb, 3), dtype=np.int32)
+            self._chk(self.L.sfh_block_list(self.h, self.level.ctypes.data, self.ijk.ctypes.data))
         self.t = C.c_double(0.0)
         self.nupd = np.zeros(self.max_level + 1, dtype=np.int64)
         self.device = device
@@ -282,9 +292,29 @@ class Mesh:
         the old mesh's ghosts of `which` first."""
         self._chk(self.L.sfh_transfer_state(src.h, which, self.h, which, _stream()))
 
+    def regrid_from_indicator(self, indicator, threshold, bind=False):
+        """The new mesh from a host indicator array (caller order); host only unless bind=True."""
+        ind = np.ascontiguousarray(indicator, dtype=np.float64)
+        assert ind.shape == (self.nb,)
+        h = C.c_void_p()
+        self._chk(self.L.sfh_regrid_from_indicator(self.h, ind.ctypes.data, float(threshold), C.byref(h)))
+        c = self.cfg
+        return Mesh(tuple(c.nb0), c.max_level, [tuple(b) for b in c.bc], tuple(c.box_len), c.gamma, c.cfl, None, None,
+                    device=self.device, lib=self.L, nscalar=c.nscalar, handle=h, bind=bind)
+
+    def regrid(self, criterion, threshold, which=0, G=1.0):
+        """The regridded mesh (sfh_regrid: blocks with indicator >= threshold get children, 2:1 closure), bound to new
+        buffers, holding the state of copy `which` moved onto it (sfh_transfer_state)."""
+        h = C.c_void_p()
+        self._chk(self.L.sfh_regrid(self.h, which, criterion, float(G), float(threshold), C.byref(h), _stream()))
+        c = self.cfg
+        new = Mesh(tuple(c.nb0), c.max_level, [tuple(b) for b in c.bc], tuple(c.box_len), c.gamma, c.cfl, None, None,
+                   device=self.device, lib=self.L, nscalar=c.nscalar, handle=h)
+        new.transfer_from(self, which)
+        return new
+
     def refine_indicator(self, criterion=0, which=0, G=1.0):
-        """Per-block refinement indicator (0: eq. 33-34 curvature, 1: h / Jeans length), caller order; fill the
-        ghosts of `which` first on refined meshes."""
+        """Per-block refinement indicator (0: eq. 33-34 curvature, 1: h / Jeans length), caller order."""
         import torch
         out = torch.empty(self.nb, dtype=torch.float64, device=self.device)
         self._chk(self.L.sfh_refine_indicator(self.h, which, criterion, float(G), out.data_ptr(), _stream()))

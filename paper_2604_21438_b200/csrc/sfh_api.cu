@@ -27,6 +27,8 @@ struct sfh_mesh {
           *d_coord = nullptr, *d_cf_block = nullptr, *d_cf_face = nullptr, *d_fh_src = nullptr,
           *d_restrict_list = nullptr, *d_reflux_list = nullptr;
   int64_t* d_perm = nullptr;
+  int32_t* d_tsrc = nullptr;            // regrid: per block of THIS (new) mesh, where its data come from (sfh_transfer_state)
+  double* d_ind = nullptr;              // regrid: refinement indicator per block, library order scratch (sfh_regrid)
   double* state[3] = {nullptr, nullptr, nullptr};
   double *ghost = nullptr, *ghost1 = nullptr, *R = nullptr, *FH = nullptr;   // ghost: slabs of U^n, ghost1: of U^{n+1/2}
   // passive scalars (ns = cfg.nscalar > 0): slabs of q^n / q^{n+1/2}, flux registers, the stage kernels' mass fluxes
@@ -524,6 +526,8 @@ int sfh_bind(sfh_mesh* m, void* d_state0, void* d_state1, void* d_state2, void* 
         {hm.restrict_list.data(), hm.restrict_list.size() * 4, (void**)&m->d_restrict_list},
         {hm.reflux_list.data(), hm.reflux_list.size() * 4, (void**)&m->d_reflux_list},
         {hm.perm.data(), hm.perm.size() * 8, (void**)&m->d_perm},
+        {nullptr, size_t(hm.nb) * 4, (void**)&m->d_tsrc},
+        {nullptr, size_t(hm.nb) * 8, (void**)&m->d_ind},
     };
     size_t total = 0;
     for (const Item& it : items) total += up(it.bytes + 1);
@@ -532,7 +536,7 @@ int sfh_bind(sfh_mesh* m, void* d_state0, void* d_state1, void* d_state2, void* 
     size_t off = 0;
     for (const Item& it : items) {
       *it.dst = m->dev_tables + off;
-      if (it.bytes) e = cudaMemcpy(m->dev_tables + off, it.src, it.bytes, cudaMemcpyHostToDevice);
+      if (it.bytes && it.src) e = cudaMemcpy(m->dev_tables + off, it.src, it.bytes, cudaMemcpyHostToDevice);
       if (e != cudaSuccess) break;
       off += up(it.bytes + 1);
     }
@@ -659,7 +663,11 @@ int sfh_transfer_state(sfh_mesh* src, int src_which, sfh_mesh* dst, int dst_whic
     return (uint64_t(l) << 60) | (uint64_t(uint32_t(c[0]) & 0xFFFFF) << 40) | (uint64_t(uint32_t(c[1]) & 0xFFFFF) << 20) |
            uint64_t(uint32_t(c[2]) & 0xFFFFF);
   };
+  // tsrc[b] of new block b: >= 0 copy of old slot; <= -2 prolongation from OLD parent slot -2 - tsrc; -1 prolongation
+  // from its parent in the NEW mesh (a block more than one level below anything the old mesh holds there: the parent
+  // was itself created by this transfer, one level earlier)
   std::vector<int32_t> tsrc;
+  std::vector<char> from_new(size_t(hd.nlev), 0);
   try {
     std::unordered_map<uint64_t, int32_t> old;
     old.reserve(size_t(hs.nb) * 2);
@@ -671,10 +679,10 @@ int sfh_transfer_state(sfh_mesh* src, int src_which, sfh_mesh* dst, int dst_whic
       if (it != old.end()) { tsrc[b] = it->second; continue; }
       const int32_t pc[3] = {hd.coord[3 * b] >> 1, hd.coord[3 * b + 1] >> 1, hd.coord[3 * b + 2] >> 1};
       it = l > 0 ? old.find(key(l - 1, pc)) : old.end();
-      if (it == old.end())
-        return fail(SFH_EMESH, "a block of the new mesh has neither itself nor its parent in the old mesh "
-                               "(refine by one level per regrid)");
-      tsrc[b] = -2 - it->second;
+      if (it != old.end()) { tsrc[b] = -2 - it->second; continue; }
+      if (l == 0) return fail(SFH_EMESH, "a root block of the new mesh is not in the old mesh");
+      tsrc[b] = -1;
+      from_new[size_t(l)] = 1;
     }
   } catch (const std::bad_alloc&) {
     return fail(SFH_ENOMEM, "out of host memory");
@@ -683,29 +691,77 @@ int sfh_transfer_state(sfh_mesh* src, int src_which, sfh_mesh* dst, int dst_whic
   // the prolongation stencils read the old mesh's coarse-fine slabs: refill them from src_which
   for (int l = 1; l < hs.nlev; ++l)
     if ((rc = fill_level(src, l, src_which, 0, 0.0, st))) return rc;
-  int32_t* d_tsrc = nullptr;
-  if (cudaMalloc((void**)&d_tsrc, tsrc.size() * 4) != cudaSuccess) return fail(SFH_ENOMEM, "cudaMalloc of the transfer table failed");
-  cudaError_t e = cudaMemcpyAsync(d_tsrc, tsrc.data(), tsrc.size() * 4, cudaMemcpyHostToDevice, st);
-  // a new block of level l reads old level l (copy) or old level l-1 (prolongation); the roles rotate per level,
-  // so the two may sit in different physical buffers
-  for (int l = 0; l < hd.nlev && e == cudaSuccess; ++l) {
+  CU(cudaMemcpyAsync(dst->d_tsrc, tsrc.data(), tsrc.size() * 4, cudaMemcpyHostToDevice, st), "upload of the transfer table");
+  // a new block of level l reads old level l (copy), old level l-1 (prolongation) or new level l-1; the roles rotate
+  // per level, so these may sit in different physical buffers
+  for (int l = 0; l < hd.nlev; ++l) {
     const int lc = l < hs.nlev ? l : hs.nlev - 1, lp = l > 0 ? (l - 1 < hs.nlev ? l - 1 : hs.nlev - 1) : 0;
     const int64_t first = hd.lev_first[l], count = hd.lev_count[l];
-    e = launch_transfer(role_buf(src, lc, src_which), role_buf(src, lp, src_which), src->ghost, src->d_face_src,
-                        d_tsrc + first, dst->d_coord + 3 * first, role_buf(dst, l, dst_which) + size_t(first) * BLK,
-                        int(count), st);
-    if (e == cudaSuccess)
-      e = launch_transfer_scalar(role_q(src, lc, src_which), role_q(src, lp, src_which), src->ghostS, src->d_face_src,
-                                 d_tsrc + first, dst->d_coord + 3 * first,
-                                 role_q(dst, l, dst_which) + size_t(first) * dst->ns * NC, int(count), dst->ns, st);
+    if (from_new[size_t(l)] && (rc = fill_level(dst, l - 1, dst_which, 0, 0.0, st))) return rc;   // slabs of the new parents
+    TransferParams tp;
+    tp.Uc = role_buf(src, lc, src_which); tp.Us = role_buf(src, lp, src_which); tp.ghost_s = src->ghost;
+    tp.face_src_s = src->d_face_src;
+    tp.Un = l > 0 ? role_buf(dst, l - 1, dst_which) : nullptr; tp.ghost_n = dst->ghost; tp.face_src_n = dst->d_face_src;
+    tp.parent_n = dst->d_parent + first;
+    tp.tsrc = dst->d_tsrc + first; tp.coord_d = dst->d_coord + 3 * first;
+    tp.Ud = role_buf(dst, l, dst_which) + size_t(first) * BLK;
+    CU(launch_transfer(tp, int(count), st), "transfer_kernel");
+    if (dst->ns > 0) {
+      tp.Uc = role_q(src, lc, src_which); tp.Us = role_q(src, lp, src_which); tp.ghost_s = src->ghostS;
+      tp.Un = l > 0 ? role_q(dst, l - 1, dst_which) : nullptr; tp.ghost_n = dst->ghostS;
+      tp.Ud = role_q(dst, l, dst_which) + size_t(first) * dst->ns * NC;
+      CU(launch_transfer_scalar(tp, int(count), dst->ns, st), "transfer_scalar_kernel");
+    }
     dst->launches += (count > 0) * (1 + (dst->ns > 0));
   }
-  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-  cudaFree(d_tsrc);
-  if (e != cudaSuccess) return cuda_fail(e, "transfer_kernel");
+  CU(cudaStreamSynchronize(st), "cudaStreamSynchronize");      // tsrc (host vector) must outlive the upload
   for (int l = 0; l < hd.nlev; ++l) {
     if (dst_which == 0) dst->bmax_valid[l] = false;
     else dst->bmax_pending[l] = false;
+  }
+  return SFH_OK;
+}
+
+int sfh_regrid(sfh_mesh* m, int which, int criterion, double G, double threshold, sfh_mesh** out, void* stream) {
+  if (!out) return fail(SFH_EINVAL, "null argument");
+  *out = nullptr;
+  int rc = check_bound(m);
+  if (rc) return rc;
+  const HostMesh& hm = m->hm;
+  std::vector<double> ind(size_t(hm.nb));
+  if ((rc = sfh_refine_indicator(m, which, criterion, G, m->d_ind, stream))) return rc;       // caller order
+  CU(cudaMemcpyAsync(ind.data(), m->d_ind, ind.size() * 8, cudaMemcpyDeviceToHost, S(stream)), "download of the indicator");
+  CU(cudaStreamSynchronize(S(stream)), "cudaStreamSynchronize");
+  return sfh_regrid_from_indicator(m, ind.data(), threshold, out);
+}
+
+int sfh_regrid_from_indicator(const sfh_mesh* m, const double* h_indicator, double threshold, sfh_mesh** out) {
+  if (!m || !h_indicator || !out) return fail(SFH_EINVAL, "null argument");
+  *out = nullptr;
+  const HostMesh& hm = m->hm;
+  std::vector<int32_t> level, ijk;
+  int rc;
+  try {
+    std::vector<double> ind_slot(size_t(hm.nb));      // caller order -> library order
+    for (int64_t s = 0; s < hm.nb; ++s) ind_slot[size_t(s)] = h_indicator[size_t(hm.perm[size_t(s)])];
+    if ((rc = regrid_block_list(hm, ind_slot.data(), threshold, level, ijk))) return rc;
+  } catch (const std::bad_alloc&) {
+    return fail(SFH_ENOMEM, "out of host memory");
+  }
+  sfh_mesh* nm = nullptr;
+  if ((rc = sfh_create_mesh(&hm.cfg, int64_t(level.size()), level.data(), ijk.data(), &nm))) return rc;
+  nm->riemann = m->riemann;
+  *out = nm;
+  return SFH_OK;
+}
+
+int sfh_block_list(const sfh_mesh* m, int32_t* level, int32_t* ijk) {
+  if (!m || !level || !ijk) return fail(SFH_EINVAL, "null argument");
+  const HostMesh& hm = m->hm;
+  for (int64_t s = 0; s < hm.nb; ++s) {
+    const int64_t b = hm.perm[size_t(s)];
+    level[b] = hm.lev[size_t(s)];
+    for (int d = 0; d < 3; ++d) ijk[3 * b + d] = hm.coord[size_t(3 * s + d)];
   }
   return SFH_OK;
 }

@@ -59,6 +59,10 @@ struct HostMesh {
 int build_host_mesh(const sfh_config& cfg, int64_t nblocks, const int32_t* level, const int32_t* ijk,
                     HostMesh& out, std::string& err);
 
+// Block list (caller order: level-major, lexicographic within a level) of the regridded tree: sfh_mesh.cpp.
+int regrid_block_list(const HostMesh& old, const double* ind, double threshold, std::vector<int32_t>& level,
+                      std::vector<int32_t>& ijk);
+
 void set_error(const std::string& s);
 
 }  // namespace sfh

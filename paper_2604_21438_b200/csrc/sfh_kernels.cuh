@@ -102,10 +102,23 @@ cudaError_t launch_ghosted(const double* U, const double* ghost, const int32_t* 
 cudaError_t launch_refine_indicator(const double* U, const double* ghost, const int32_t* face_src, const int64_t* perm,
                                     int first, int count, int prim, double gamma, int criterion, double G, double h,
                                     double* out, cudaStream_t st);
-// regrid: block d of the new mesh <- old slot tsrc[d] (copy) or prolongation from old parent -2 - tsrc[d]
-// Uc / Us: the old buffers holding the block's own level (copies) and its parent level (prolongation)
-cudaError_t launch_transfer(const double* Uc, const double* Us, const double* ghost_s, const int32_t* face_src_s,
-                            const int32_t* tsrc, const int32_t* coord_d, double* Ud, int count, cudaStream_t st);
+// regrid: block d of the new mesh <- old slot tsrc[d] >= 0 (copy), prolongation from OLD parent -2 - tsrc[d]
+// (tsrc[d] <= -2), or prolongation from its parent in the NEW mesh (tsrc[d] == -1; that parent was filled one level
+// earlier by the same transfer).  The arrays are the hydro parts [.][5][512] or the scalar parts [.][ns][512].
+struct TransferParams {
+  const double* Uc;            // old buffer holding the block's own level (copies)
+  const double* Us;            // old buffer holding the parent level
+  const double* ghost_s;       // old mesh: coarse-fine slabs of that copy
+  const int32_t* face_src_s;
+  const double* Un;            // new buffer holding the parent level (or null at level 0)
+  const double* ghost_n;       // new mesh: coarse-fine slabs
+  const int32_t* face_src_n;
+  const int32_t* parent_n;     // new mesh: parent slot per block of this launch
+  const int32_t* tsrc;         // per block of this launch
+  const int32_t* coord_d;
+  double* Ud;                  // destination blocks of this launch
+};
+cudaError_t launch_transfer(const TransferParams& p, int count, cudaStream_t st);
 cudaError_t configure_kernels(int* sm_count);
 
 // ---- passive scalars (sfh_kernels_scalar.cu): Q[nb][ns][512] behind the hydro part of every state buffer ----------
@@ -142,9 +155,7 @@ cudaError_t launch_reflux_scalar(double* Q, const double* RS, const double* FHS,
                                  const double* dt_dev, cudaStream_t st);
 cudaError_t launch_permute_scalar(const double* src, double* dst, const int64_t* perm, int first, int count, int ns,
                                   int to_internal, cudaStream_t st);
-cudaError_t launch_transfer_scalar(const double* Qc, const double* Qs, const double* ghost_s, const int32_t* face_src_s,
-                                   const int32_t* tsrc, const int32_t* coord_d, double* Qd, int count, int ns,
-                                   cudaStream_t st);
+cudaError_t launch_transfer_scalar(const TransferParams& p, int count, int ns, cudaStream_t st);
 // fp64 issue-rate microbenchmark: `ctas` CTAs of 1024 threads, each thread `iters` x 16 x `chains` DFMAs
 cudaError_t launch_dfma_rate(int chains, int ctas, int iters, double* sink, cudaStream_t st);
 

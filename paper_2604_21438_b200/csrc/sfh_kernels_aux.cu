@@ -551,25 +551,27 @@ cudaError_t launch_refine_indicator(const double* U, const double* ghost, const 
 // the new mesh.  tsrc[d] >= 0: the block exists in the old mesh, slot tsrc[d]: copy.  tsrc[d] <= -2: it is
 // new; its parent is old slot -2 - tsrc[d]: every fine cell is the slope-limited conservative prolongation
 // (reading R3) of the parent's cell and its six neighbours, which lie in the parent, in its same-level
-// neighbour, behind an outflow face (zero gradient) or in the old mesh's prolonged ghost slab.
+// neighbour, behind an outflow face (zero gradient) or in the old mesh's prolonged ghost slab.  tsrc[d] == -1:
+// the parent is new as well (created one level earlier by the same transfer): the same prolongation from the
+// NEW mesh's buffers, so a regrid may deepen the tree by any number of levels.
 // =====================================================================================================
-// Uc: the old buffer that holds the block's own level (copies), Us: the one that holds the parent level.
-__global__ void __launch_bounds__(256) transfer_kernel(const double* __restrict__ Uc, const double* __restrict__ Us,
-                                                       const double* __restrict__ ghost_s,
-                                                       const int32_t* __restrict__ face_src_s,
-                                                       const int32_t* __restrict__ tsrc,
-                                                       const int32_t* __restrict__ coord_d, double* __restrict__ Ud) {
+__global__ void __launch_bounds__(256) transfer_kernel(const TransferParams p) {
   const int d = blockIdx.x;
-  const int t = tsrc[d];
-  double* out = Ud + size_t(d) * BLK;
+  const int t = p.tsrc[d];
+  double* out = p.Ud + size_t(d) * BLK;
   if (t >= 0) {
-    const double2* from = reinterpret_cast<const double2*>(Uc + size_t(t) * BLK);
+    const double2* from = reinterpret_cast<const double2*>(p.Uc + size_t(t) * BLK);
     double2* to = reinterpret_cast<double2*>(out);
     for (int q = threadIdx.x; q < BLK / 2; q += 256) to[q] = from[q];
     return;
   }
-  const int P = -2 - t;
-  const int oct[3] = {coord_d[3 * d] & 1, coord_d[3 * d + 1] & 1, coord_d[3 * d + 2] & 1};
+  // the parent: in the old mesh (t <= -2) or in the new one (t == -1)
+  const bool in_new = t == -1;
+  const int P = in_new ? p.parent_n[d] : -2 - t;
+  const double* Us = in_new ? p.Un : p.Us;
+  const double* ghost = in_new ? p.ghost_n : p.ghost_s;
+  const int32_t* face_src = in_new ? p.face_src_n : p.face_src_s;
+  const int oct[3] = {p.coord_d[3 * d] & 1, p.coord_d[3 * d + 1] & 1, p.coord_d[3 * d + 2] & 1};
   const double* Up = Us + size_t(P) * BLK;
   auto fetch = [&](int c0, int c1, int c2, double q[NV]) {       // coarse cell of the parent's neighbourhood
     int c[3] = {c0, c1, c2};
@@ -579,7 +581,7 @@ __global__ void __launch_bounds__(256) transfer_kernel(const double* __restrict_
     if (axis < 0) from = Up + (c[2] * 8 + c[1]) * 8 + c[0];
     else {
       const int side = c[axis] >= N;
-      const int src = face_src_s[P * 6 + 2 * axis + side];
+      const int src = face_src[P * 6 + 2 * axis + side];
       if (src == SRC_OUTFLOW) {
         c[axis] = side ? N - 1 : 0;
         from = Up + (c[2] * 8 + c[1]) * 8 + c[0];
@@ -587,7 +589,7 @@ __global__ void __launch_bounds__(256) transfer_kernel(const double* __restrict_
         c[axis] += side ? -N : N;
         from = Us + size_t(src) * BLK + (c[2] * 8 + c[1]) * 8 + c[0];
       } else {
-        from = ghost_s + size_t(-2 - src) * SLAB +
+        from = ghost + size_t(-2 - src) * SLAB +
                slab_pos(axis, side ? 0 : NG - 1, axis == 0 ? c[1] : c[0], axis == 2 ? c[1] : c[2]);
         vs = NG * FACE;
       }
@@ -615,10 +617,9 @@ __global__ void __launch_bounds__(256) transfer_kernel(const double* __restrict_
   }
 }
 
-cudaError_t launch_transfer(const double* Uc, const double* Us, const double* ghost_s, const int32_t* face_src_s,
-                            const int32_t* tsrc, const int32_t* coord_d, double* Ud, int count, cudaStream_t st) {
+cudaError_t launch_transfer(const TransferParams& p, int count, cudaStream_t st) {
   if (count <= 0) return cudaSuccess;
-  transfer_kernel<<<count, 256, 0, st>>>(Uc, Us, ghost_s, face_src_s, tsrc, coord_d, Ud);
+  transfer_kernel<<<count, 256, 0, st>>>(p);
   return cudaGetLastError();
 }
 

@@ -309,31 +309,29 @@ cudaError_t launch_permute_scalar(const double* src, double* dst, const int64_t*
 // =====================================================================================================
 // Regrid: scalars of a new mesh from an old one (transfer_kernel of sfh_kernels_aux.cu on Q and the scalar slabs)
 // =====================================================================================================
-__global__ void __launch_bounds__(256) transfer_scalar_kernel(const double* __restrict__ Qc, const double* __restrict__ Qs,
-                                                              const double* __restrict__ ghost_s,
-                                                              const int32_t* __restrict__ face_src_s,
-                                                              const int32_t* __restrict__ tsrc,
-                                                              const int32_t* __restrict__ coord_d, double* __restrict__ Qd,
-                                                              int ns) {
+__global__ void __launch_bounds__(256) transfer_scalar_kernel(const TransferParams p, int ns) {
   const int d = blockIdx.x;
-  const int t = tsrc[d];
-  double* out = Qd + size_t(d) * ns * NC;
+  const int t = p.tsrc[d];
+  double* out = p.Ud + size_t(d) * ns * NC;
   if (t >= 0) {
-    const double2* from = reinterpret_cast<const double2*>(Qc + size_t(t) * ns * NC);
+    const double2* from = reinterpret_cast<const double2*>(p.Uc + size_t(t) * ns * NC);
     double2* to = reinterpret_cast<double2*>(out);
     for (int q = threadIdx.x; q < ns * NC / 2; q += 256) to[q] = from[q];
     return;
   }
-  const int P = -2 - t;
-  const int oct[3] = {coord_d[3 * d] & 1, coord_d[3 * d + 1] & 1, coord_d[3 * d + 2] & 1};
+  const bool in_new = t == -1;
+  const int P = in_new ? p.parent_n[d] : -2 - t;
+  const double* Qs = in_new ? p.Un : p.Us;
+  const double* ghost = in_new ? p.ghost_n : p.ghost_s;
+  const int32_t* face_src = in_new ? p.face_src_n : p.face_src_s;
+  const int oct[3] = {p.coord_d[3 * d] & 1, p.coord_d[3 * d + 1] & 1, p.coord_d[3 * d + 2] & 1};
   for (int v = 0; v < ns; ++v)
     for (int cell = threadIdx.x; cell < NC; cell += 256) {
       const int f[3] = {cell & 7, (cell >> 3) & 7, cell >> 6};
       const int c[3] = {oct[0] * 4 + (f[0] >> 1), oct[1] * 4 + (f[1] >> 1), oct[2] * 4 + (f[2] >> 1)};
-      auto fetch = [&](int c0, int c1, int c2) {
+      auto fetch = [&](int c0, int c1, int c2) {       // one ghost layer is reached at most: the slab layer next to the face
         int vs;
-        const double* from = ghost_src(Qs, ns, ghost_s, ns, face_src_s, P, c0, c1, c2, &vs);
-        // one ghost layer only: layer index next to the face (ghost_src addresses layer c - N / c + NG of the slab)
+        const double* from = ghost_src(Qs, ns, ghost, ns, face_src, P, c0, c1, c2, &vs);
         return from[v * vs];
       };
       const double Q = fetch(c[0], c[1], c[2]);
@@ -349,11 +347,9 @@ __global__ void __launch_bounds__(256) transfer_scalar_kernel(const double* __re
     }
 }
 
-cudaError_t launch_transfer_scalar(const double* Qc, const double* Qs, const double* ghost_s, const int32_t* face_src_s,
-                                   const int32_t* tsrc, const int32_t* coord_d, double* Qd, int count, int ns,
-                                   cudaStream_t st) {
+cudaError_t launch_transfer_scalar(const TransferParams& p, int count, int ns, cudaStream_t st) {
   if (count <= 0 || ns <= 0) return cudaSuccess;
-  transfer_scalar_kernel<<<count, 256, 0, st>>>(Qc, Qs, ghost_s, face_src_s, tsrc, coord_d, Qd, ns);
+  transfer_scalar_kernel<<<count, 256, 0, st>>>(p, ns);
   return cudaGetLastError();
 }
 

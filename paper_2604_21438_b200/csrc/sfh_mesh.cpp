@@ -222,4 +222,76 @@ int build_host_mesh(const sfh_config& cfg, int64_t nblocks, const int32_t* level
   return SFH_OK;
 }
 
+// ---- regrid: the block list of the new tree (reading R31) ----------------
+// ind[slot]: refinement indicator of every block of the old mesh (library order).  New tree: all root blocks; the
+// octet under every old block of level < max_level that is still in the new tree and has ind >= threshold (eq. 33 is
+// written with >=); then the closure under proper nesting over the 26 neighbours (reading R25), adding whole octets
+// and their ancestors.  Output: level-major, (bx, by, bz) lexicographic within a level.
+int regrid_block_list(const HostMesh& old, const double* ind, double threshold, std::vector<int32_t>& level,
+                      std::vector<int32_t>& ijk) {
+  const sfh_config& cfg = old.cfg;
+  const int nlev = old.nlev;
+  std::vector<std::unordered_map<uint64_t, char>> have(nlev);     // per level: key -> present
+  std::vector<std::vector<int32_t>> list(nlev);                   // per level: coordinates, 3 per block
+  auto add = [&](int l, int x, int y, int z) {
+    if (have[l].emplace(hkey(l, x, y, z), 1).second) { list[l].push_back(x); list[l].push_back(y); list[l].push_back(z); return true; }
+    return false;
+  };
+  auto add_octet = [&](int l, int px, int py, int pz) {           // children of (px,py,pz) of level l-1
+    bool any = false;
+    for (int q = 0; q < 8; ++q) any |= add(l, 2 * px + (q & 1), 2 * py + ((q >> 1) & 1), 2 * pz + ((q >> 2) & 1));
+    return any;
+  };
+  for (int64_t s = 0; s < old.nb && old.lev[s] == 0; ++s) add(0, old.coord[3 * s], old.coord[3 * s + 1], old.coord[3 * s + 2]);
+  for (int64_t s = 0; s < old.nb; ++s) {                          // slots are level-major: parents come first
+    const int l = old.lev[s];
+    if (l + 1 >= nlev || !(ind[s] >= threshold)) continue;
+    const int x = old.coord[3 * s], y = old.coord[3 * s + 1], z = old.coord[3 * s + 2];
+    if (have[l].count(hkey(l, x, y, z))) add_octet(l + 1, x, y, z);
+  }
+  // closure: a work list of blocks whose 26 neighbour positions still have to be checked
+  struct Item { int l, x, y, z; };
+  std::vector<Item> work;
+  for (int l = 2; l < nlev; ++l)
+    for (size_t q = 0; q + 2 < list[l].size(); q += 3) work.push_back({l, list[l][q], list[l][q + 1], list[l][q + 2]});
+  // make block (x,y,z) of level l exist: its octet, after the parent's; new blocks of level >= 2 join the work list
+  auto ensure = [&](auto&& self, int l, int x, int y, int z) -> void {
+    if (l == 0 || have[l].count(hkey(l, x, y, z))) return;
+    self(self, l - 1, x >> 1, y >> 1, z >> 1);
+    const size_t before = list[l].size();
+    add_octet(l, x >> 1, y >> 1, z >> 1);
+    if (l >= 2)
+      for (size_t q = before; q + 2 < list[l].size(); q += 3) work.push_back({l, list[l][q], list[l][q + 1], list[l][q + 2]});
+  };
+  while (!work.empty()) {
+    const Item it = work.back();
+    work.pop_back();
+    for (int dz = -1; dz <= 1; ++dz) for (int dy = -1; dy <= 1; ++dy) for (int dx = -1; dx <= 1; ++dx) {
+      int c[3] = {it.x + dx, it.y + dy, it.z + dz};
+      bool outside = false;
+      for (int d = 0; d < 3; ++d) {
+        const int n = cfg.nb0[d] << it.l;
+        if (c[d] < 0) { if (cfg.bc[d][0] != 0) outside = true; else c[d] += n; }
+        else if (c[d] >= n) { if (cfg.bc[d][1] != 0) outside = true; else c[d] -= n; }
+      }
+      if (!outside) ensure(ensure, it.l - 1, c[0] >> 1, c[1] >> 1, c[2] >> 1);
+    }
+  }
+  level.clear();
+  ijk.clear();
+  for (int l = 0; l < nlev; ++l) {
+    const size_t n = list[l].size() / 3;
+    std::vector<size_t> order(n);
+    std::iota(order.begin(), order.end(), size_t(0));
+    const std::vector<int32_t>& c = list[l];
+    std::sort(order.begin(), order.end(), [&](size_t a, size_t b) {
+      if (c[3 * a] != c[3 * b]) return c[3 * a] < c[3 * b];
+      if (c[3 * a + 1] != c[3 * b + 1]) return c[3 * a + 1] < c[3 * b + 1];
+      return c[3 * a + 2] < c[3 * b + 2];
+    });
+    for (size_t q : order) { level.push_back(l); ijk.push_back(c[3 * q]); ijk.push_back(c[3 * q + 1]); ijk.push_back(c[3 * q + 2]); }
+  }
+  return SFH_OK;
+}
+
 }  // namespace sfh

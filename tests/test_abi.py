@@ -117,3 +117,28 @@ def test_compute_calls_fail_loudly_without_binding():
     if not torch.cuda.is_available():
         with pytest.raises(sfh.SfhError):
             m.bind()
+
+
+def test_regrid_block_list_host_logic_matches_the_stated_rules():
+    """sfh_regrid_from_indicator (host only): the same block list as the dense-array construction of
+    sfh_inputs.Tree (children of flagged blocks present in the new tree, 2:1 closure), in the documented order."""
+    from sfh_inputs import Tree
+    rng = np.random.default_rng(5)
+    for periodic, offset in (((True, True, True), (0, 0, 0)), ((False, True, False), (-1, 0, 1))):
+        t = small_amr_tree(periodic=periodic, offset=offset)
+        bc = tuple((0, 0) if per else (1, 1) for per in periodic)
+        m, level, ijk = _mesh(t, bc=bc)
+        for thr in (0.15, 0.5, 0.85):
+            ind = rng.random(len(level))
+            new = m.regrid_from_indicator(ind, thr)
+            ref = Tree(t.nb0, t.max_level, periodic)
+            for l in range(t.max_level):
+                f = np.zeros_like(ref.exists[l])
+                sel = (level == l) & (ind >= thr)
+                f[ijk[sel, 0], ijk[sel, 1], ijk[sel, 2]] = True
+                ref.refine(l, f)
+            lev, ij = ref.pad_2to1().block_list()
+            assert np.array_equal(new.level, lev) and np.array_equal(new.ijk, ij)
+            assert new.cfg.nscalar == m.cfg.nscalar and new.max_level == m.max_level
+    with pytest.raises(sfh.SfhError):       # null indicator: a defined error
+        m._chk(m.L.sfh_regrid_from_indicator(m.h, None, 0.5, C.byref(C.c_void_p())))

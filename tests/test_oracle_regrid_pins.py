@@ -111,3 +111,87 @@ def test_coarsening_keeps_the_restricted_parents_and_two_levels_are_created_at_o
     scale = np.abs(d2).max(axis=(0, 2, 3, 4))[None, :, None, None, None]
     assert (np.abs(d.get_state() - d2) <= 6e-16 * scale).all()
     assert np.array_equal(d2[p.level == 0], c.get_state())
+
+
+# ------------------------------------------------------------------ the regrid's block list (orc_regrid)
+def tree_from_flags(p, flagged, periodic):
+    """The same rules with an unrelated implementation (dense boolean arrays and dilation, sfh_inputs.Tree): children
+    of flagged blocks that exist in the new tree, then the 2:1 closure."""
+    t = Tree(p.nb0, p.max_level, periodic)
+    for l in range(p.max_level):
+        f = np.zeros_like(t.exists[l])
+        sel = (p.level == l) & flagged
+        f[p.ijk[sel, 0], p.ijk[sel, 1], p.ijk[sel, 2]] = True
+        t.refine(l, f)
+    return t.pad_2to1().block_list()
+
+
+def properly_nested(level, ijk, nb0, periodic, max_level):
+    have = [set() for _ in range(max_level + 1)]
+    for l, c in zip(level, ijk):
+        have[l].add(tuple(int(x) for x in c))
+    for l in range(1, max_level + 1):
+        for c in have[l]:
+            if (c[0] >> 1, c[1] >> 1, c[2] >> 1) not in have[l - 1]:
+                return False
+            if l >= 2:
+                for d in np.ndindex(3, 3, 3):
+                    pos, ok = [], True
+                    for a in range(3):
+                        x, n = c[a] + d[a] - 1, nb0[a] << l
+                        if x < 0 or x >= n:
+                            if not periodic[a]:
+                                ok = False
+                            x %= n
+                        pos.append(x >> 1)
+                    if ok and tuple(pos) not in have[l - 1]:
+                        return False
+    return True
+
+
+import pytest
+
+
+@pytest.mark.parametrize("periodic,offset", [((True, True, True), (0, 0, 0)), ((False, True, False), (-1, 0, 1))])
+@pytest.mark.parametrize("quantile", [0.2, 0.6, 0.9])
+def test_regrid_block_list_follows_the_stated_rules(periodic, offset, quantile):
+    p = problem_from_tree(small_amr_tree(periodic=periodic, offset=offset), mode=1)
+    m = consistent(p)
+    m.advance(1, 1)
+    m.fill_ghosts(-1, 0, 0, 0.0)
+    ind = m.refine_indicator(0)
+    thr = float(np.sort(ind)[int(quantile * len(ind))])
+    new = m.regrid(0, thr)
+    lev, ijk = tree_from_flags(p, ind >= thr, periodic)
+    assert np.array_equal(new.level, lev) and np.array_equal(new.ijk, ijk)
+    assert properly_nested(new.level, new.ijk, p.nb0, periodic, p.max_level)
+    # flagged blocks that survive have their 8 children; the tree is at most one level deeper than the old one anywhere
+    old = {(int(l), *map(int, c)) for l, c in zip(p.level, p.ijk)}
+    newset = {(int(l), *map(int, c)) for l, c in zip(new.level, new.ijk)}
+    for b in np.nonzero((ind >= thr) & (p.level < p.max_level))[0]:
+        k = (int(p.level[b]), *map(int, p.ijk[b]))
+        if k in newset:
+            assert (k[0] + 1, 2 * k[1], 2 * k[2], 2 * k[3]) in newset
+    for (l, x, y, z) in newset:
+        assert l == 0 or (l, x, y, z) in old or (l - 1, x >> 1, y >> 1, z >> 1) in old
+    # and the state moved with it: blocks kept are copies, the hierarchy is restriction-consistent
+    U0, U1 = m.get_state(), new.get_state()
+    where = {(int(l), *map(int, c)): n for n, (l, c) in enumerate(zip(p.level, p.ijk))}
+    for n, (l, c) in enumerate(zip(new.level, new.ijk)):
+        k = (int(l), *map(int, c))
+        if k in where:
+            assert np.array_equal(U1[n], U0[where[k]])
+    new.restrict_all(0)
+    scale = np.abs(U1).max(axis=(0, 2, 3, 4))[None, :, None, None, None]
+    assert (np.abs(new.get_state() - U1) <= 6e-16 * scale).all()
+
+
+def test_regrid_with_nothing_flagged_returns_the_root_grid_and_everything_flagged_deepens_by_one_level():
+    p = problem_from_tree(small_amr_tree(max_level=1), mode=1)
+    p.max_level = 3
+    m = consistent(p)
+    m.fill_ghosts(-1, 0, 0, 0.0)
+    none = m.regrid(0, 1e300)
+    assert (none.level == 0).all() and len(none.level) == 64
+    full = m.regrid(0, -1.0)
+    assert [int((full.level == l).sum()) for l in range(4)] == [64, 512, 512, 0]       # level 2 under the old level-1 patch only
