@@ -4,11 +4,17 @@
     ncu -i rep.ncu-rep --page raw --csv | python -m paper_2604_21438_b200.ncu_summary --figures --cells N \
         --source "<the ncu command that wrote the report>" > profiles/<name>_figures.json
 
+    ncu -i rep.ncu-rep --page source --csv | python -m paper_2604_21438_b200.ncu_summary --source-page --cells N
+
 Default: a markdown table, one column per profiled launch, of the metrics that explain a kernel of this library
 (duration, DRAM bytes, pipe and issue utilisation, shared-memory wavefronts, stall reasons).  --figures: the
-numbers bench.py reads back (per-launch DRAM traffic of the corrector, fp64 instructions per cell-update of the two
-stage kernels; N = cells one launch updates).  Reads only its standard input; runs nothing.
+numbers bench.py reads back (per-launch DRAM traffic of the corrector; N = cells one launch updates); with
+--source-csv FILE (the `--page source --csv` export of the same report) also the fp64 instructions the two stage
+kernels execute per cell-update (DFMA + DMUL + DADD + DSETP thread instructions, predicated on).  --source-page:
+per kernel the SASS opcode mix (share of warp instructions, thread instructions per cell-update, shared-memory
+wavefronts) and the warp-stall samples by reason.  Reads only its inputs; runs nothing.
 """
+import collections
 import argparse
 import csv
 import json
@@ -63,32 +69,104 @@ def si(launch, units, name):
     return v * SCALE.get(units.get(name, ""), 1.0)
 
 
+FP64_OPS = ("DFMA", "DMUL", "DADD", "DSETP")
+STALL_COLS = ("stall_barrier", "stall_branch_resolving", "stall_dispatch", "stall_long_sb", "stall_math", "stall_mio",
+              "stall_no_inst", "stall_not_selected", "stall_selected", "stall_short_sb", "stall_wait", "stall_lg")
+
+
+def read_source(stream):
+    """{kernel name: [row dict per SASS instruction]} from `ncu --page source --csv`."""
+    out, kern, hdr = collections.OrderedDict(), None, None
+    for r in csv.reader(stream):
+        if not r:
+            continue
+        if r[0] == "Kernel Name":
+            kern = r[1]
+            out[kern] = []
+        elif r[0] == "Address":
+            hdr = r
+        elif kern is not None and hdr is not None and len(r) == len(hdr):
+            out[kern].append(dict(zip(hdr, r)))
+    return out
+
+
+def opcode_of(row):
+    src = re.sub(r"^@!?U?P\w+\s+", "", row["Source"].strip())
+    return src.split()[0].split(".")[0] if src else "?"
+
+
+def count(row, name):
+    try:
+        return int(row.get(name) or 0)
+    except ValueError:
+        return 0
+
+
+def fp64_per_cell(kernels, cells):
+    """fp64 thread instructions (predicated on) per cell of the predictor + corrector launches in a source export."""
+    tot = 0.0
+    for name, rows in kernels.items():
+        if re.search(r"stage_kernel|predictor_kernel|corrector_kernel", name):
+            tot += sum(count(r, "Predicated-On Thread Instructions Executed") for r in rows if opcode_of(r) in FP64_OPS)
+    return tot / cells if cells > 0 else None
+
+
+def source_page(kernels, cells, kernel_re):
+    for name, rows in kernels.items():
+        if not re.search(kernel_re, name):
+            continue
+        warp, thr, wf, stalls = collections.Counter(), collections.Counter(), collections.Counter(), collections.Counter()
+        for r in rows:
+            op = opcode_of(r)
+            warp[op] += count(r, "Instructions Executed")
+            thr[op] += count(r, "Predicated-On Thread Instructions Executed")
+            wf[op] += count(r, "L1 Wavefronts Shared")
+            for c in STALL_COLS:
+                stalls[c] += count(r, c)
+        tot = sum(warp.values()) or 1
+        print("### %s" % re.sub(r"^void |sfh::|\(int\)|\(bool\)|\(sfh::.*$", "", name))
+        print()
+        print("warp instructions %d; fp64 thread instructions per cell %.1f" %
+              (tot, sum(thr[o] for o in FP64_OPS) / cells if cells > 0 else float("nan")))
+        print()
+        print("| opcode | share of warp instructions % | thread instructions per cell | shared-memory wavefronts |")
+        print("|---|---|---|---|")
+        for op, n in warp.most_common(24):
+            print("| %s | %.2f | %.2f | %d |" % (op, 100.0 * n / tot, thr[op] / cells if cells > 0 else 0.0, wf[op]))
+        ts = sum(stalls.values()) or 1
+        print()
+        print("warp-stall samples: " + ", ".join("%s %.1f %%" % (c[6:], 100.0 * v / ts) for c, v in stalls.most_common()))
+        print()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--kernel", default=".", help="regex on the kernel name")
     ap.add_argument("--figures", action="store_true")
     ap.add_argument("--cells", type=float, default=0.0, help="--figures: cells one stage launch updates")
     ap.add_argument("--source", default="", help="--figures: the ncu command that wrote the report")
+    ap.add_argument("--source-csv", default="", help="--figures: `--page source --csv` export of the same report")
+    ap.add_argument("--source-page", action="store_true", help="standard input is a `--page source --csv` export")
     a = ap.parse_args()
+    if a.source_page:
+        source_page(read_source(sys.stdin), a.cells, a.kernel)
+        return
     names, units, launches = read_raw(sys.stdin)
     launches = [l for l in launches if re.search(a.kernel, l["Kernel Name"])]
     if a.figures:
         out = {"source": a.source, "cells_per_launch": a.cells}
-        f64 = 0.0
         for stage, key in ((0, "predictor"), (1, "corrector")):
             sel = [l for l in launches if re.search(r"stage_kernel<(\(int\))?%d\b" % stage, l["Kernel Name"])]
             if not sel:
                 continue
             n = len(sel)
             traffic = sum(si(l, units, "dram__bytes_read.sum") + si(l, units, "dram__bytes_write.sum") for l in sel) / n
-            inst = sum(number(l.get("sm__inst_executed_pipe_fp64.sum", "")) or 0.0 for l in sel) / n
             out[key + "_dram_bytes_per_launch"] = traffic
-            out[key + "_fp64_warp_inst_per_launch"] = inst
             out[key + "_time_us_under_ncu"] = sum(si(l, units, "gpu__time_duration.sum") for l in sel) / n * 1e6
             out[key + "_launches_averaged"] = n
-            f64 += inst * 32.0
-        if a.cells > 0 and f64 > 0:
-            out["fp64_thread_inst_per_cell_update"] = f64 / a.cells
+        if a.source_csv and a.cells > 0:
+            with open(a.source_csv) as f:
+                out["fp64_thread_inst_per_cell_update"] = fp64_per_cell(read_source(f), a.cells)
         json.dump(out, sys.stdout, indent=1)
         print()
         return
