@@ -198,18 +198,45 @@ class Mesh:
         self._chk(self.L.sfh_set_riemann(self.h, {"hllc": 0, "roe": 1}.get(solver, solver)))
 
     # ---- device
-    def bind(self):
+    def bind(self, guard=0, poison=False):
+        """Allocates the three state buffers and the work buffer and binds them.  Debugging aids (compute-sanitizer
+        is not available on every pool): guard > 0 puts `guard` doubles of a canary pattern before and after every
+        buffer (check_guards() tells whether any kernel wrote outside its buffer); poison fills everything the
+        library does not initialise itself with NaN, so that a read of never-written memory shows up in the results."""
         import torch
         if not torch.cuda.is_available():
             raise SfhError(-4, "no CUDA device: libsfh has no CPU fallback")
         dev = torch.device(self.device)
         torch.cuda.set_device(dev)
-        self.state = [torch.empty(self.state_bytes() // 8, dtype=torch.float64, device=dev) for _ in range(3)]
-        self.work = torch.empty(self.work_bytes() // 8, dtype=torch.float64, device=dev)
+        guard = (int(guard) + 31) // 32 * 32        # keeps the 256-byte alignment sfh_bind asks for
+        sizes = [self.state_bytes() // 8] * 3 + [self.work_bytes() // 8]
+        self._guard = guard
+        self._raw = [torch.empty(n + 2 * guard, dtype=torch.float64, device=dev) for n in sizes]
+        for r in self._raw:
+            if poison:
+                r.fill_(float("nan"))
+            if guard:
+                r[:guard] = self._CANARY
+                r[r.numel() - guard:] = self._CANARY
+        bufs = [r[guard:r.numel() - guard] for r in self._raw]
+        self.state, self.work = bufs[:3], bufs[3]
         torch.cuda.synchronize()
         self._chk(self.L.sfh_bind(self.h, self.state[0].data_ptr(), self.state[1].data_ptr(),
                                   self.state[2].data_ptr(), self.work.data_ptr()))
+        if poison:      # sfh_bind zeroes the work buffer; only its last 4 KB (device scalars: time, dt, counters) must stay
+            self.work[: self.work.numel() - 512] = float("nan")
+            torch.cuda.synchronize()
         self.bound = True
+
+    _CANARY = -6.02214076e23
+
+    def check_guards(self):
+        """True if the canaries around the four buffers are intact (bind(guard=n))."""
+        import torch
+        torch.cuda.synchronize()
+        g = self._guard
+        return all(bool((r[:g] == self._CANARY).all()) and bool((r[r.numel() - g:] == self._CANARY).all())
+                   for r in self._raw) if g else True
 
     def _dev_state(self, U):
         import torch

@@ -690,3 +690,35 @@ def test_scalar_count_is_validated_and_host_path_carries_scalars():
     hout = torch.empty_like(hin).pin_memory()
     g.advance_host(hin, hout, 2, 0)
     assert torch.equal(hout, ref.reshape(hout.shape))
+
+
+@pytest.mark.parametrize("name", ["C1", "amr-small", "amr-outflow", "C4/4", "ragged"])
+@pytest.mark.parametrize("scalars", [False, True])
+def test_guarded_and_poisoned_buffers(name, scalars):
+    """Own memcheck / initcheck (compute-sanitizer is closed on this GPU pool): every buffer the library is bound to
+    sits between canary regions, and everything the library does not initialise itself starts as NaN.  A kernel that
+    writes outside its buffer breaks a canary; one that reads memory nobody wrote puts a NaN into the result, which
+    the comparison with the oracle then sees.  Both drivers, the step-wise calls, the regrid pieces and get_ghosted
+    run on the guarded buffers."""
+    p = PROBLEMS[name]()
+    if scalars:
+        from sfh_inputs import add_scalars
+        p = add_scalars(p, scalar_fields())
+    o = oracle_for(p)
+    o.restrict_all(0)
+    g = sfh.Mesh.from_problem(p, bind=False)
+    g.bind(guard=4096, poison=True)
+    g.set_state(p.U)
+    g.restrict_all(0)
+    for mode in (p.mode, 0):
+        o.advance(2, mode)
+        g.advance(2, mode)
+        assert g.check_guards(), "a kernel wrote outside its buffer"
+        Ug, Uo = g.get_state().cpu().numpy(), o.get_state()
+        assert np.isfinite(Ug).all(), "uninitialised memory reached the state"
+        assert (parity_errors(Ug[:, :5], Uo[:, :5], p.gamma) <= TOL10).all()
+    g.fill_ghosts(-1, 0, 0, 0.0)
+    G = g.get_ghosted(0).cpu().numpy()
+    ind = g.refine_indicator(0).cpu().numpy()
+    assert np.isfinite(ind).all() and np.isfinite(G[:, :, 2:-2, 2:-2, 2:-2]).all()
+    assert g.check_guards()
