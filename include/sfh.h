@@ -58,7 +58,7 @@ typedef struct sfh_mesh sfh_mesh; /* opaque, library-owned */
 
 typedef struct {
   int32_t nb0[3];     /* root (level-0) blocks per axis */
-  int32_t ncell;      /* cells per block edge; only 8 is supported */
+  int32_t ncell;      /* cells per block edge: 8 or 16, see below */
   int32_t nghost;     /* ghost layers; only 2 is supported     */
   int32_t max_level;  /* finest level that may hold blocks (0 = uniform grid)                    */
   int32_t bc[3][2];   /* per axis, low/high face: 0 periodic, 1 outflow (zero gradient, R1)      */
@@ -68,6 +68,17 @@ typedef struct {
   int32_t nscalar;    /* passive scalars advected with the gas, 0..SFH_MAX_SCALARS   PAPER.md:80-88 (eq. 12-13) */
 } sfh_config;
 #define SFH_MAX_SCALARS 8
+
+/* Blocks of 16^3 cells (ncell = 16; the paper's faster GPU variant, Table 5).
+ * The scheme does not depend on how cells are grouped into blocks, and this library never stores ghost cells, so
+ * the halo-to-interior argument for larger blocks does not apply to it: a 16^3 block (l; I, J, K) is handled as its
+ * eight 8^3 octants (l; 2I + cx, 2J + cy, 2K + cz), octant c = cx + 2 cy + 4 cz, of a root grid of 2 nb0 blocks.
+ * What changes is the CALLER'S layout: every state array that crosses this interface (sfh_set_state,
+ * sfh_get_state, sfh_advance_host) is double [nblocks][5 + nscalar][16][16][16], and nb0, `level`, `ijk` of
+ * sfh_create_mesh count 16^3 blocks.  Everything that is counted or indexed per block elsewhere in this header
+ * (sfh_num_blocks, sfh_level_range, sfh_block_order, sfh_get_ghosted, sfh_refine_indicator, sfh_block_list, the
+ * per-block arguments of sfh_regrid*) then refers to the octants: entry e = 8 * block + c.  A mesh that sfh_regrid
+ * derives from a 16^3 mesh is a mesh of 8^3 blocks (refinement is decided per octant). */
 
 /* ---- mesh: octree block table and neighbour map -------------------------- */
 

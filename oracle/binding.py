@@ -1,6 +1,7 @@
 """ctypes binding of oracle/libsfh_oracle.so (test infrastructure only; see sfh_oracle.cpp).
 
-The oracle keeps GHOSTED 12^3 blocks in host memory, in the caller's block order.
+The oracle keeps GHOSTED 12^3 blocks in host memory, in the caller's block order (20^3 for the build with blocks
+of 16^3 cells, ncell = 16: the same source compiled with -DSFH_ORACLE_N=16).
 """
 import ctypes as C
 import os
@@ -18,13 +19,12 @@ class Config(C.Structure):
                 ("nscalar", C.c_int32)]
 
 
-_lib = None
+_libs = {}
 
 
-def lib():
-    global _lib
-    if _lib is None:
-        path = _build.build()
+def lib(ncell=N):
+    if ncell not in _libs:
+        path = _build.build(ncell=ncell)
         L = C.CDLL(path)
         L.orc_create_mesh.argtypes = [C.POINTER(Config), C.c_int64, C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p)]
         L.orc_destroy_mesh.argtypes = [C.c_void_p]
@@ -66,11 +66,11 @@ def lib():
         L.orc_num_blocks.argtypes = [C.c_void_p]
         L.orc_num_blocks.restype = C.c_int64
         L.orc_block_list.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
-        _lib = L
-    return _lib
+        _libs[ncell] = L
+    return _libs[ncell]
 
 
-def make_config(nb0, max_level, bc, box_len, gamma, cfl, nscalar=0):
+def make_config(nb0, max_level, bc, box_len, gamma, cfl, nscalar=0, ncell=N):
     cfg = Config()
     cfg.nscalar = int(nscalar)
     for d in range(3):
@@ -78,7 +78,7 @@ def make_config(nb0, max_level, bc, box_len, gamma, cfl, nscalar=0):
         cfg.box_len[d] = float(box_len[d])
         for s in range(2):
             cfg.bc[d][s] = int(bc[d][s])
-    cfg.ncell, cfg.nghost, cfg.max_level = N, G, int(max_level)
+    cfg.ncell, cfg.nghost, cfg.max_level = int(ncell), G, int(max_level)
     cfg.gamma, cfg.cfl = float(gamma), float(cfl)
     return cfg
 
@@ -102,10 +102,11 @@ def roe(WL, WR, d, gamma):
 class OracleMesh:
     """Oracle mesh + three ghosted state copies (0: U^n, 1: U^{n+1/2}, 2: U^{n+1})."""
 
-    def __init__(self, nb0, max_level, bc, box_len, gamma, cfl, level, ijk, nscalar=0, handle=None):
-        self.L = lib()
+    def __init__(self, nb0, max_level, bc, box_len, gamma, cfl, level, ijk, nscalar=0, handle=None, ncell=N):
+        self.L = lib(ncell)
+        self.n = int(ncell)                  # cells per block edge; ghosted blocks are (n + 4)^3
         self.nv = NV + int(nscalar)          # 5 hydro variables + passive scalars rho*s
-        self.cfg = make_config(nb0, max_level, bc, box_len, gamma, cfl, nscalar)
+        self.cfg = make_config(nb0, max_level, bc, box_len, gamma, cfl, nscalar, ncell)
         if handle is None:
             self.level = np.ascontiguousarray(level, dtype=np.int32)
             self.ijk = np.ascontiguousarray(ijk, dtype=np.int32).reshape(-1, 3)
@@ -121,7 +122,7 @@ class OracleMesh:
             self.level = np.zeros(self.nb, dtype=np.int32)
             self.ijk = np.zeros((self.nb, 3), dtype=np.int32)
             self.L.orc_block_list(self.h, self.level.ctypes.data, self.ijk.ctypes.data)
-        self.U = [np.zeros((self.nb, self.nv, M, M, M)) for _ in range(3)]
+        self.U = [np.zeros((self.nb, self.nv) + (self.n + 2 * G,) * 3) for _ in range(3)]
         self.L.orc_bind(self.h, *[u.ctypes.data for u in self.U])
         self.max_level = int(max_level)
         self.t = C.c_double(0.0)
@@ -138,10 +139,12 @@ class OracleMesh:
 
     # state access (interior cells, [nb][5][8][8][8] indexed [b][v][k][j][i])
     def set_state(self, Uint, copy=0):
-        self.U[copy][:, :, G:G + N, G:G + N, G:G + N] = Uint
+        n = self.n
+        self.U[copy][:, :, G:G + n, G:G + n, G:G + n] = Uint
 
     def get_state(self, copy=0):
-        return self.U[copy][:, :, G:G + N, G:G + N, G:G + N].copy()
+        n = self.n
+        return self.U[copy][:, :, G:G + n, G:G + n, G:G + n].copy()
 
     def is_leaf(self):
         return np.array([self.L.orc_is_leaf(self.h, b) for b in range(self.nb)], dtype=bool)
@@ -227,6 +230,7 @@ def oracle_for(p, U=None):
     """OracleMesh of a problem description `p` (fields nb0, max_level, bc, box_len, gamma, cfl, level, ijk, U:
     sfh_inputs.Problem), holding U (default p.U) as its copy 0."""
     U = p.U if U is None else U
-    m = OracleMesh(p.nb0, p.max_level, p.bc, p.box_len, p.gamma, p.cfl, p.level, p.ijk, nscalar=U.shape[1] - NV)
+    m = OracleMesh(p.nb0, p.max_level, p.bc, p.box_len, p.gamma, p.cfl, p.level, p.ijk, nscalar=U.shape[1] - NV,
+                   ncell=U.shape[-1])
     m.set_state(U)
     return m

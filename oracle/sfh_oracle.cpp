@@ -48,7 +48,11 @@
 
 namespace {
 
-constexpr int N = 8;    // cells per block edge
+#ifndef SFH_ORACLE_N
+#define SFH_ORACLE_N 8
+#endif
+constexpr int N = SFH_ORACLE_N;   // cells per block edge: 8; built a second time with 16
+constexpr int NF = N * N;         // cells of a block face
 constexpr int G = 2;    // ghost layers                    BASELINE.json configs
 constexpr int M = N + 2 * G;
 constexpr int NV = 5;   // rho, rho vx, rho vy, rho vz, rho E
@@ -85,7 +89,7 @@ struct Mesh {
   double* U[3] = {nullptr, nullptr, nullptr};
   // flux registers (Berger & Colella as cited): per flagged (block, face)
   std::vector<int> rslot, fslot;     // [nb*6] -> slot or -1
-  std::vector<double> R, FH;         // [slot][NV][8][8]
+  std::vector<double> R, FH;         // [slot][nv][N][N]
   int reflux_on = 1;
   int riemann = 0;                   // 0 HLLC, 1 Roe (PAPER.md:126 names both)
   char err[256] = {0};
@@ -147,10 +151,10 @@ inline bool apply_bc(const Mesh& m, int l, int idx[3]) {
 bool get(const Mesh& m, int l, int I, int J, int K, const Src* srcs, double out[NVMAX]) {
   int idx[3] = {I, J, K};
   apply_bc(m, l, idx);
-  const int b = find(m, l, idx[0] >> 3, idx[1] >> 3, idx[2] >> 3);
+  const int b = find(m, l, idx[0] / N, idx[1] / N, idx[2] / N);
   if (b >= 0) {
     if (srcs[l].mode < 0) return false;
-    cell_value(m, b, idx[0] & 7, idx[1] & 7, idx[2] & 7, srcs[l], out);
+    cell_value(m, b, idx[0] % N, idx[1] % N, idx[2] % N, srcs[l], out);
     return true;
   }
   if (l == 0) return false;
@@ -300,7 +304,7 @@ inline void riemann_flux(const Mesh& m, const double WL[NV], const double WR[NV]
   else hllc(WL, WR, d, m.cfg.gamma, F);
 }
 
-inline int fidx(int v, int f, int a, int b) { return ((v * 9 + f) * N + b) * N + a; }  // face f=0..8, tangential (a fastest)
+inline int fidx(int v, int f, int a, int b) { return ((v * (N + 1) + f) * N + b) * N + a; }  // face f=0..N, tangential (a fastest)
 
 inline void cell_of(int d, int c, int a, int b, int& i, int& j, int& k) {
   // c along d; (a,b) = the other two axes in increasing axis order
@@ -323,9 +327,9 @@ inline void all_prims(const Mesh& m, const double* U, int i, int j, int k, doubl
   for (int v = NV; v < m.nv; ++v) w[v] = U[gidx(v, i, j, k)] / u[0];
 }
 
-// U_out = U^n - lam * ((dFx + dFy) + dFz) on the interior cells, all nv variables; F = [3][nv][9][8][8]
+// U_out = U^n - lam * ((dFx + dFy) + dFz) on the interior cells, all nv variables; F = [3][nv][N+1][N][N]
 void flux_update(const Mesh& m, const double* Un, double* Uout, const std::vector<double>& F, double lam) {
-  const int fs = m.nv * 9 * N * N;
+  const int fs = m.nv * (N + 1) * N * N;
   const double* Fx = F.data(); const double* Fy = Fx + fs; const double* Fz = Fy + fs;
   for (int k = 0; k < N; ++k) for (int j = 0; j < N; ++j) for (int i = 0; i < N; ++i)
     for (int v = 0; v < m.nv; ++v) {
@@ -338,7 +342,7 @@ void flux_update(const Mesh& m, const double* Un, double* Uout, const std::vecto
 
 // ------------------------------------------------------------------ predictor (a4; reading R8)
 void predictor_block(Mesh& m, int b, double dt) {
-  const int nv = m.nv, fs = nv * 9 * N * N;
+  const int nv = m.nv, fs = nv * (N + 1) * N * N;
   const double h = h_of(m, m.lev[b]);
   const double* Un = m.U[0] + int64_t(b) * m.blk;
   double* Uh = m.U[1] + int64_t(b) * m.blk;
@@ -365,7 +369,7 @@ void predictor_block(Mesh& m, int b, double dt) {
 
 // ------------------------------------------------------------------ corrector (a6, a7; readings R11-R14)
 void corrector_block(Mesh& m, int b, double dt) {
-  const int nv = m.nv, fs = nv * 9 * N * N;
+  const int nv = m.nv, fs = nv * (N + 1) * N * N;
   const double h = h_of(m, m.lev[b]);
   const double* Un = m.U[0] + int64_t(b) * m.blk;
   const double* Uh = m.U[1] + int64_t(b) * m.blk;
@@ -401,8 +405,8 @@ void corrector_block(Mesh& m, int b, double dt) {
     const int rs = m.rslot[int64_t(b) * 6 + face], fsl = m.fslot[int64_t(b) * 6 + face];
     for (int v = 0; v < nv; ++v) for (int tb = 0; tb < N; ++tb) for (int ta = 0; ta < N; ++ta) {
       const double val = Fd[fidx(v, f, ta, tb)];
-      if (rs >= 0) m.R[(int64_t(rs) * nv + v) * 64 + tb * N + ta] += dt * val;
-      if (fsl >= 0) m.FH[(int64_t(fsl) * nv + v) * 64 + tb * N + ta] = val;
+      if (rs >= 0) m.R[(int64_t(rs) * nv + v) * NF + tb * N + ta] += dt * val;
+      if (fsl >= 0) m.FH[(int64_t(fsl) * nv + v) * NF + tb * N + ta] = val;
     }
   }
 }
@@ -422,8 +426,8 @@ void restrict_level(Mesh& m, int lc, int src_copy, int dst_copy) {   // level lc
         double sum = 0.0;
         for (int c = 0; c < 8; ++c) {   // fixed child-cell order c = cx + 2 cy + 4 cz
           const int fi = I + (c & 1), fj = J + ((c >> 1) & 1), fk = K + ((c >> 2) & 1);
-          const int fb = find(m, lc + 1, fi >> 3, fj >> 3, fk >> 3);
-          sum += m.U[src_copy][int64_t(fb) * m.blk + gidx(v, fi & 7, fj & 7, fk & 7)];
+          const int fb = find(m, lc + 1, fi / N, fj / N, fk / N);
+          sum += m.U[src_copy][int64_t(fb) * m.blk + gidx(v, fi % N, fj % N, fk % N)];
         }
         dst[gidx(v, i, j, k)] = 0.125 * sum;
       }
@@ -462,15 +466,15 @@ void reflux_level(Mesh& m, int lc, int copy, double dt_coarse) {
               if (ff[dd] < 0) ff[dd] += nf[dd];
               if (ff[dd] >= nf[dd]) ff[dd] -= nf[dd];
             }
-            const int fb = find(m, lc + 1, ff[0] >> 3, ff[1] >> 3, ff[2] >> 3);
+            const int fb = find(m, lc + 1, ff[0] / N, ff[1] / N, ff[2] / N);
             const int rs = m.rslot[int64_t(fb) * 6 + (2 * d + (1 - side))];
             int fa, fbb;
-            if (d == 0) { fa = ff[1] & 7; fbb = ff[2] & 7; }
-            else if (d == 1) { fa = ff[0] & 7; fbb = ff[2] & 7; }
-            else { fa = ff[0] & 7; fbb = ff[1] & 7; }
-            sumR += m.R[(int64_t(rs) * m.nv + v) * 64 + fbb * N + fa];
+            if (d == 0) { fa = ff[1] % N; fbb = ff[2] % N; }
+            else if (d == 1) { fa = ff[0] % N; fbb = ff[2] % N; }
+            else { fa = ff[0] % N; fbb = ff[1] % N; }
+            sumR += m.R[(int64_t(rs) * m.nv + v) * NF + fbb * N + fa];
           }
-          const double FHv = m.FH[(int64_t(fs) * m.nv + v) * 64 + tb * N + ta];
+          const double FHv = m.FH[(int64_t(fs) * m.nv + v) * NF + tb * N + ta];
           U[gidx(v, i, j, k)] = U[gidx(v, i, j, k)] - (s / h) * (0.25 * sumR - dt_coarse * FHv);
         }
       }
@@ -505,11 +509,11 @@ double cfl_dt_level(const Mesh& m, int l, int copy) {
 void zero_registers(Mesh& m, int lc) {   // registers of the (lc, lc+1) interface
   for (int b : m.of_level[lc + 1]) for (int f = 0; f < 6; ++f) {
     const int rs = m.rslot[int64_t(b) * 6 + f];
-    if (rs >= 0) std::fill_n(&m.R[int64_t(rs) * m.nv * 64], m.nv * 64, 0.0);
+    if (rs >= 0) std::fill_n(&m.R[int64_t(rs) * m.nv * NF], m.nv * NF, 0.0);
   }
   for (int b : m.of_level[lc]) for (int f = 0; f < 6; ++f) {
     const int fs = m.fslot[int64_t(b) * 6 + f];
-    if (fs >= 0) std::fill_n(&m.FH[int64_t(fs) * m.nv * 64], m.nv * 64, 0.0);
+    if (fs >= 0) std::fill_n(&m.FH[int64_t(fs) * m.nv * NF], m.nv * NF, 0.0);
   }
 }
 
@@ -603,8 +607,8 @@ int orc_create_mesh(const Config* cfg, int64_t nblocks, const int32_t* level, co
     if (nbk < 0) { if (l > 0) m->rslot[b * 6 + face] = nr++; }
     else if (m->leaf[b] && !m->leaf[nbk]) m->fslot[b * 6 + face] = nf++;
   }
-  m->R.assign(int64_t(nr) * m->nv * 64, 0.0);
-  m->FH.assign(int64_t(nf) * m->nv * 64, 0.0);
+  m->R.assign(int64_t(nr) * m->nv * NF, 0.0);
+  m->FH.assign(int64_t(nf) * m->nv * NF, 0.0);
   *out = m;
   return 0;
 }

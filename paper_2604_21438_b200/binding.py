@@ -117,7 +117,7 @@ class Mesh:
     double [nb][5][8][8][8] (interior cells, [block][var][k][j][i])."""
 
     def __init__(self, nb0, max_level, bc, box_len, gamma, cfl, level, ijk, device="cuda:0", bind=True, lib=None,
-                 nscalar=0, handle=None):
+                 nscalar=0, handle=None, ncell=N):
         self.L = lib or load_library()
         cfg = SfhConfig()
         for d in range(3):
@@ -125,7 +125,8 @@ class Mesh:
             cfg.box_len[d] = float(box_len[d])
             for s in range(2):
                 cfg.bc[d][s] = int(bc[d][s])
-        cfg.ncell, cfg.nghost, cfg.max_level = N, 2, int(max_level)
+        cfg.ncell, cfg.nghost, cfg.max_level = int(ncell), 2, int(max_level)
+        self.ncell = int(ncell)              # 8, or 16: states cross the interface as [nb][nv][16][16][16] (sfh.h)
         cfg.gamma, cfg.cfl = float(gamma), float(cfl)
         cfg.nscalar = int(nscalar)
         self.nv = NV + int(nscalar)          # variables per cell in the caller layout
@@ -154,6 +155,7 @@ class Mesh:
     @classmethod
     def from_problem(cls, p, **kw):
         kw.setdefault("nscalar", p.U.shape[1] - NV)
+        kw.setdefault("ncell", p.U.shape[-1])
         return cls(p.nb0, p.max_level, p.bc, p.box_len, p.gamma, p.cfl, p.level, p.ijk, **kw)
 
     def __del__(self):
@@ -166,13 +168,17 @@ class Mesh:
             raise SfhError(rc, self.L.sfh_last_error().decode())
 
     # ---- host-only queries
+    def nentries(self):
+        """Blocks as the library counts them: self.nb, or 8 * self.nb (the octants) for ncell = 16 (sfh.h)."""
+        return int(self.L.sfh_num_blocks(self.h))
+
     def level_range(self, l):
         a, b = C.c_int64(), C.c_int64()
         self._chk(self.L.sfh_level_range(self.h, l, C.byref(a), C.byref(b)))
         return a.value, b.value
 
     def block_order(self):
-        perm = np.zeros(self.nb, dtype=np.int64)
+        perm = np.zeros(self.nentries(), dtype=np.int64)
         self._chk(self.L.sfh_block_order(self.h, perm.ctypes.data))
         return perm
 
@@ -243,7 +249,7 @@ class Mesh:
         if isinstance(U, np.ndarray):
             U = torch.from_numpy(np.ascontiguousarray(U, dtype=np.float64))
         U = U.to(device=self.device, dtype=torch.float64).contiguous()
-        assert U.numel() == self.nb * self.nv * N ** 3, "state must be [nb][5 + nscalar][8][8][8]"
+        assert U.numel() == self.nb * self.nv * self.ncell ** 3, "state must be [nb][5 + nscalar][ncell]^3"
         return U
 
     def set_state(self, U, which=0):
@@ -255,13 +261,13 @@ class Mesh:
     def get_state(self, which=0):
         """torch tensor [nb][5][8][8][8] on the device."""
         import torch
-        out = torch.empty((self.nb, self.nv, N, N, N), dtype=torch.float64, device=self.device)
+        out = torch.empty((self.nb, self.nv) + (self.ncell,) * 3, dtype=torch.float64, device=self.device)
         self._chk(self.L.sfh_get_state(self.h, which, out.data_ptr(), _stream()))
         return out
 
     def get_ghosted(self, which=0):
         import torch
-        out = torch.empty((self.nb, NV, N + 4, N + 4, N + 4), dtype=torch.float64, device=self.device)
+        out = torch.empty((self.nentries(), NV, N + 4, N + 4, N + 4), dtype=torch.float64, device=self.device)
         self._chk(self.L.sfh_get_ghosted(self.h, which, out.data_ptr(), _stream()))
         return out
 
@@ -322,7 +328,7 @@ class Mesh:
     def regrid_from_indicator(self, indicator, threshold, bind=False):
         """The new mesh from a host indicator array (caller order); host only unless bind=True."""
         ind = np.ascontiguousarray(indicator, dtype=np.float64)
-        assert ind.shape == (self.nb,)
+        assert ind.shape == (self.nentries(),)
         h = C.c_void_p()
         self._chk(self.L.sfh_regrid_from_indicator(self.h, ind.ctypes.data, float(threshold), C.byref(h)))
         c = self.cfg
@@ -343,7 +349,7 @@ class Mesh:
     def refine_indicator(self, criterion=0, which=0, G=1.0):
         """Per-block refinement indicator (0: eq. 33-34 curvature, 1: h / Jeans length), caller order."""
         import torch
-        out = torch.empty(self.nb, dtype=torch.float64, device=self.device)
+        out = torch.empty(self.nentries(), dtype=torch.float64, device=self.device)
         self._chk(self.L.sfh_refine_indicator(self.h, which, criterion, float(G), out.data_ptr(), _stream()))
         return out
 

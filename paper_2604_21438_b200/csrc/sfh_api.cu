@@ -587,9 +587,9 @@ int sfh_set_state(sfh_mesh* m, int which, const double* d_U, void* stream) {
     if (which == 0) m->bmax_valid[l] = false;
     if (which == 2) m->bmax_pending[l] = false;
     CU(launch_permute(d_U, role_buf(m, l, which), m->d_perm, int(m->hm.lev_first[l]), int(m->hm.lev_count[l]), 1,
-                      which == 1, m->hm.cfg.gamma, m->ns, S(stream)), "permute_kernel");
+                      which == 1, m->hm.cfg.gamma, m->ns, m->hm.bs16, S(stream)), "permute_kernel");
     CU(launch_permute_scalar(d_U, role_q(m, l, which), m->d_perm, int(m->hm.lev_first[l]), int(m->hm.lev_count[l]),
-                             m->ns, 1, S(stream)), "permute_scalar_kernel");
+                             m->ns, 1, m->hm.bs16, S(stream)), "permute_scalar_kernel");
     m->launches += (m->hm.lev_count[l] > 0) * (1 + (m->ns > 0));
   }
   return SFH_OK;
@@ -601,9 +601,9 @@ int sfh_get_state(sfh_mesh* m, int which, double* d_U, void* stream) {
   if (which < 0 || which > 2 || !d_U) return fail(SFH_EINVAL, "bad argument");
   for (int l = 0; l < m->hm.nlev; ++l) {
     CU(launch_permute(role_buf(m, l, which), d_U, m->d_perm, int(m->hm.lev_first[l]), int(m->hm.lev_count[l]), 0,
-                      which == 1, m->hm.cfg.gamma, m->ns, S(stream)), "permute_kernel");
+                      which == 1, m->hm.cfg.gamma, m->ns, m->hm.bs16, S(stream)), "permute_kernel");
     CU(launch_permute_scalar(role_q(m, l, which), d_U, m->d_perm, int(m->hm.lev_first[l]), int(m->hm.lev_count[l]),
-                             m->ns, 0, S(stream)), "permute_scalar_kernel");
+                             m->ns, 0, m->hm.bs16, S(stream)), "permute_scalar_kernel");
     m->launches += (m->hm.lev_count[l] > 0) * (1 + (m->ns > 0));
   }
   return SFH_OK;

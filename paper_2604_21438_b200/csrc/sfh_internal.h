@@ -28,7 +28,9 @@ constexpr int NBR_COARSE = -1;   // no same-level block there (inside the domain
 constexpr int NBR_OUTSIDE = -2;  // beyond an outflow boundary
 
 struct HostMesh {
-  sfh_config cfg{};
+  sfh_config cfg{};                   // as the library works on it: ncell = 8 (a 16^3 mesh: nb0 doubled)
+  int bs16 = 0;                       // the caller's blocks hold 16^3 cells: entry e of the block list below is
+                                      // octant e & 7 of the caller's block e >> 3
   int64_t nb = 0;
   int nlev = 0;
   std::vector<int64_t> perm;          // library slot -> caller index

@@ -91,11 +91,21 @@ cudaError_t launch_dt_finalize(const unsigned long long* smax_bits, const LevelI
                                double* t_dev, cudaStream_t st);
 cudaError_t launch_count_bad(const double* U, int first, int count, double gamma, int prim, unsigned long long* nbad,
                              int sms, cudaStream_t st);
+// Position (in double2 units) of cell pair t2 = cell / 2 of variable v of caller entry e, in a caller array with nvt
+// variables per cell.  Blocks of 8^3 cells: [e][nvt][512].  Blocks of 16^3 cells (bs16): the
+// library handles a 16^3 block as its eight 8^3 octants, e = 8 * block + octant (octant c = cx + 2 cy + 4 cz), and
+// the caller's array is [block][nvt][16][16][16]: an octant's rows of 8 cells are contiguous.
+__host__ __device__ inline size_t caller_pos2(int64_t e, int v, int t2, int nvt, int bs16) {
+  if (!bs16) return (size_t(e) * nvt + v) * (NC / 2) + t2;
+  const int c = int(e & 7), i = 2 * (t2 & 3), j = (t2 >> 2) & 7, k = t2 >> 5;
+  const size_t row = ((size_t(e >> 3) * nvt + v) * 16 + 8 * (c >> 2) + k) * 16 + 8 * ((c >> 1) & 1) + j;
+  return (row * 16 + 8 * (c & 1) + i) / 2;
+}
 // dst[slot][...] = src[perm[slot]][...] (to_internal) or the inverse, for slots [first, first+count)
 // prim: the internal copy holds primitives (role 1); the caller's copy is always conserved
 // ns: passive scalars per cell: the caller's blocks are [5 + ns][512], the internal hydro blocks [5][512]
 cudaError_t launch_permute(const double* src, double* dst, const int64_t* perm, int first, int count, int to_internal,
-                           int prim, double gamma, int ns, cudaStream_t st);
+                           int prim, double gamma, int ns, int bs16, cudaStream_t st);
 cudaError_t launch_ghosted(const double* U, const double* ghost, const int32_t* face_src, const int64_t* perm,
                            int first, int count, int prim, double gamma, double* G, cudaStream_t st);
 // per-block refinement indicator (criterion 0: eq. 33-34, 1: h / Jeans length) of slots [first, first+count), caller order
@@ -154,7 +164,7 @@ cudaError_t launch_reflux_scalar(double* Q, const double* RS, const double* FHS,
                                  const int32_t* fslot, const int32_t* fh_src, int count, int ns, double h, double dt,
                                  const double* dt_dev, cudaStream_t st);
 cudaError_t launch_permute_scalar(const double* src, double* dst, const int64_t* perm, int first, int count, int ns,
-                                  int to_internal, cudaStream_t st);
+                                  int to_internal, int bs16, cudaStream_t st);
 cudaError_t launch_transfer_scalar(const TransferParams& p, int count, int ns, cudaStream_t st);
 // fp64 issue-rate microbenchmark: `ctas` CTAs of 1024 threads, each thread `iters` x 16 x `chains` DFMAs
 cudaError_t launch_dfma_rate(int chains, int ctas, int iters, double* sink, cudaStream_t st);

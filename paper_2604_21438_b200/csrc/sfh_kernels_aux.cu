@@ -369,39 +369,47 @@ cudaError_t launch_count_bad(const double* U, int first, int count, double gamma
 // =====================================================================================================
 __global__ void __launch_bounds__(256) permute_kernel(const double2* __restrict__ src, double2* __restrict__ dst,
                                                       const int64_t* __restrict__ perm, int first, int to_internal,
-                                                      int ns) {
+                                                      int ns, int bs16) {
   const int s = first + blockIdx.x;
-  const size_t a = size_t(s) * (BLK / 2), b = size_t(perm[s]) * ((NV + ns) * NC / 2);
-  const double2* from = src + (to_internal ? b : a);
-  double2* to = dst + (to_internal ? a : b);
-  for (int t = threadIdx.x; t < BLK / 2; t += 256) to[t] = from[t];
+  const int64_t e = perm[s];
+  const size_t a = size_t(s) * (BLK / 2);
+  for (int t = threadIdx.x; t < BLK / 2; t += 256) {
+    const size_t b = caller_pos2(e, t / (NC / 2), t % (NC / 2), NV + ns, bs16);
+    if (to_internal) dst[a + t] = src[b];
+    else dst[b] = src[a + t];
+  }
 }
 
 __global__ void __launch_bounds__(256) permute_prim_kernel(const double* __restrict__ src, double* __restrict__ dst,
                                                            const int64_t* __restrict__ perm, int first, int to_internal,
-                                                           double gamma, int ns) {
+                                                           double gamma, int ns, int bs16) {
   const int s = first + blockIdx.x;
-  const size_t a = size_t(s) * BLK, b = size_t(perm[s]) * (NV + ns) * NC;
-  const double* from = src + (to_internal ? b : a);
-  double* to = dst + (to_internal ? a : b);
+  const int64_t e = perm[s];
+  const size_t a = size_t(s) * BLK;
   const double gm1 = gamma - 1.0, igm1 = 1.0 / gm1;
   for (int c = threadIdx.x; c < NC; c += 256) {
     double x[NV], y[NV];
+    size_t b[NV];
 #pragma unroll
-    for (int v = 0; v < NV; ++v) x[v] = from[v * NC + c];
+    for (int v = 0; v < NV; ++v) b[v] = 2 * caller_pos2(e, v, c >> 1, NV + ns, bs16) + (c & 1);
+#pragma unroll
+    for (int v = 0; v < NV; ++v) x[v] = to_internal ? src[b[v]] : src[a + v * NC + c];
     if (to_internal) cons_to_prim(x, gm1, y);
     else prim_to_cons(x, igm1, y);
 #pragma unroll
-    for (int v = 0; v < NV; ++v) to[v * NC + c] = y[v];
+    for (int v = 0; v < NV; ++v) {
+      if (to_internal) dst[a + v * NC + c] = y[v];
+      else dst[b[v]] = y[v];
+    }
   }
 }
 
 cudaError_t launch_permute(const double* src, double* dst, const int64_t* perm, int first, int count, int to_internal,
-                           int prim, double gamma, int ns, cudaStream_t st) {
+                           int prim, double gamma, int ns, int bs16, cudaStream_t st) {
   if (count <= 0) return cudaSuccess;
-  if (prim) permute_prim_kernel<<<count, 256, 0, st>>>(src, dst, perm, first, to_internal, gamma, ns);
+  if (prim) permute_prim_kernel<<<count, 256, 0, st>>>(src, dst, perm, first, to_internal, gamma, ns, bs16);
   else permute_kernel<<<count, 256, 0, st>>>(reinterpret_cast<const double2*>(src), reinterpret_cast<double2*>(dst), perm,
-                                             first, to_internal, ns);
+                                             first, to_internal, ns, bs16);
   return cudaGetLastError();
 }
 

@@ -289,20 +289,23 @@ cudaError_t launch_reflux_scalar(double* Q, const double* RS, const double* FHS,
 // =====================================================================================================
 __global__ void __launch_bounds__(256) permute_scalar_kernel(const double2* __restrict__ src, double2* __restrict__ dst,
                                                              const int64_t* __restrict__ perm, int first, int ns,
-                                                             int to_internal) {
+                                                             int to_internal, int bs16) {
   const int s = first + blockIdx.x;
+  const int64_t e = perm[s];
   const size_t in = size_t(s) * ns * (NC / 2);                               // internal: scalars only
-  const size_t ca = (size_t(perm[s]) * (NV + ns) + NV) * (NC / 2);           // caller: behind the 5 hydro variables
-  const double2* from = src + (to_internal ? ca : in);
-  double2* to = dst + (to_internal ? in : ca);
-  for (int t = threadIdx.x; t < ns * (NC / 2); t += 256) to[t] = from[t];
+  for (int t = threadIdx.x; t < ns * (NC / 2); t += 256) {
+    // caller: behind the 5 hydro variables
+    const size_t ca = caller_pos2(e, NV + t / (NC / 2), t % (NC / 2), NV + ns, bs16);
+    if (to_internal) dst[in + t] = src[ca];
+    else dst[ca] = src[in + t];
+  }
 }
 
 cudaError_t launch_permute_scalar(const double* src, double* dst, const int64_t* perm, int first, int count, int ns,
-                                  int to_internal, cudaStream_t st) {
+                                  int to_internal, int bs16, cudaStream_t st) {
   if (count <= 0 || ns <= 0) return cudaSuccess;
   permute_scalar_kernel<<<count, 256, 0, st>>>(reinterpret_cast<const double2*>(src), reinterpret_cast<double2*>(dst),
-                                               perm, first, ns, to_internal);
+                                               perm, first, ns, to_internal, bs16);
   return cudaGetLastError();
 }
 

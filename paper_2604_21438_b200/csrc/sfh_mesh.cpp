@@ -52,10 +52,40 @@ struct Lookup {
 
 }  // namespace
 
-int build_host_mesh(const sfh_config& cfg, int64_t nblocks, const int32_t* level, const int32_t* ijk,
+// A mesh of 16^3-cell blocks is the mesh of their 8^3 octants: block (l; I, J, K) is the eight
+// blocks (l; 2I + cx, 2J + cy, 2K + cz) of a root grid twice as fine in blocks, with the same cells.  The scheme does
+// not depend on how cells are grouped into blocks, so nothing else changes; only the caller's arrays are laid out in
+// 16^3 blocks (caller_pos2 in sfh_kernels.cuh).
+int build_host_mesh(const sfh_config& cfg_in, int64_t nblocks_in, const int32_t* level_in, const int32_t* ijk_in,
                     HostMesh& m, std::string& err) {
   char buf[256];
-  if (cfg.ncell != N || cfg.nghost != NG) { err = "only ncell=8, nghost=2 are supported"; return SFH_EINVAL; }
+  if ((cfg_in.ncell != N && cfg_in.ncell != 2 * N) || cfg_in.nghost != NG) {
+    err = "only ncell = 8 or 16 and nghost = 2 are supported";
+    return SFH_EINVAL;
+  }
+  const bool bs16 = cfg_in.ncell == 2 * N;
+  sfh_config cfg = cfg_in;
+  int64_t nblocks = nblocks_in;
+  const int32_t *level = level_in, *ijk = ijk_in;
+  std::vector<int32_t> level8, ijk8;
+  if (bs16) {
+    if (nblocks_in <= 0 || nblocks_in > (int64_t(1) << 25) || !level_in || !ijk_in) { err = "bad block list"; return SFH_EINVAL; }
+    cfg.ncell = N;
+    for (int d = 0; d < 3; ++d) {
+      if (cfg.nb0[d] < 1 || cfg.nb0[d] > (1 << 19)) { err = "nb0 out of range"; return SFH_EINVAL; }
+      cfg.nb0[d] *= 2;
+    }
+    nblocks = 8 * nblocks_in;
+    level8.resize(size_t(nblocks));
+    ijk8.resize(size_t(3 * nblocks));
+    for (int64_t b = 0; b < nblocks_in; ++b)
+      for (int c = 0; c < 8; ++c) {
+        level8[8 * b + c] = level_in[b];
+        for (int d = 0; d < 3; ++d) ijk8[3 * (8 * b + c) + d] = 2 * ijk_in[3 * b + d] + ((c >> d) & 1);
+      }
+    level = level8.data();
+    ijk = ijk8.data();
+  }
   if (cfg.max_level < 0 || cfg.max_level >= MAX_LEVELS) { err = "max_level out of range"; return SFH_EINVAL; }
   if (nblocks <= 0 || nblocks > (int64_t(1) << 28) || !level || !ijk) { err = "bad block list"; return SFH_EINVAL; }
   for (int d = 0; d < 3; ++d) {
@@ -69,6 +99,7 @@ int build_host_mesh(const sfh_config& cfg, int64_t nblocks, const int32_t* level
 
   m = HostMesh();
   m.cfg = cfg;
+  m.bs16 = bs16;
   m.nb = nblocks;
   m.nlev = cfg.max_level + 1;
   for (int l = 0; l < m.nlev; ++l) m.h[l] = cfg.box_len[0] / (double(cfg.nb0[0]) * N * double(1 << l));

@@ -11,3 +11,4 @@ from .fields import (gaussian_random_field, lognormal_density, velocity_field, h
                      prim_to_cons)
 from .configs import make_config, CONFIG_NAMES, Problem  # noqa: F401
 from .small import small_amr_tree, smooth_fields, problem_from_tree, add_scalars  # noqa: F401
+from .blocks16 import to16, tree16_problem, split_state, merge_state, split_blocks  # noqa: F401

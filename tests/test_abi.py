@@ -142,3 +142,22 @@ def test_regrid_block_list_host_logic_matches_the_stated_rules():
             assert new.cfg.nscalar == m.cfg.nscalar and new.max_level == m.max_level
     with pytest.raises(sfh.SfhError):       # null indicator: a defined error
         m._chk(m.L.sfh_regrid_from_indicator(m.h, None, 0.5, C.byref(C.c_void_p())))
+
+
+def test_mesh_of_16_cell_blocks_is_the_mesh_of_their_octants():
+    """ncell = 16 (sfh.h): the block list counts 16^3 blocks; tables, level ranges and the block
+    order refer to their 8^3 octants, entry 8 * block + octant."""
+    t = small_amr_tree()
+    level, ijk = t.block_list()
+    m16 = sfh.Mesh(t.nb0, t.max_level, ((0, 0),) * 3, (1.0, 1.0, 1.0), 1.4, 0.4, level, ijk, bind=False, ncell=16)
+    from sfh_inputs import split_blocks
+    l8, ijk8 = split_blocks(level, ijk)
+    m8 = sfh.Mesh(tuple(2 * n for n in t.nb0), t.max_level, ((0, 0),) * 3, (1.0, 1.0, 1.0), 1.4, 0.4, l8, ijk8, bind=False)
+    assert m16.nentries() == 8 * len(level) == m8.nentries()
+    assert np.array_equal(m16.block_order(), m8.block_order())
+    assert m16.num_faces() == m8.num_faces() and m16.state_bytes() == m8.state_bytes()
+    assert m16.cell_width(1) == m8.cell_width(1) == 1.0 / (t.nb0[0] * 16 * 2)
+    for l in range(t.max_level + 1):
+        assert m16.level_range(l) == m8.level_range(l)
+    with pytest.raises(sfh.SfhError):
+        sfh.Mesh(t.nb0, t.max_level, ((0, 0),) * 3, (1.0, 1.0, 1.0), 1.4, 0.4, level, ijk, bind=False, ncell=12)

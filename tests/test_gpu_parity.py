@@ -722,3 +722,58 @@ def test_guarded_and_poisoned_buffers(name, scalars):
     ind = g.refine_indicator(0).cpu().numpy()
     assert np.isfinite(ind).all() and np.isfinite(G[:, :, 2:-2, 2:-2, 2:-2]).all()
     assert g.check_guards()
+
+
+def amr16_tree(periodic=(True, True, True)):
+    t = Tree((4, 3, 3), 2, periodic)
+    f0 = np.zeros_like(t.exists[0]); f0[1:2, 1:2, 1:2] = True
+    t.refine(0, f0)
+    f1 = np.zeros_like(t.exists[1]); f1[2:3, 2:4, 3:4] = True
+    t.refine(1, f1)
+    return t.pad_2to1()
+
+
+@pytest.mark.parametrize("case", ["C2/4", "C1", "amr", "amr-outflow+scalars", "amr-roe"])
+def test_blocks_of_16_cells(case):
+    """a mesh of 16^3-cell blocks, states crossing the interface as
+    [nb][nv][16][16][16].  Against the oracle built with N = 16 (north_star tolerances), and bitwise against the same
+    cells handed over as 8^3 blocks (the library runs both on the same octants)."""
+    from sfh_inputs import add_scalars, split_state, to16, tree16_problem
+    if case in ("C2/4", "C1"):
+        p16, p8 = to16(PROBLEMS[case]())
+    else:
+        p16, p8 = tree16_problem(amr16_tree((False, True, False) if "outflow" in case else (True, True, True)), mode=1)
+        if "scalars" in case:
+            p16, p8 = to16(add_scalars(p8, scalar_fields()))
+    assert p16.U.shape[-1] == 16 and p16.U.shape[0] * 8 == p8.U.shape[0]
+    o = oracle_for(p16)
+    g16, g8 = sfh.Mesh.from_problem(p16), sfh.Mesh.from_problem(p8)
+    assert g16.ncell == 16 and g16.nb * 8 == g8.nb
+    for m, p in ((o, p16), (g16, p16), (g8, p8)):
+        if "roe" in case:
+            m.set_riemann("roe")
+        if m is not o:
+            m.set_state(p.U)
+        m.restrict_all(0)
+    assert np.array_equal(g16.get_state().cpu().numpy(), o.get_state())
+    nv = p16.U.shape[1]
+    for nsteps, tol in ((1, TOL1), (9, TOL10)):
+        for m in (o, g16, g8):
+            m.advance(nsteps, p16.mode)
+        U16 = g16.get_state().cpu().numpy()
+        assert np.array_equal(split_state(U16), g8.get_state().cpu().numpy())
+        assert abs(g16.t.value - o.t.value) <= TOLDT * o.t.value and np.array_equal(g16.nupd, o.nupd)
+        assert (parity_errors(U16[:, :5], o.get_state()[:, :5], p16.gamma) <= tol).all()
+        if nv > 5:
+            assert np.abs(U16[:, 5:] - o.get_state()[:, 5:]).max() <= tol * np.abs(o.get_state()[:, 5:]).max()
+    # the end-to-end call moves the same layout
+    import torch
+    hin = torch.from_numpy(p16.U.copy()).pin_memory()
+    hout = torch.empty_like(hin).pin_memory()
+    g16.set_state(p16.U)
+    g16.restrict_all(0)
+    ref = g16.get_state().cpu()
+    g16.advance(1, p16.mode)
+    want = g16.get_state().cpu().numpy()
+    g16.advance_host(ref.pin_memory(), hout, 1, p16.mode)
+    assert np.array_equal(hout.numpy(), want)
