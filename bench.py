@@ -53,6 +53,9 @@ def parse():
     ap.add_argument("--per-config", default="C3,C4,C5", help="other full-size configs reported in config.per_config")
     ap.add_argument("--no-per-config", action="store_true")
     ap.add_argument("--peaks", action="store_true", help="print the measured fp64 issue rates of this device and exit")
+    ap.add_argument("--ncell", type=int, default=8, choices=[8, 16],
+                    help="hand the workload over in blocks of 16^3 cells (sfh.h; PAPER.md:536, 579): the same cells and the "
+                         "same kernels on the 8^3 octants, only the caller's layout differs")
     ap.add_argument("--extras", action="store_true",
                     help="also time the regrid pieces (refinement indicators, state transfer) on this config")
     return ap.parse_args()
@@ -155,8 +158,8 @@ class ClockSampler:
                 "power_w_max": max(r[3] for r in rows), "source": "nvml" if self.nv else "nvidia-smi"}
 
 
-def cell_updates(census, nupd):
-    return float(sum(512 * c * int(n) for c, n in zip(census, nupd)))
+def cell_updates(census, nupd, ncell=8):
+    return float(sum(ncell ** 3 * c * int(n) for c, n in zip(census, nupd)))
 
 
 def max_over_ranks(ms, world, device="cpu"):
@@ -231,6 +234,9 @@ def measure(sfh, torch, name, args, dev, world, barrier, steps, warmup, sampler_
     length), kernel-span pass (same runs with events around every launch), optionally the end-to-end pass."""
     from sfh_inputs import make_config
     p = make_config(name, args.scale)
+    if args.ncell == 16:
+        from sfh_inputs import to16
+        p = to16(p)[0]
     census = p.census()
     g = sfh.Mesh.from_problem(p, device=dev)
     g.set_riemann(args.riemann)
@@ -269,7 +275,7 @@ def measure(sfh, torch, name, args, dev, world, barrier, steps, warmup, sampler_
         windows.append((t0, time.time()))
         ms += e0.elapsed_time(e1)
         launches += g.launch_count() - l0
-        cu += cell_updates(census, g.nupd)
+        cu += cell_updates(census, g.nupd, args.ncell)
         nupd_tot = g.nupd.copy() if nupd_tot is None else nupd_tot + g.nupd
         bad = max(bad, g.status())
     clocks = sampler.stop(windows) if sampler else None
@@ -330,7 +336,7 @@ def measure(sfh, torch, name, args, dev, world, barrier, steps, warmup, sampler_
             e1.record()
             barrier()
             ms_e2e += e0.elapsed_time(e1)
-            cu_e2e += cell_updates(census, g.nupd)
+            cu_e2e += cell_updates(census, g.nupd, args.ncell)
         ms_e2e = max_over_ranks(ms_e2e, world, dev)
         out["e2e"] = {"value": whole_job_value(cu_e2e, ms_e2e, world), "unit": UNIT, "h2d_bytes_per_step": state_bytes,
                       "d2h_bytes_per_step": state_bytes, "ms_per_step": ms_e2e / sum(runs)}
@@ -460,7 +466,7 @@ def main():
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": m["workload"], "config": args.config, "scale": args.scale, "riemann": args.riemann,
                    "blocks_per_level": m["census"], "updates_per_level": [int(x) for x in m["nupd"]],
-                   "mode": m["mode"],
+                   "mode": m["mode"], "cells_per_block_edge": args.ncell,
                    "timed_runs": m["runs"],
                    "l2": "inputs larger than L2 (one state copy %.0f MB vs 126 MB L2)" % (m["state_bytes"] / 1e6),
                    "kernel_spans": "second pass of the same runs with CUDA events around every launch",
