@@ -182,3 +182,37 @@ def test_c5_full_size_every_cell_one_coarse_step():
     err = parity_errors(g.get_state().cpu().numpy(), o.get_state(), p.gamma)
     print("C5 full size: updates/level", list(g.nupd), "parity", err)
     assert (err <= TOL1).all(), err
+
+
+def test_c3_full_size_every_cell_one_step():
+    """All 1.3e8 cells of C3 against the oracle after one step (the oracle's three ghosted copies take 54 GB of host
+    memory).  The Mach-10 input puts a few cells at non-positive pressure in this very step (R28: no floors on
+    either side; what such a cell holds is undefined, and its neighbours read it only in the NEXT step), so the
+    comparison covers every cell whose oracle value is finite with positive density and pressure, and the number of
+    cells left out is reported and bounded."""
+    import os
+    ram_gb = os.sysconf("SC_PAGE_SIZE") * os.sysconf("SC_PHYS_PAGES") / 2 ** 30
+    if ram_gb < 110:
+        pytest.skip("the oracle's three ghosted copies of C3 need 54 GB (+ inputs): host has %.0f GB" % ram_gb)
+    p = make_config("C3")
+    o = oracle_for(p)
+    g = gpu_for(p)
+    o.advance(1, 0)
+    g.advance(1, 0)
+    assert abs(g.t.value - o.t.value) <= TOLDT * o.t.value
+    Uo = o.get_state()
+    Ug = g.get_state().cpu().numpy()
+    rho, E = Uo[:, 0], Uo[:, 4]
+    P = (p.gamma - 1.0) * (E - 0.5 * (Uo[:, 1] ** 2 + Uo[:, 2] ** 2 + Uo[:, 3] ** 2) / rho)
+    good = np.isfinite(Uo).all(axis=1) & (rho > 0.0) & (P > 0.0)
+    nbad = int((~good).sum())
+    print("C3 full size, one step: %d of %d cells left out (oracle not positive), oracle status %d, CUDA status %d"
+          % (nbad, good.size, o.status(), g.status()))
+    assert nbad <= 100 and nbad == o.status() and g.status() == nbad
+    scale = np.array([np.abs(Uo[:, 0][good]).max(), 0.0, 0.0, 0.0, np.abs(Uo[:, 4][good]).max()])
+    cs = np.sqrt(p.gamma * P[good] / rho[good])
+    mscale = max((np.abs(Uo[:, v][good]) + rho[good] * cs).max() for v in (1, 2, 3))
+    scale[1:4] = mscale
+    for v in range(5):
+        d = np.abs(Ug[:, v][good] - Uo[:, v][good]).max() / scale[v]
+        assert d <= TOL1, (v, d)
