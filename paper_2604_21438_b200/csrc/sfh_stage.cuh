@@ -48,7 +48,7 @@ struct Cfg {
   static constexpr int TS = NVW * CVS;                // tile stride (doubles): 896 / 640, a multiple of 1 KB
   static constexpr int LAND = NTILE * TS;             // one staged block
   static constexpr int NDF = STAGE == 0 ? 1 : 2;      // flux-difference buffers that fit beside the staging
-  static constexpr int SMEM = (2 * LAND + NDF * DF_DOUBLES) * 8 + 256 + 1024;   // + barriers, + alignment slack
+  static constexpr int SMEM = (2 * LAND + NDF * DF_DOUBLES) * 8 + 384 + 1024;   // + barriers, + alignment slack
 };
 static_assert(Cfg<0>::SMEM <= 232448 && Cfg<1>::SMEM <= 232448, "shared memory of one SM");
 static_assert((Cfg<0>::TS * 8) % 1024 == 0 && (Cfg<1>::TS * 8) % 1024 == 0, "swizzled tiles start on 1 KB");
@@ -220,19 +220,18 @@ __device__ __forceinline__ void corrector_flux(const double WLs[5], const double
 // in registers, so that the twelve walker warps run ONE straight-line body: a third of the instruction
 // footprint of three direction instantiations, and no loop-carried register rotation.
 struct WalkGeom {
-  int cp[8];     // cells f0-2 .. f0+5 of the half pencil
+  int cp[12];    // cells -2 .. 9 of the pencil (a half pencil reads -2 .. 4 or 2 .. 9)
   int ov[3];     // offsets of the normal and the two tangential velocities
-  int di[4];     // flux-difference positions of cells f0 .. f0+3
+  int di[8];     // flux-difference positions of cells 0 .. 7
 };
 template <int STAGE, int D>
-__device__ __forceinline__ void walk_geom(int a, int b, int f0, WalkGeom& g) {
+__device__ __forceinline__ void walk_geom(int a, int b, WalkGeom& g) {
   constexpr int TS = Cfg<STAGE>::TS;
 #pragma unroll
-  for (int cc = 0; cc < 8; ++cc) g.cp[cc] = cell_pos<TS, D>(f0 - 2 + cc, a, b);
+  for (int cc = 0; cc < 12; ++cc) g.cp[cc] = cell_pos<TS, D>(cc - 2, a, b);
   g.ov[0] = (1 + D) * CVS; g.ov[1] = (1 + (D + 1) % 3) * CVS; g.ov[2] = (1 + (D + 2) % 3) * CVS;
 #pragma unroll
-  for (int cc = 0; cc < 4; ++cc)
-    g.di[cc] = D == 0 ? dfx_idx(f0 + cc, a, b) : D == 1 ? dfy_idx(a, f0 + cc, b) : dfz_idx(a, b, f0 + cc);
+  for (int cc = 0; cc < 8; ++cc) g.di[cc] = D == 0 ? dfx_idx(cc, a, b) : D == 1 ? dfy_idx(a, cc, b) : dfz_idx(a, b, cc);
 }
 __device__ __forceinline__ void load_cell_g(const double* __restrict__ Wl, int o, const int ov[3], double w[5]) {
   w[0] = Wl[o]; w[1] = Wl[o + ov[0]]; w[2] = Wl[o + ov[1]]; w[3] = Wl[o + ov[2]]; w[4] = Wl[o + 4 * CVS];
@@ -240,28 +239,37 @@ __device__ __forceinline__ void load_cell_g(const double* __restrict__ Wl, int o
 // REGS: the level has flux-register faces
 template <int RS, bool REGS, bool MFX>
 __device__ __forceinline__ void walk_corrector_generic(const double* __restrict__ Wl, double* __restrict__ dF,
-                                                       const WalkGeom& g, int D, int a, int b, int f0, double gamma,
+                                                       const WalkGeom& g, int D, int a, int b, double gamma,
                                                        double igm1, const StageParams& p, int blk, double dt,
                                                        uint32_t bar_empty, uint32_t par_empty, bool wait_empty,
-                                                       double* __restrict__ mf) {
+                                                       double* __restrict__ mf, bool upper, uint32_t bar_pair,
+                                                       uint32_t par_pair) {
   double wp[5], wc[5], wn[5], dp[5], dn[5], L[5], Ln[5], R[5], Fa[5], Fb[5];
+  const int f0 = upper ? 4 : 0;                               // faces f0 .. f0+4 (upper) or f0 .. f0+3 (lower)
+  int cp[8], di[4];                                           // cells f0-2 .. f0+5, flux-difference slots of cells f0 .. f0+3
+#pragma unroll
+  for (int cc = 0; cc < 8; ++cc) cp[cc] = upper ? g.cp[cc + 4] : g.cp[cc];
+#pragma unroll
+  for (int cc = 0; cc < 4; ++cc) di[cc] = upper ? g.di[cc + 4] : g.di[cc];
+  const int ds = g.di[3];                                     // cell 3's slot: face 4 goes through it to the lower half
   int rsrc = 0, rfs = -1;                                     // my boundary face: halo source, coarse-side register
   if (REGS) {
     const int f = blk * 6 + 2 * D + (f0 != 0);
     rsrc = p.face_src[f];
     rfs = p.fslot[f];
   }
-  load_cell_g(Wl, g.cp[0], g.ov, wp);
-  load_cell_g(Wl, g.cp[1], g.ov, wc);
-  load_cell_g(Wl, g.cp[2], g.ov, wn);
+  load_cell_g(Wl, cp[0], g.ov, wp);
+  load_cell_g(Wl, cp[1], g.ov, wc);
+  load_cell_g(Wl, cp[2], g.ov, wn);
 #pragma unroll
   for (int v = 0; v < 5; ++v) { dp[v] = wc[v] - wp[v]; dn[v] = wn[v] - wc[v]; }
   limited_states(wc, dn, dp, R, L);                           // L = left state of face f0
 #pragma unroll
   for (int ff = 0; ff < 5; ++ff) {                            // face f0+ff, between cells cc = ff+1 and ff+2
+    if (ff == 4 && !upper) break;                             // face 4 comes from the upper half pencil (warp-uniform)
 #pragma unroll
     for (int v = 0; v < 5; ++v) { wc[v] = wn[v]; dp[v] = dn[v]; }
-    load_cell_g(Wl, g.cp[ff + 3], g.ov, wn);
+    load_cell_g(Wl, cp[ff + 3], g.ov, wn);
 #pragma unroll
     for (int v = 0; v < 5; ++v) dn[v] = wn[v] - wc[v];
     limited_states(wc, dn, dp, R, Ln);                        // right state of this face, left state of the next
@@ -272,12 +280,23 @@ __device__ __forceinline__ void walk_corrector_generic(const double* __restrict_
     if (ff == 0) {
       if (REGS && f0 == 0 && (rsrc <= -2 || rfs >= 0)) store_regs(rsrc, rfs, p.R, p.FH, D, b * 8 + a, Fa, dt);
       if (wait_empty) mbar_wait(bar_empty, par_empty);        // the update two blocks back has read this dF buffer
+      if (upper) {                                            // face 4: hand the flux to the lower half through cell 3's slot
+#pragma unroll
+        for (int q = 0; q < 5; ++q) dF[ds + q * NC] = Fa[q];
+        __syncwarp();
+        if ((threadIdx.x & 31) == 0) mbar_arrive(bar_pair);
+      }
     } else {
 #pragma unroll
-      for (int q = 0; q < 5; ++q) dF[g.di[ff - 1] + q * NC] = (ff & 1) ? Fb[q] - Fa[q] : Fa[q] - Fb[q];
+      for (int q = 0; q < 5; ++q) dF[di[ff - 1] + q * NC] = (ff & 1) ? Fb[q] - Fa[q] : Fa[q] - Fb[q];
     }
   }
   if (REGS && f0 != 0 && (rsrc <= -2 || rfs >= 0)) store_regs(rsrc, rfs, p.R, p.FH, D, b * 8 + a, Fa, dt);
+  if (!upper) {                                               // cell 3: F(face 4) - F(face 3), face 3 is in Fb
+    mbar_wait(bar_pair, par_pair);
+#pragma unroll
+    for (int q = 0; q < 5; ++q) dF[ds + q * NC] = dF[ds + q * NC] - Fb[q];
+  }
 }
 
 // ---- helpers: staging ----------------------------------------------------------------------------------
@@ -458,6 +477,9 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
   auto full = [&](int d) { return bar0 + 32u + 8u * d; };
   auto empty = [&](int d) { return bar0 + 48u + 8u * d; };
   auto conv = [&](int s) { return bar0 + 64u + 8u * s; };   // predictor: the walkers have converted buffer s
+  // pair[P][it & 1]: the upper half pencils of (axis, pencil half) P have stored face 4 of block it.  Two per pair: the
+  // upper warp may be a block ahead of the lower one, never two (the staging of block it + 2 waits for `full` of block it).
+  auto pair = [&](int P, int it) { return bar0 + 224u + 8u * (2 * P + (it & 1)); };
 
   const int tid = threadIdx.x;
   const int stride = gridDim.x;
@@ -471,6 +493,7 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
       mbar_init(full(s), WALK_WARPS);
       mbar_init(empty(s), HELP_WARPS);
     }
+    for (int P = 0; P < 12; ++P) mbar_init(bar0 + 224u + 8u * P, 1);
     fence_mbar_init();
   }
   __syncthreads();
@@ -481,12 +504,23 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
     // ------------------------------------------------------------------------------ walkers
 
     const double igm1 = 1.0 / gm1;
-    const int D = tid >> 7, f0 = ((tid >> 6) & 1) * 4, pen = tid & 63, a = pen & 7, b = pen >> 3;
+    // Predictor: thread (D, half, pencil) walks faces 4 half .. 4 half + 4 (face 4 twice: its single flux-difference
+    // buffer makes the walkers meet at every block anyway, measured: sharing face 4 loses 4 % there).
+    // Corrector: no face is computed twice.  Warp w owns (axis D, pencils 32 q .. 32 q + 31) and one HALF: the upper half
+    // computes faces 4..8 and hands face 4 to the lower half through cell 3's flux-difference slot, the lower half
+    // computes faces 0..3.  The halves change hands every block, so that every warp averages 4.5 faces per block (its
+    // two flux-difference buffers let a warp run up to a block ahead of the others), and they are dealt so that each
+    // sub-partition (warp & 3) carries 14 or 13 faces per pencil at any time instead of 15.
+    const int wp = tid >> 5, sub = wp & 3, slot = wp >> 2;
+    const int P = STAGE == 0 ? (wp >> 2) + 3 * (wp & 1) : (sub >> 1) * 3 + slot;      // P = D + 3 q
+    const int D = P % 3;
+    const bool upper0 = STAGE == 0 ? ((wp >> 1) & 1) != 0 : ((sub & 1) ? slot == 2 : slot < 2);
+    const int f0 = upper0 ? 4 : 0, pen = (P / 3) * 32 + (tid & 31), a = pen & 7, b = pen >> 3;
     WalkGeom geom;
     if (STAGE == 1) {
-      if (D == 0) walk_geom<1, 0>(a, b, f0, geom);
-      else if (D == 1) walk_geom<1, 1>(a, b, f0, geom);
-      else walk_geom<1, 2>(a, b, f0, geom);
+      if (D == 0) walk_geom<1, 0>(a, b, geom);
+      else if (D == 1) walk_geom<1, 1>(a, b, geom);
+      else walk_geom<1, 2>(a, b, geom);
     }
     auto convert_next = [&](int it) {                  // predictor: my share of block it, then both arrivals
       const int s = it & 1;
@@ -505,14 +539,15 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
       const uint32_t pe = ((it / C::NDF) - 1) & 1;
       mbar_wait(ready(s), (it >> 1) & 1);
       const int blk = blk0 + it * stride;
-      // mass fluxes of the block: [axis][face 0..8][pencil] (face 4 is written by both half pencils, same bits)
+      // mass fluxes of the block: [axis][face 0..8][pencil]
       double* mf = MFX ? p.mf + (size_t(blk) * 3 + D) * (9 * FACE) + pen : nullptr;
       if (STAGE == 0) {
         if (D == 0) walk_predictor<RS, 0, MFX>(Wl, dF, a, b, f0, gm1, igm1, empty(d), pe, we, mf);
         else if (D == 1) walk_predictor<RS, 1, MFX>(Wl, dF, a, b, f0, gm1, igm1, empty(d), pe, we, mf);
         else walk_predictor<RS, 2, MFX>(Wl, dF, a, b, f0, gm1, igm1, empty(d), pe, we, mf);
       } else {
-        walk_corrector_generic<RS, REGS, MFX>(Wl, dF, geom, D, a, b, f0, gamma, igm1, p, blk, dt, empty(d), pe, we, mf);
+        walk_corrector_generic<RS, REGS, MFX>(Wl, dF, geom, D, a, b, gamma, igm1, p, blk, dt, empty(d), pe, we, mf,
+                                              upper0 != bool(it & 1), pair(P, it), (it >> 1) & 1);
       }
       __syncwarp();
       if ((tid & 31) == 0) mbar_arrive(full(d));
