@@ -45,6 +45,11 @@ struct sfh_mesh {
   int role[MAX_LEVELS][3];              // role -> physical state buffer, per level
   TensorMaps tm[3];                     // per physical state buffer
   int64_t launches = 0;
+  // eq. (15) needs the finer level's CFL step on the host once per parent step.  The reduction does not depend on the
+  // parent's own update, so it is enqueued BEFORE the parent's stage kernels, copied to pinned memory, and the host
+  // waits on an event that has long fired when it gets there: the device never idles for the round trip.
+  unsigned long long* h_smax = nullptr;  // pinned, [MAX_LEVELS]
+  cudaEvent_t ev_smax[MAX_LEVELS] = {nullptr};
   // optional per-kernel-class timing (sfh_profile / sfh_kernel_times)
   bool profiling = false;
   struct Span { int cls; cudaEvent_t a, b; };
@@ -359,6 +364,35 @@ int cfl_host(sfh_mesh* m, int level, double* dt_out, cudaStream_t st) {
   return SFH_OK;
 }
 
+// The CFL step of level l in two halves: request (reduction + copy to pinned memory + event, all on the stream) and
+// fetch (wait for the event, form the step).  Between the two the caller may enqueue work that does not change role 0
+// of level l.
+int cfl_request(sfh_mesh* m, int l, cudaStream_t st) {
+  int rc;
+  if (!m->h_smax) {
+    CU(cudaHostAlloc(reinterpret_cast<void**>(&m->h_smax), sizeof(unsigned long long) * MAX_LEVELS, cudaHostAllocDefault),
+       "cudaHostAlloc");
+  }
+  if (!m->ev_smax[l]) CU(cudaEventCreateWithFlags(&m->ev_smax[l], cudaEventDisableTiming), "cudaEventCreate");
+  if ((rc = max_speed_level(m, l, st))) return rc;
+  CU(cudaMemcpyAsync(m->h_smax + l, m->smax + l, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st), "memcpy smax");
+  CU(cudaEventRecord(m->ev_smax[l], st), "cudaEventRecord");
+  return SFH_OK;
+}
+int cfl_fetch(sfh_mesh* m, int l, double* dt_out) {
+  CU(cudaEventSynchronize(m->ev_smax[l]), "cudaEventSynchronize");
+  double s;
+  std::memcpy(&s, m->h_smax + l, 8);
+  const double dtl = m->hm.cfg.cfl * m->hm.h[l] / s;
+  if (!(dtl > 0.0) || !std::isfinite(dtl)) {
+    char buf[128];
+    snprintf(buf, sizeof buf, "CFL step of level %d is not finite and positive (max speed %g): bad cells? (sfh_status)", l, s);
+    return fail(SFH_ESTATE, buf);
+  }
+  *dt_out = dtl;
+  return SFH_OK;
+}
+
 // eq. (14)-(15): smallest n >= 0 with dtH 2^-n <= dt_cfl (reading R18)
 constexpr int MAX_SUBSTEP_EXPONENT = 20;   // 2^20 sub-steps of one parent step: beyond any sane hierarchy
 int substep_exponent(double dtH, double dt_cfl) {
@@ -372,12 +406,15 @@ int advance_adaptive(sfh_mesh* m, int l, double dt, double tau, double dtau, int
   const int interp = l > 0;
   int rc;
   // the coarser level has finished its step: its three time copies give both ghost fills in one gather
+  const bool has_finer = l + 1 < hm.nlev && hm.lev_count[l + 1] > 0;
+  // the finer level's CFL step (for eq. 15 below) does not depend on this level's update: ask for it first
+  if (has_finer && (rc = cfl_request(m, l + 1, st))) return rc;
   if ((rc = fill_level(m, l, 0, interp, tau, st, interp != 0, tau + 0.5 * dtau))) return rc;
   if ((rc = hydro_level(m, l, Dt{dt, nullptr}, interp, tau, dtau, st, interp != 0))) return rc;
   if (nupd) nupd[l] += 1;
-  if (l + 1 < hm.nlev && hm.lev_count[l + 1] > 0) {
+  if (has_finer) {
     double dtc;
-    if ((rc = cfl_host(m, l + 1, &dtc, st))) return rc;
+    if ((rc = cfl_fetch(m, l + 1, &dtc))) return rc;
     const int n = substep_exponent(dt, dtc);
     if (n > MAX_SUBSTEP_EXPONENT) {
       char buf[160];
@@ -458,6 +495,8 @@ int sfh_destroy_mesh(sfh_mesh* m) {
   if (!m) return SFH_OK;
   for (auto& sp : m->spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
   for (cudaEvent_t e : m->event_pool) cudaEventDestroy(e);
+  for (cudaEvent_t e : m->ev_smax) if (e) cudaEventDestroy(e);
+  if (m->h_smax) cudaFreeHost(m->h_smax);
   if (m->dev_tables) cudaFree(m->dev_tables);
   delete m;
   return SFH_OK;
