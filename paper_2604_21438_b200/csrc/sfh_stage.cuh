@@ -613,7 +613,7 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
       __syncwarp();
       if (lane0) mbar_arrive(empty(d));                // the walkers may store the next flux differences
       store_block<STAGE == 0>(un, gm1, p.Udst + size_t(blk) * BLK, hid);
-      if (it + 2 < n) prepare(it + 2);
+      if (STAGE == 0 && it + 2 < n) prepare(it + 2);
       if (STAGE == 1 && p.bmax) {
         // The block's maximum CFL speed for the next step's dt (reading R16) from the updated cells still in
         // registers, after everything the walkers wait for has been handed over.  (Measured: these 26 fp64
@@ -628,6 +628,8 @@ __global__ void __launch_bounds__(STAGE_THREADS, 1) stage_kernel(const __grid_co
         asm volatile("bar.sync 1, %0;" ::"n"(HELP_THREADS) : "memory");
         if (hid == 0) p.bmax[blk] = fmax(fmax(hm[0], hm[1]), fmax(hm[2], hm[3]));
       }
+      // (corrector: after the block maximum, whose arithmetic covers the landing of the copies issued above)
+      if (STAGE == 1 && it + 2 < n) prepare(it + 2);
     }
   }
 }
