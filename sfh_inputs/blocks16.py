@@ -64,7 +64,6 @@ def to16(p8):
 
 def tree16_problem(t16, **kw):
     """Problem on the 16^3-block octree t16 (sfh_inputs.Tree) and the same problem on its 8^3 octants."""
-    from .mesh import Tree
     from .small import problem_from_tree
     level16, ijk16 = t16.block_list()
     level8, ijk8 = split_blocks(level16, ijk16)
