@@ -2,13 +2,13 @@
  * of arxiv/paper_2604_21438 (SFUMATO#), B200 (sm_100a) only.
  *
  * What the calls compute is defined by PAPER.md (cited per call as PAPER.md:<line>) and, where the
- * paper is silent, by the readings R1..R31 of DESIGN.md.  There is no CPU fallback: every call that
+ * paper is silent, by the readings R1..R34 of DESIGN.md.  There is no CPU fallback: every call that
  * touches field data launches CUDA kernels on the caller's stream and returns SFH_ECUDA when no
  * device is usable.
  *
  * Conventions
- *   - Blocks: N^3 = 8^3 cells, fixed; level l has cell width h_l = box_len[0] / (nb0[0]*8*2^l)
- *     (PAPER.md:96).  A block of level l has integer coordinates (bx,by,bz) in [0, nb0_d * 2^l);
+ *   - Blocks: N^3 = 8^3 cells (16^3: see "Blocks of 16^3 cells" below); level l has cell width
+ *     h_l = box_len[0] / (nb0[0]*8*2^l).  A block of level l has integer coordinates (bx,by,bz) in [0, nb0_d * 2^l);
  *     child c = cx + 2 cy + 4 cz of (bx,by,bz) is (2bx+cx, 2by+cy, 2bz+cz) at level l+1.
  *     EVERY block of every level holds data and is updated, covered (non-leaf) blocks too.
  *   - Conserved variables, in this order: rho, rho*vx, rho*vy, rho*vz, rho*E with
