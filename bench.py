@@ -53,6 +53,9 @@ def parse():
     ap.add_argument("--per-config", default="C3,C4,C5", help="other full-size configs reported in config.per_config")
     ap.add_argument("--no-per-config", action="store_true")
     ap.add_argument("--peaks", action="store_true", help="print the measured fp64 issue rates of this device and exit")
+    ap.add_argument("--nscalar", type=int, default=0,
+                    help="passive scalars advected with the gas (eq. 12-13, PAPER.md:80-88; SURVEY.md 8(f) row 4): smooth "
+                         "seeded concentrations, 40 B more per scalar and cell-update")
     ap.add_argument("--ncell", type=int, default=8, choices=[8, 16],
                     help="hand the workload over in blocks of 16^3 cells (sfh.h; PAPER.md:536, 579): the same cells and the "
                          "same kernels on the 8^3 octants, only the caller's layout differs")
@@ -234,6 +237,12 @@ def measure(sfh, torch, name, args, dev, world, barrier, steps, warmup, sampler_
     length), kernel-span pass (same runs with events around every launch), optionally the end-to-end pass."""
     from sfh_inputs import make_config
     p = make_config(name, args.scale)
+    if args.nscalar > 0:
+        import numpy as np
+        from sfh_inputs import add_scalars
+        tp = 2.0 * np.pi
+        p = add_scalars(p, [(lambda X, Y, Z, q=q: 0.5 + 0.4 * np.sin(tp * (X + 0.13 * q)) * np.cos(tp * (Y - 0.07 * q)) *
+                             np.cos(tp * Z)) for q in range(args.nscalar)])
     if args.ncell == 16:
         from sfh_inputs import to16
         p = to16(p)[0]
@@ -466,7 +475,8 @@ def main():
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": m["workload"], "config": args.config, "scale": args.scale, "riemann": args.riemann,
                    "blocks_per_level": m["census"], "updates_per_level": [int(x) for x in m["nupd"]],
-                   "mode": m["mode"], "cells_per_block_edge": args.ncell,
+                   "mode": m["mode"], "cells_per_block_edge": args.ncell, "passive_scalars": args.nscalar,
+                   "algorithmic_bytes_per_cell_update": STEP_BYTES_PER_CELL_UPDATE + 40.0 * args.nscalar,
                    "timed_runs": m["runs"],
                    "l2": "inputs larger than L2 (one state copy %.0f MB vs 126 MB L2)" % (m["state_bytes"] / 1e6),
                    "kernel_spans": "second pass of the same runs with CUDA events around every launch",

@@ -19,9 +19,10 @@ __device__ __forceinline__ int gpos(int i, int j, int k) { return ((k + NG) * M1
 
 // Source of one variable of ghosted cell (i, j, k) of block s: the block itself, the same-level neighbour, the block's
 // own edge layer (outflow) or the coarse-fine slab.  Edge / corner ghosts (no stage reads them): returns null.
-// U: array [nb][nvar][512] (+ v * NC selects the variable); slab: [ncf][nslabvar][128] (+ v * 128).
+// U: array [nb][nvar][512] (+ v * NC selects the variable); slab: [ncf][nslabvar][128] (+ v * 128); fsrc6: the six
+// face sources of block s.
 __device__ __forceinline__ const double* ghost_src(const double* __restrict__ U, int nvar, const double* __restrict__ slab,
-                                                   int nslabvar, const int32_t* __restrict__ face_src, int s, int i, int j,
+                                                   int nslabvar, const int32_t* __restrict__ fsrc6, int s, int i, int j,
                                                    int k, int* vstride) {
   const int o[3] = {i < 0 ? -1 : i >= N ? 1 : 0, j < 0 ? -1 : j >= N ? 1 : 0, k < 0 ? -1 : k >= N ? 1 : 0};
   const int nout = (o[0] != 0) + (o[1] != 0) + (o[2] != 0);
@@ -29,7 +30,7 @@ __device__ __forceinline__ const double* ghost_src(const double* __restrict__ U,
   if (nout == 0) return U + size_t(s) * nvar * NC + (k * 8 + j) * 8 + i;
   if (nout > 1) return nullptr;
   const int axis = o[0] ? 0 : o[1] ? 1 : 2, side = o[axis] > 0;
-  const int src = face_src[s * 6 + 2 * axis + side];
+  const int src = fsrc6[2 * axis + side];
   int q[3] = {i, j, k};
   if (src == SRC_OUTFLOW) {
     q[axis] = side ? N - 1 : 0;
@@ -45,41 +46,76 @@ __device__ __forceinline__ const double* ghost_src(const double* __restrict__ U,
 }
 
 // =====================================================================================================
-// Scalar stage: one CTA of 256 threads per block.  rho and s = q / rho of the block and its two-layer face halos go
-// to shared memory (gathered like the stage kernels gather: neighbour interiors, outflow copies, coarse-fine slabs);
-// every thread then updates two cells: the six face fluxes of a cell (each face is evaluated by both its cells,
-// a few flops), dF in the order (x + y) + z, q_out = q^n - lambda dF.  STAGE 1 also feeds the scalar flux registers
-// of coarse-fine faces (fine side += dt F, coarse leaf side = F; one contributor per entry: no atomics needed).
+// Scalar stage: one CTA of 256 threads per block.  1 / rho and s = q / rho of the block and its two-layer face halos
+// go to shared memory (gathered like the stage kernels gather: neighbour interiors, outflow copies, coarse-fine
+// slabs; every thread resolves the sources of its up to seven ghosted cells ONCE, for all scalars), and so do the
+// block's mass fluxes (read coalesced, stored face-fastest / row-contiguous so that the cells of a warp read them
+// without bank conflicts).  Every thread then updates two cells per scalar: the six face fluxes of a cell (each
+// face is evaluated by both its cells, a few flops), dF in the order (x + y) + z, q_out = q^n - lambda dF.
+// STAGE 1 also feeds the scalar flux registers of coarse-fine faces (fine side += dt F, coarse leaf side = F; one
+// contributor per entry: no atomics needed).
 // =====================================================================================================
+constexpr int GPT = (G3 + 255) / 256;        // ghosted cells per thread (7)
+// mass fluxes of one block in shared memory: x faces [k][j][9], y faces [k][9][i], z faces [9][j][i]
+__device__ __forceinline__ int mfs_pos(int d, int f, int ta, int tb) {   // face f of pencil (ta, tb) (lower axis first)
+  return d == 0 ? (tb * 8 + ta) * 9 + f : d == 1 ? 576 + (tb * 9 + f) * 8 + ta : 1152 + (f * 8 + tb) * 8 + ta;
+}
+
 template <int STAGE>
-__global__ void __launch_bounds__(256) scalar_stage_kernel(const ScalarStageParams p) {
-  __shared__ double rho[G3];
+__global__ void __launch_bounds__(256, 4) scalar_stage_kernel(const ScalarStageParams p) {
+  __shared__ double irho[G3];
   __shared__ double sv[G3];
+  __shared__ double mfs[3 * 9 * FACE];
   const int s = p.first + blockIdx.x;
   const int t = threadIdx.x;
   const double dt = p.dt_dev ? *p.dt_dev : p.dt;
   const double lam = (STAGE == 0 ? 0.5 : 1.0) * dt / p.h;
-  for (int c = t; c < G3; c += 256) {
-    const int i = c % M12 - NG, j = (c / M12) % M12 - NG, k = c / (M12 * M12) - NG;
-    int vs;
-    const double* from = ghost_src(p.Hsrc, NV, p.ghostH, NV, p.face_src, s, i, j, k, &vs);
-    rho[c] = from ? from[0] : 1.0;          // variable 0 of both the conserved and the primitive copies is rho
-  }
+  // the block's mass fluxes [axis][face 0..8][pencil]: coalesced read, transposed store
+  __shared__ int fsrc6[6];                 // the face sources first: the gathers below must not wait for them one by one
+  if (t < 6) fsrc6[t] = p.face_src[s * 6 + t];
   const double* mf = p.mf + size_t(s) * 3 * 9 * FACE;
-  for (int v = 0; v < p.ns; ++v) {
-    __syncthreads();                         // rho is complete / the previous scalar's sv is no longer read
-    for (int c = t; c < G3; c += 256) {
+  for (int c = t; c < 3 * 9 * FACE; c += 256) {
+    const int d = c / (9 * FACE), f = (c / FACE) % 9, pen = c & (FACE - 1);
+    mfs[mfs_pos(d, f, pen & 7, pen >> 3)] = mf[c];
+  }
+  // sources of my ghosted cells: variable 0 of the scalars (null: an edge or corner ghost, which no stage reads)
+  __syncthreads();
+  const double* qsrc[GPT];
+  const double* hsrc[GPT];
+  unsigned slabbed = 0;                    // bit r: the source is a coarse-fine slab (variable stride 128, not 512)
+#pragma unroll
+  for (int r = 0; r < GPT; ++r) {
+    const int c = t + 256 * r;
+    qsrc[r] = nullptr;
+    hsrc[r] = nullptr;
+    if (c < G3) {
       const int i = c % M12 - NG, j = (c / M12) % M12 - NG, k = c / (M12 * M12) - NG;
       int vs;
-      const double* from = ghost_src(p.Qsrc, p.ns, p.ghostS, p.ns, p.face_src, s, i, j, k, &vs);
-      sv[c] = from ? from[v * vs] / rho[c] : 0.0;
+      hsrc[r] = ghost_src(p.Hsrc, NV, p.ghostH, NV, fsrc6, s, i, j, k, &vs);
+      qsrc[r] = ghost_src(p.Qsrc, p.ns, p.ghostS, p.ns, fsrc6, s, i, j, k, &vs);
+      slabbed |= unsigned(vs != NC) << r;
+    }
+  }
+  double rh[GPT];                          // (all loads in flight before the first reciprocal)
+#pragma unroll
+  for (int r = 0; r < GPT; ++r) rh[r] = (t + 256 * r < G3 && hsrc[r]) ? hsrc[r][0] : 1.0;   // variable 0 of both copies is rho
+#pragma unroll
+  for (int r = 0; r < GPT; ++r) if (t + 256 * r < G3) irho[t + 256 * r] = rcp_fast(rh[r]);
+  for (int v = 0; v < p.ns; ++v) {
+    __syncthreads();                         // irho, mfs complete / the previous scalar's sv is no longer read
+#pragma unroll
+    for (int r = 0; r < GPT; ++r) {
+      const int c = t + 256 * r;
+      if (c < G3) sv[c] = qsrc[r] ? qsrc[r][v * ((slabbed >> r) & 1 ? NG * FACE : NC)] * irho[c] : 0.0;
     }
     __syncthreads();
-#pragma unroll 1
+#pragma unroll
     for (int cell = t; cell < NC; cell += 256) {
       const int ijk[3] = {cell & 7, (cell >> 3) & 7, cell >> 6};
       const int st[3] = {1, M12, M12 * M12};
       const int m0 = gpos(ijk[0], ijk[1], ijk[2]);
+      const size_t o = (size_t(s) * p.ns + v) * NC + cell;
+      const double qn = p.Qn[o];
       double dF[3];
 #pragma unroll
       for (int d = 0; d < 3; ++d) {
@@ -93,7 +129,7 @@ __global__ void __launch_bounds__(256) scalar_stage_kernel(const ScalarStagePara
             sL = sL + 0.5 * minmod(sv[mr] - sv[ml], sv[ml] - sv[ml - st[d]]);
             sR = sR - 0.5 * minmod(sv[mr + st[d]] - sv[mr], sv[mr] - sv[ml]);
           }
-          const double fm = mf[(d * 9 + c + e) * FACE + tb * 8 + ta];
+          const double fm = mfs[mfs_pos(d, c + e, ta, tb)];
           F[e] = fm * (fm >= 0.0 ? sL : sR);
         }
         dF[d] = F[1] - F[0];
@@ -107,8 +143,7 @@ __global__ void __launch_bounds__(256) scalar_stage_kernel(const ScalarStagePara
           if (fs >= 0) p.FHS[(size_t(fs) * p.ns + v) * FACE + tb * 8 + ta] = F[e];
         }
       }
-      const size_t o = (size_t(s) * p.ns + v) * NC + cell;
-      p.Qdst[o] = p.Qn[o] - lam * ((dF[0] + dF[1]) + dF[2]);
+      p.Qdst[o] = qn - lam * ((dF[0] + dF[1]) + dF[2]);
     }
   }
 }
@@ -334,7 +369,7 @@ __global__ void __launch_bounds__(256) transfer_scalar_kernel(const TransferPara
       const int c[3] = {oct[0] * 4 + (f[0] >> 1), oct[1] * 4 + (f[1] >> 1), oct[2] * 4 + (f[2] >> 1)};
       auto fetch = [&](int c0, int c1, int c2) {       // one ghost layer is reached at most: the slab layer next to the face
         int vs;
-        const double* from = ghost_src(Qs, ns, ghost, ns, face_src, P, c0, c1, c2, &vs);
+        const double* from = ghost_src(Qs, ns, ghost, ns, face_src + P * 6, P, c0, c1, c2, &vs);
         return from[v * vs];
       };
       const double Q = fetch(c[0], c[1], c[2]);
