@@ -55,7 +55,6 @@ __device__ __forceinline__ const double* ghost_src(const double* __restrict__ U,
 // STAGE 1 also feeds the scalar flux registers of coarse-fine faces (fine side += dt F, coarse leaf side = F; one
 // contributor per entry: no atomics needed).
 // =====================================================================================================
-constexpr int GPT = (G3 + 255) / 256;        // ghosted cells per thread (7)
 // mass fluxes of one block in shared memory: x faces [k][j][9], y faces [k][9][i], z faces [9][j][i]
 __device__ __forceinline__ int mfs_pos(int d, int f, int ta, int tb) {   // face f of pencil (ta, tb) (lower axis first)
   return d == 0 ? (tb * 8 + ta) * 9 + f : d == 1 ? 576 + (tb * 9 + f) * 8 + ta : 1152 + (f * 8 + tb) * 8 + ta;
@@ -63,51 +62,79 @@ __device__ __forceinline__ int mfs_pos(int d, int f, int ta, int tb) {   // face
 
 template <int STAGE>
 __global__ void __launch_bounds__(256, 4) scalar_stage_kernel(const ScalarStageParams p) {
-  __shared__ double irho[G3];
-  __shared__ double sv[G3];
+  __shared__ double sv[G3];                // s = q / rho on the ghosted block (edges and corners are never read)
   __shared__ double mfs[3 * 9 * FACE];
   const int s = p.first + blockIdx.x;
   const int t = threadIdx.x;
   const double dt = p.dt_dev ? *p.dt_dev : p.dt;
   const double lam = (STAGE == 0 ? 0.5 : 1.0) * dt / p.h;
-  // the block's mass fluxes [axis][face 0..8][pencil]: coalesced read, transposed store
   __shared__ int fsrc6[6];                 // the face sources first: the gathers below must not wait for them one by one
   if (t < 6) fsrc6[t] = p.face_src[s * 6 + t];
+  // the block's mass fluxes [axis][face 0..8][pencil]: coalesced read, transposed store; warp pair w2 = t >> 6 takes
+  // the (axis, face) rows w2, w2 + 4, ...
   const double* mf = p.mf + size_t(s) * 3 * 9 * FACE;
-  for (int c = t; c < 3 * 9 * FACE; c += 256) {
-    const int d = c / (9 * FACE), f = (c / FACE) % 9, pen = c & (FACE - 1);
-    mfs[mfs_pos(d, f, pen & 7, pen >> 3)] = mf[c];
+#pragma unroll
+  for (int rr = 0; rr < 7; ++rr) {
+    const int row = (t >> 6) + 4 * rr, pen = t & (FACE - 1);
+    if (row < 27) mfs[mfs_pos(row / 9, row % 9, pen & 7, pen >> 3)] = mf[row * FACE + pen];
   }
-  // sources of my ghosted cells: variable 0 of the scalars (null: an edge or corner ghost, which no stage reads)
   __syncthreads();
-  const double* qsrc[GPT];
-  const double* hsrc[GPT];
+  // My five cells of the ghosted block: interior cells t and t + 256, and items t, t + 256, t + 512 of the six
+  // two-layer face halos (item h: face h >> 7 -- warp-uniform --, layer (h >> 6) & 1, in-face position h & 63).  For
+  // each: where it goes in the 12^3 arrays, and where variable 0 of rho / of the scalars comes from (the block itself,
+  // the same-level neighbour, the block's own edge layer at an outflow face, or the coarse-fine slab).
+  constexpr int NI = 5;
+  int dst[NI];
+  const double* qsrc[NI];
+  const double* hsrc[NI];
   unsigned slabbed = 0;                    // bit r: the source is a coarse-fine slab (variable stride 128, not 512)
 #pragma unroll
-  for (int r = 0; r < GPT; ++r) {
-    const int c = t + 256 * r;
-    qsrc[r] = nullptr;
-    hsrc[r] = nullptr;
-    if (c < G3) {
-      const int i = c % M12 - NG, j = (c / M12) % M12 - NG, k = c / (M12 * M12) - NG;
-      int vs;
-      hsrc[r] = ghost_src(p.Hsrc, NV, p.ghostH, NV, fsrc6, s, i, j, k, &vs);
-      qsrc[r] = ghost_src(p.Qsrc, p.ns, p.ghostS, p.ns, fsrc6, s, i, j, k, &vs);
-      slabbed |= unsigned(vs != NC) << r;
+  for (int r = 0; r < 2; ++r) {
+    const int cell = t + 256 * r;
+    dst[r] = gpos(cell & 7, (cell >> 3) & 7, cell >> 6);
+    hsrc[r] = p.Hsrc + size_t(s) * NV * NC + cell;
+    qsrc[r] = p.Qsrc + size_t(s) * p.ns * NC + cell;
+  }
+#pragma unroll
+  for (int r = 0; r < 3; ++r) {
+    const int h = t + 256 * r, f = h >> 7, axis = f >> 1, side = f & 1, ll = (h >> 6) & 1, ta = h & 7, tb = (h >> 3) & 7;
+    const int src = fsrc6[f];
+    int q[3];                              // the ghost cell, block-local
+    q[axis] = side ? N + ll : ll - NG;
+    q[axis == 0 ? 1 : 0] = ta;
+    q[axis == 2 ? 1 : 2] = tb;
+    dst[2 + r] = gpos(q[0], q[1], q[2]);
+    if (src <= -2) {                       // coarse-fine slab
+      const int pos = slab_pos(axis, ll, ta, tb);
+      hsrc[2 + r] = p.ghostH + size_t(-2 - src) * NV * (NG * FACE) + pos;
+      qsrc[2 + r] = p.ghostS + size_t(-2 - src) * p.ns * (NG * FACE) + pos;
+      slabbed |= 1u << (2 + r);
+    } else {
+      const int blk = src >= 0 ? src : s;  // same-level neighbour, or the block's own edge layer (outflow)
+      q[axis] = src >= 0 ? q[axis] + (side ? -N : N) : (side ? N - 1 : 0);
+      const int cell = (q[2] * 8 + q[1]) * 8 + q[0];
+      hsrc[2 + r] = p.Hsrc + size_t(blk) * NV * NC + cell;
+      qsrc[2 + r] = p.Qsrc + size_t(blk) * p.ns * NC + cell;
     }
   }
-  double rh[GPT];                          // (all loads in flight before the first reciprocal)
+  // All loads of the first scalar are in flight together with those of rho; the loads of scalar v + 1 are issued
+  // before scalar v is computed (one memory latency per block instead of one per phase).
+  double rh[NI], qv[NI];
+  auto load_q = [&](int v) {
 #pragma unroll
-  for (int r = 0; r < GPT; ++r) rh[r] = (t + 256 * r < G3 && hsrc[r]) ? hsrc[r][0] : 1.0;   // variable 0 of both copies is rho
+    for (int r = 0; r < NI; ++r) qv[r] = qsrc[r][v * ((slabbed >> r) & 1 ? NG * FACE : NC)];
+  };
 #pragma unroll
-  for (int r = 0; r < GPT; ++r) if (t + 256 * r < G3) irho[t + 256 * r] = rcp_fast(rh[r]);
+  for (int r = 0; r < NI; ++r) rh[r] = hsrc[r][0];                 // variable 0 of both copies is rho
+  load_q(0);
+  double ir[NI];
+#pragma unroll
+  for (int r = 0; r < NI; ++r) ir[r] = rcp_fast(rh[r]);
   for (int v = 0; v < p.ns; ++v) {
-    __syncthreads();                         // irho, mfs complete / the previous scalar's sv is no longer read
+    __syncthreads();                         // the previous scalar's sv is no longer read
 #pragma unroll
-    for (int r = 0; r < GPT; ++r) {
-      const int c = t + 256 * r;
-      if (c < G3) sv[c] = qsrc[r] ? qsrc[r][v * ((slabbed >> r) & 1 ? NG * FACE : NC)] * irho[c] : 0.0;
-    }
+    for (int r = 0; r < NI; ++r) sv[dst[r]] = qv[r] * ir[r];
+    if (v + 1 < p.ns) load_q(v + 1);
     __syncthreads();
 #pragma unroll
     for (int cell = t; cell < NC; cell += 256) {
