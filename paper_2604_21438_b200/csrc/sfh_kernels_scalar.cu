@@ -69,7 +69,8 @@ __global__ void __launch_bounds__(256, 4) scalar_stage_kernel(const ScalarStageP
   const double dt = p.dt_dev ? *p.dt_dev : p.dt;
   const double lam = (STAGE == 0 ? 0.5 : 1.0) * dt / p.h;
   __shared__ int fsrc6[6];                 // the face sources first: the gathers below must not wait for them one by one
-  if (t < 6) fsrc6[t] = p.face_src[s * 6 + t];
+  __shared__ int fslot6[6];
+  if (t < 6) { fsrc6[t] = p.face_src[s * 6 + t]; fslot6[t] = STAGE == 1 ? p.fslot[s * 6 + t] : -1; }
   // the block's mass fluxes [axis][face 0..8][pencil]: coalesced read, transposed store; warp pair w2 = t >> 6 takes
   // the (axis, face) rows w2, w2 + 4, ...
   const double* mf = p.mf + size_t(s) * 3 * 9 * FACE;
@@ -147,22 +148,25 @@ __global__ void __launch_bounds__(256, 4) scalar_stage_kernel(const ScalarStageP
 #pragma unroll
       for (int d = 0; d < 3; ++d) {
         const int ta = d == 0 ? ijk[1] : ijk[0], tb = d == 2 ? ijk[1] : ijk[2], c = ijk[d];
+        // s of the cells c-1, c, c+1 (and c-2, c+2 for the corrector's three limited slopes): each slope once
+        const double s0 = sv[m0], sm = sv[m0 - st[d]], sp = sv[m0 + st[d]];
+        double sL[2] = {sm, s0}, sR[2] = {s0, sp};            // left / right states of the lower and the upper face
+        if (STAGE == 1) {
+          const double smm = sv[m0 - 2 * st[d]], spp = sv[m0 + 2 * st[d]];
+          const double d1 = sm - smm, d2 = s0 - sm, d3 = sp - s0, d4 = spp - sp;
+          const double hm = 0.5 * minmod(d2, d1), h0 = 0.5 * minmod(d3, d2), hp = 0.5 * minmod(d4, d3);
+          sL[0] = sm + hm; sR[0] = s0 - h0; sL[1] = s0 + h0; sR[1] = sp - hp;
+        }
         double F[2];
 #pragma unroll
         for (int e = 0; e < 2; ++e) {        // the cell's lower (e = 0) and upper face: face index c + e
-          const int ml = m0 + (e - 1) * st[d], mr = ml + st[d];     // cells left and right of the face
-          double sL = sv[ml], sR = sv[mr];
-          if (STAGE == 1) {
-            sL = sL + 0.5 * minmod(sv[mr] - sv[ml], sv[ml] - sv[ml - st[d]]);
-            sR = sR - 0.5 * minmod(sv[mr + st[d]] - sv[mr], sv[mr] - sv[ml]);
-          }
           const double fm = mfs[mfs_pos(d, c + e, ta, tb)];
-          F[e] = fm * (fm >= 0.0 ? sL : sR);
+          F[e] = fm * (fm >= 0.0 ? sL[e] : sR[e]);
         }
         dF[d] = F[1] - F[0];
         if (STAGE == 1 && (c == 0 || c == N - 1)) {        // flux registers (a7 for the scalars)
-          const int e = c == 0 ? 0 : 1, f = s * 6 + 2 * d + e;
-          const int src = p.face_src[f], fs = p.fslot[f];
+          const int e = c == 0 ? 0 : 1, f = 2 * d + e;
+          const int src = fsrc6[f], fs = fslot6[f];
           if (src <= -2) {
             double* r = p.RS + (size_t(-2 - src) * p.ns + v) * FACE + tb * 8 + ta;
             *r = *r + dt * F[e];
