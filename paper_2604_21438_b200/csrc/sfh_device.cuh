@@ -68,6 +68,14 @@ __device__ __forceinline__ double minmod(double a, double b) {
   return (a * b <= 0.0) ? 0.0 : copysign(m, a);
 }
 
+// minmod(a, b) / 2 without multiplying the arguments: the difference of smaller magnitude, times 1/2 if the signs
+// agree and 0 if not (compare + select; the form the corrector's walk uses)
+__device__ __forceinline__ double half_minmod(double a, double b) {
+  const double m = fabs(a) < fabs(b) ? a : b;
+  const bool same = (__double2hiint(a) ^ __double2hiint(b)) >= 0;
+  return __hiloint2double(same ? 0x3fe00000 : 0, 0) * m;
+}
+
 // eq. (16)-(17): quadratic interpolation in time through U^n, U^{n+1/2}, U^{n+1}
 __device__ __forceinline__ double time_interp(double U0, double Uh, double U1, double tau) {
   const double U1st = 2.0 * Uh - U0;                                   // eq. (17): first-order estimate of U^{n+1}

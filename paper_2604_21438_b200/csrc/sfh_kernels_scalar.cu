@@ -154,7 +154,7 @@ __global__ void __launch_bounds__(256, 4) scalar_stage_kernel(const ScalarStageP
         if (STAGE == 1) {
           const double smm = sv[m0 - 2 * st[d]], spp = sv[m0 + 2 * st[d]];
           const double d1 = sm - smm, d2 = s0 - sm, d3 = sp - s0, d4 = spp - sp;
-          const double hm = 0.5 * minmod(d2, d1), h0 = 0.5 * minmod(d3, d2), hp = 0.5 * minmod(d4, d3);
+          const double hm = half_minmod(d2, d1), h0 = half_minmod(d3, d2), hp = half_minmod(d4, d3);
           sL[0] = sm + hm; sR[0] = s0 - h0; sL[1] = s0 + h0; sR[1] = sp - hp;
         }
         double F[2];
