@@ -17,7 +17,7 @@ constexpr int M12 = N + 2 * NG;      // ghosted edge
 // The ghosted block in shared memory: rows of 12 cells at a stride of 24 doubles, so that the two rows a half warp
 // reads (8 cells of row j, 8 of row j + 1) fall on disjoint banks (a stride of 12 gives two-way conflicts: measured
 // 43 % of the kernel's shared-memory wavefronts).
-constexpr int ROW = 24, PLANE = M12 * ROW;
+constexpr int ROW = 24, PLANE = M12 * ROW + 2;   // (+ 2: the x-halo stores, one cell per (j, k), spread over the banks)
 constexpr int G3 = M12 * PLANE;
 __device__ __forceinline__ int gpos(int i, int j, int k) { return (k + NG) * PLANE + (j + NG) * ROW + (i + NG); }
 
