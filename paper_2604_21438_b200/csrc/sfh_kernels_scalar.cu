@@ -135,6 +135,14 @@ __global__ void __launch_bounds__(256, 4) scalar_stage_kernel(const ScalarStageP
   double ir[NI];
 #pragma unroll
   for (int r = 0; r < NI; ++r) ir[r] = rcp_fast(rh[r]);
+  // my two cells (i, j, k0) and (i, j, k0 + 4): positions in the ghosted array and of their lower faces' mass fluxes
+  // (the upper faces and the second cell are constant offsets away)
+  const int ci = t & 7, cj = (t >> 3) & 7, ck0 = t >> 6;
+  const int m00 = gpos(ci, cj, ck0);
+  const int fpos[3] = {mfs_pos(0, ci, cj, ck0), mfs_pos(1, cj, ci, ck0), mfs_pos(2, ck0, ci, cj)};
+  constexpr int st[3] = {1, ROW, PLANE};
+  constexpr int fup[3] = {1, 8, FACE};                                  // next face along the pencil
+  constexpr int fk4[3] = {4 * 8 * 9, 4 * 9 * 8, 4 * FACE};              // the same pencil position four planes up
   for (int v = 0; v < p.ns; ++v) {
     __syncthreads();                         // the previous scalar's sv is no longer read
 #pragma unroll
@@ -142,16 +150,15 @@ __global__ void __launch_bounds__(256, 4) scalar_stage_kernel(const ScalarStageP
     if (v + 1 < p.ns) load_q(v + 1);
     __syncthreads();
 #pragma unroll
-    for (int cell = t; cell < NC; cell += 256) {
-      const int ijk[3] = {cell & 7, (cell >> 3) & 7, cell >> 6};
-      const int st[3] = {1, ROW, PLANE};
-      const int m0 = gpos(ijk[0], ijk[1], ijk[2]);
+    for (int r = 0; r < 2; ++r) {
+      const int cell = t + 256 * r, m0 = m00 + 4 * r * PLANE;
+      const int ijk[3] = {ci, cj, ck0 + 4 * r};
       const size_t o = (size_t(s) * p.ns + v) * NC + cell;
       const double qn = p.Qn[o];
       double dF[3];
 #pragma unroll
       for (int d = 0; d < 3; ++d) {
-        const int ta = d == 0 ? ijk[1] : ijk[0], tb = d == 2 ? ijk[1] : ijk[2], c = ijk[d];
+        const int c = ijk[d];
         // s of the cells c-1, c, c+1 (and c-2, c+2 for the corrector's three limited slopes): each slope once
         const double s0 = sv[m0], sm = sv[m0 - st[d]], sp = sv[m0 + st[d]];
         double sL[2] = {sm, s0}, sR[2] = {s0, sp};            // left / right states of the lower and the upper face
@@ -164,16 +171,17 @@ __global__ void __launch_bounds__(256, 4) scalar_stage_kernel(const ScalarStageP
         double F[2];
 #pragma unroll
         for (int e = 0; e < 2; ++e) {        // the cell's lower (e = 0) and upper face: face index c + e
-          const double fm = mfs[mfs_pos(d, c + e, ta, tb)];
+          const double fm = mfs[fpos[d] + r * fk4[d] + e * fup[d]];
           F[e] = fm * (fm >= 0.0 ? sL[e] : sR[e]);
         }
         dF[d] = F[1] - F[0];
         if (STAGE == 1 && (c == 0 || c == N - 1)) {        // flux registers (a7 for the scalars)
+          const int ta = d == 0 ? ijk[1] : ijk[0], tb = d == 2 ? ijk[1] : ijk[2];
           const int e = c == 0 ? 0 : 1, f = 2 * d + e;
           const int src = fsrc6[f], fs = fslot6[f];
           if (src <= -2) {
-            double* r = p.RS + (size_t(-2 - src) * p.ns + v) * FACE + tb * 8 + ta;
-            *r = *r + dt * F[e];
+            double* rg = p.RS + (size_t(-2 - src) * p.ns + v) * FACE + tb * 8 + ta;
+            *rg = *rg + dt * F[e];
           }
           if (fs >= 0) p.FHS[(size_t(fs) * p.ns + v) * FACE + tb * 8 + ta] = F[e];
         }
