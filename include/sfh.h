@@ -203,6 +203,31 @@ int sfh_transfer_state(sfh_mesh* src, int src_which, sfh_mesh* dst, int dst_whic
  * positive (a level without a single finite positive speed: see sfh_status). */
 int sfh_cfl_dt(sfh_mesh* m, int level, double* dt_host, void* stream);
 
+/* The CFL step of ONE level without any allocation, for callers that cannot call cudaMalloc: a program whose
+ * memory pool already owns the device (an allocation from inside this library would fail or fragment the pool), a
+ * time-critical loop in which cudaMalloc / cudaFree would stall every stream of the device, a plug-in whose host
+ * forbids allocations after start-up.  Such callers cannot use sfh_cfl_dt, because that needs a bound mesh and
+ * sfh_bind allocates the device copy of the mesh tables.  This call needs no mesh:
+ *   d_U      DEVICE, double [nblocks][5][8][8][8] ([block][var][k][j][i], the 5 hydro variables, conserved): the
+ *            blocks of one level, any order; read only;
+ *   h        cell width of that level; gamma, cfl as in sfh_config;
+ *   d_out    DEVICE, double[2], written: d_out[0] = cfl * h / s, d_out[1] = s = max over all cells of
+ *            max_d |v_d| + c_s (reading R16; the same arithmetic as sfh_cfl_dt).  Cells with a NaN speed
+ *            are ignored as in sfh_cfl_dt; if no cell has a positive speed, s = 0 and d_out[0] = inf (this call cannot
+ *            report that as SFH_ESTATE: it does not wait for the result).
+ * The per-block maxima and the running maximum, which every other path keeps in the caller's work buffer, live in an
+ * array built into the library image: SFH_NOALLOC_MAX_BLOCKS * 8 + 256 bytes (512.25 KB) of device memory on every
+ * GPU that loads libsfh.so, held until the process exits.  nblocks > SFH_NOALLOC_MAX_BLOCKS gives SFH_EINVAL (use
+ * sfh_cfl_dt with a work buffer of your own), as do nblocks < 1, null pointers, gamma <= 1, cfl <= 0, h <= 0.
+ * The first call on each device looks up the array's device address (the device must be current, as for every call
+ * here): make that first call before any stream capture.  All calls share the array and it keeps the previous
+ * call's contents; each call clears what it needs on `stream` first, so calls on one stream (or ordered by events)
+ * are independent, while calls that may run on the GPU at the same time -- two streams, two host threads --
+ * race on it and return garbage.  Asynchronous on `stream`; calls no cudaMalloc, cudaFree or allocating routine. */
+#define SFH_NOALLOC_MAX_BLOCKS 65536
+int sfh_cfl_dt_noalloc(const double* d_U, int64_t nblocks, double gamma, double cfl, double h, double* d_out,
+                       void* stream);
+
 /* One predictor-corrector update of `level` (-1: every level) by dt   (R8-R14):
  *   zero the flux registers of the (level, level+1) interface;
  *   predictor: U^{n+1/2} = U^n - dt/(2h) sum_d dF_d, first-order HLLC fluxes      (role 0 -> 1);

@@ -5,5 +5,5 @@ package only marshals arguments (torch is used for device memory and streams).  
 fallback: importing works without a GPU (so that the ABI can be inspected), every compute call
 needs one.
 """
-from .binding import (Mesh, SfhError, load_library, library_path, declared_symbols, measure_fp64_rate,  # noqa: F401
+from .binding import (Mesh, SfhError, load_library, library_path, declared_symbols, measure_fp64_rate, cfl_dt_noalloc,  # noqa: F401
                       N, NV, BLK)

@@ -68,6 +68,7 @@ def load_library(path=None):
         "sfh_fill_ghosts": (i32, [vp, i32, i32, i32, dbl, vp]),
         "sfh_get_ghosted": (i32, [vp, i32, vp, vp]),
         "sfh_cfl_dt": (i32, [vp, i32, C.POINTER(dbl), vp]),
+        "sfh_cfl_dt_noalloc": (i32, [vp, i64, dbl, dbl, dbl, vp, vp]),
         "sfh_refine_indicator": (i32, [vp, i32, i32, dbl, vp, vp]),
         "sfh_transfer_state": (i32, [vp, i32, vp, i32, vp]),
         "sfh_regrid": (i32, [vp, i32, i32, dbl, dbl, C.POINTER(vp), vp]),
@@ -108,6 +109,28 @@ def measure_fp64_rate(chains=8):
     if rc != 0:
         raise SfhError(rc, L.sfh_last_error().decode())
     return r.value
+
+
+def cfl_dt_noalloc(U, gamma, cfl, h, out=None):
+    """sfh_cfl_dt_noalloc: the CFL step of one level for callers that may not allocate device memory (a memory pool
+    owns the GPU, a loop that must not stall on cudaMalloc, a host program that forbids it): no mesh, no work buffer;
+    the reduction's intermediates live in an array built into libsfh.so (at most SFH_NOALLOC_MAX_BLOCKS = 65536
+    blocks; shared by all calls, so calls that overlap on the GPU race).  U: CUDA float64 tensor [nb][5][8][8][8];
+    `out`: CUDA float64 tensor of 2 elements to receive (dt, max speed) -- pass one you already own, since the one
+    torch creates when it is None is an allocation of the caller's (never of the library).  Asynchronous on
+    torch's current stream; returns `out`."""
+    import torch
+    L = load_library()
+    assert U.is_cuda and U.dtype == torch.float64 and U.is_contiguous() and U.numel() % BLK == 0
+    if out is None:
+        out = torch.empty(2, dtype=torch.float64, device=U.device)
+    assert out.is_cuda and out.dtype == torch.float64 and out.numel() >= 2 and out.is_contiguous()
+    with torch.cuda.device(U.device):
+        rc = L.sfh_cfl_dt_noalloc(U.data_ptr(), U.numel() // BLK, float(gamma), float(cfl), float(h), out.data_ptr(),
+                                  _stream())
+    if rc != 0:
+        raise SfhError(rc, L.sfh_last_error().decode())
+    return out
 
 
 class Mesh:

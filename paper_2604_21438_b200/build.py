@@ -11,7 +11,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = ["sfh_mesh.cpp", "sfh_kernels.cu", "sfh_kernels_mf.cu", "sfh_kernels_aux.cu", "sfh_kernels_scalar.cu", "sfh_api.cu"]
+SOURCES = ["sfh_mesh.cpp", "sfh_kernels.cu", "sfh_kernels_mf.cu", "sfh_kernels_aux.cu", "sfh_kernels_scalar.cu", "sfh_api.cu", "sfh_noalloc.cu"]
 HEADERS = ["sfh_internal.h", "sfh_device.cuh", "sfh_kernels.cuh", "sfh_stage.cuh", os.path.join("..", "..", "include", "sfh.h")]
 
 
