@@ -33,7 +33,7 @@ CORRECTOR_BYTES_PER_CELL = 120.0   # read U^n, W^{n+1/2}, w
 STEP_BYTES_PER_CELL_UPDATE = 200.0  # predictor 80 + corrector 120
 # Figures that come from an ncu capture, not from this run: per-launch DRAM traffic of the corrector and the
 # fp64 instructions the two stage kernels execute per cell-update.  Written by
-#   ncu -i <report> --page raw --csv | python -m paper_2604_21438_b200.ncu_summary --json
+#   ncu -i <report> --page raw --csv | python ncu_summary.py --json
 # (the full command is in the file) and tracked under profiles/.
 NCU_FIGURES = os.path.join(ROOT, "profiles", "r2_c2_stage_figures.json")
 
@@ -74,11 +74,19 @@ def peaks():
 
 
 def ncu_figures():
+    """The figures file, plus "stale": True when the stage-kernel sources differ from the ones it was captured on
+    (or the file does not say which those were)."""
     try:
         with open(NCU_FIGURES) as f:
-            return json.load(f)
+            fig = json.load(f)
     except Exception:
         return {}
+    try:
+        import ncu_summary
+        fig["stale"] = fig.get("stage_source_sha256") != ncu_summary.stage_source_hash()
+    except Exception:
+        fig["stale"] = True
+    return fig
 
 
 class ClockSampler:
@@ -314,6 +322,7 @@ def measure(sfh, torch, name, args, dev, world, barrier, steps, warmup, sampler_
                 "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
                 "traffic": figs.get("corrector_dram_bytes_per_launch") if is_ref_case else None,
                 "traffic_source": figs.get("source") if is_ref_case else None,
+                "traffic_stale": bool(figs.get("stale", True)) if is_ref_case else None,
                 "algorithmic_bytes_per_launch": corr_bytes / max(c_n, 1), "launches": c_n,
                 "avg_launch_ms": c_ms / max(c_n, 1),
                 "kernel_ms": {k: round(v[0], 4) for k, v in kt.items()},
@@ -400,7 +409,7 @@ def main():
         f64 = ipc * m["cu"] / (stage_ms * 1e-3) if stage_ms > 0 else 0.0
         roofline_fp64 = {"bound": "alu", "kernel": "stage_kernel<0> + stage_kernel<1>", "achieved": f64,
                          "peak": fp64_peak, "unit": "fp64 inst/s", "frac": f64 / fp64_peak, "inst_per_cell_update": ipc,
-                         "inst_source": figs.get("source"),
+                         "inst_source": figs.get("source"), "inst_stale": bool(figs.get("stale", True)),
                          "peak_source": "measured in this run (sfh_measure_fp64_rate, 8 chains per thread)"}
 
     if rank != 0:
@@ -456,6 +465,13 @@ def main():
             del q
             torch.cuda.empty_cache()
 
+    # the driver's parsed record keeps the scalar entries of `config` only: the headline figures of the other configs
+    # once more as scalars (value in cell-updates/s, fraction of the 200 B per cell-update HBM roofline)
+    per_config_flat = {}
+    for name, q in per_config.items():
+        per_config_flat["%s_value" % name] = q["value"]
+        per_config_flat["%s_step_frac_at_200B_per_update" % name] = q["step_frac_at_200B_per_update"]
+
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         # the oracle as it stands on this box's host cores, on a bounded sample: whole coarse steps of
@@ -481,7 +497,7 @@ def main():
                    "l2": "inputs larger than L2 (one state copy %.0f MB vs 126 MB L2)" % (m["state_bytes"] / 1e6),
                    "kernel_spans": "second pass of the same runs with CUDA events around every launch",
                    "parallelism": "replicas x%d" % world, "bad_cells": int(m["bad"]),
-                   "bad_cells_after_warmup": int(m["bad_warm"]), "per_config": per_config},
+                   "bad_cells_after_warmup": int(m["bad_warm"]), "per_config": per_config, **per_config_flat},
         "clocks": m["clocks"],
         "e2e": m["e2e"],
         "gpu_launches": int(m["launches"]),

@@ -1,10 +1,10 @@
 """Turns `ncu --page raw --csv` output into the text summaries kept under profiles/.
 
-    ncu -i rep.ncu-rep --page raw --csv | python -m paper_2604_21438_b200.ncu_summary [--kernel REGEX] > summary.md
-    ncu -i rep.ncu-rep --page raw --csv | python -m paper_2604_21438_b200.ncu_summary --figures --cells N \
+    ncu -i rep.ncu-rep --page raw --csv | python ncu_summary.py [--kernel REGEX] > summary.md
+    ncu -i rep.ncu-rep --page raw --csv | python ncu_summary.py --figures --cells N \
         --source "<the ncu command that wrote the report>" > profiles/<name>_figures.json
 
-    ncu -i rep.ncu-rep --page source --csv | python -m paper_2604_21438_b200.ncu_summary --source-page --cells N
+    ncu -i rep.ncu-rep --page source --csv | python ncu_summary.py --source-page --cells N
 
 Default: a markdown table, one column per profiled launch, of the metrics that explain a kernel of this library
 (duration, DRAM bytes, pipe and issue utilisation, shared-memory wavefronts, stall reasons).  --figures: the
@@ -20,6 +20,22 @@ import csv
 import json
 import re
 import sys
+
+# The kernel sources the stage-kernel figures depend on: their hash goes into the figures file, bench.py compares it
+# with the sources it runs and flags a stale file.
+STAGE_SOURCES = ("sfh_stage.cuh", "sfh_device.cuh", "sfh_kernels.cuh")
+
+
+def stage_source_hash():
+    import hashlib
+    import os
+    h = hashlib.sha256()
+    csrc = os.path.join(os.path.dirname(os.path.abspath(__file__)), "paper_2604_21438_b200", "csrc")
+    for name in STAGE_SOURCES:
+        with open(os.path.join(csrc, name), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()
+
 
 METRICS = [
     "gpu__time_duration.sum",
@@ -154,7 +170,7 @@ def main():
     names, units, launches = read_raw(sys.stdin)
     launches = [l for l in launches if re.search(a.kernel, l["Kernel Name"])]
     if a.figures:
-        out = {"source": a.source, "cells_per_launch": a.cells}
+        out = {"source": a.source, "cells_per_launch": a.cells, "stage_source_sha256": stage_source_hash()}
         for stage, key in ((0, "predictor"), (1, "corrector")):
             sel = [l for l in launches if re.search(r"stage_kernel<(\(int\))?%d\b" % stage, l["Kernel Name"])]
             if not sel:
