@@ -1,9 +1,10 @@
 """Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (sfh_advance on the
 whole problem, one persistent CTA per SM).
 
-* C2 (256^3), C4 (128^3 + 3 levels, all 10 coarse steps) and C5 (1.8e5 blocks on 5 levels, one coarse step:
+* C2 (256^3), C4 (128^3 + 3 levels, all 10 coarse steps) and C5 (1.8e5 blocks on 5 levels, all 5 coarse steps;
   the oracle's three ghosted copies take 38 GB of host memory) are compared with the oracle in every cell.
-* C3 (512^3): the oracle recomputes sampled outputs.  One step of the scheme reaches 3 cells (1 for the
+* C3 (512^3): every cell after one step, and every cell outside the reach of the oracle's non-positive cells after the
+  configured ten; besides, the oracle recomputes sampled outputs.  One step of the scheme reaches 3 cells (1 for the
   predictor, 2 for the corrector), so the inner 2^3 blocks of a sub-box cut out of the full initial state
   with a margin of 3 cells per step (outflow on the cut faces), stepped with the full problem's dt
   sequence, are exactly the full problem's values there: one step on 4^3-block boxes, the configured ten
@@ -94,7 +95,7 @@ def test_c3_full_size_sampled_sub_boxes():
             states[step] = g.get_state().cpu().numpy()
     rng = np.random.default_rng(3)
     report = {}
-    for nsteps, S, margin, nbox, tol in ((1, 4, 1, 6, TOL1), (p.nsteps, 10, 4, 3, TOL10)):
+    for nsteps, S, margin, nbox, tol in ((1, 4, 1, 6, TOL1), (p.nsteps, 10, 4, 5, TOL10)):
         Ug = states[nsteps]
         compared = nonfinite = 0
         for _ in range(nbox):
@@ -117,7 +118,8 @@ def test_c3_full_size_sampled_sub_boxes():
             compared += 1
         report[nsteps] = (compared, nonfinite)
     print("C3 sub-boxes (steps: compared, non-finite):", report, "bad cells after %d steps: %d" % (p.nsteps, g.status()))
-    assert report[1][0] >= 4 and report[p.nsteps][0] >= 1, report
+    # every box whose oracle values stayed finite was compared above; at least two of the ten-step boxes must have been
+    assert report[1][0] >= 4 and report[p.nsteps][0] >= 2, report
 
 
 def leaf_mask(level, ijk):
@@ -143,7 +145,8 @@ def test_c5_full_size_conservation_and_subcycling():
     U0 = g.get_state().cpu().numpy()
     t0 = totals(U0, p.level, leaf, p.max_level)
     del U0
-    g.advance(1, 1)
+    assert p.nsteps == 5
+    g.advance(p.nsteps, 1)                     # the configured 5 coarse steps
     U1 = g.get_state().cpu().numpy()
     assert np.isfinite(U1).all()
     t1 = totals(U1, p.level, leaf, p.max_level)
@@ -154,16 +157,18 @@ def test_c5_full_size_conservation_and_subcycling():
     assert (np.abs(t1[1:4] - t0[1:4]) <= 1e-12 * mscale).all(), (t0, t1)
     # eq. (14)-(15): each level takes 2^n sub-steps of its parent, n >= 0
     n = g.nupd
-    assert n[0] == 1
+    assert n[0] == p.nsteps
     for l in range(1, p.max_level + 1):
-        r = n[l] // n[l - 1]
-        assert n[l] == r * n[l - 1] and r >= 1 and (r & (r - 1)) == 0, n
+        # per coarse step the ratio is a power of two (checked step by step in test_gpu_parity); over several steps the
+        # counts add up, so only "a whole number of sub-steps per parent update, at least one" holds for the totals
+        assert n[l] >= n[l - 1], n
     assert g.status() == 0
 
 
-def test_c5_full_size_every_cell_one_coarse_step():
-    """The whole 182 008-block hierarchy against the oracle for one adaptive coarse step (every level sub-cycles:
-    ~2e9 cell-updates, a few minutes of oracle time on 16 cores; 38 GB of host memory for its ghosted copies)."""
+def test_c5_full_size_every_cell_all_coarse_steps():
+    """The whole 182 008-block hierarchy against the oracle in every cell: after one adaptive coarse step (1e-12) and
+    after the configured 5 (BASELINE.json configs[4]; 1e-10), every level sub-cycling, equal update counts per level
+    (a few minutes of oracle time on 16 cores; 38 GB of host memory for its ghosted copies)."""
     import os
     ram_gb = os.sysconf("SC_PAGE_SIZE") * os.sysconf("SC_PHYS_PAGES") / 2 ** 30
     print("host RAM %.0f GB, %d cores" % (ram_gb, len(os.sched_getaffinity(0))))
@@ -180,8 +185,17 @@ def test_c5_full_size_every_cell_one_coarse_step():
     assert abs(g.t.value - o.t.value) <= TOLDT * o.t.value
     assert o.status() == 0 and g.status() == 0
     err = parity_errors(g.get_state().cpu().numpy(), o.get_state(), p.gamma)
-    print("C5 full size: updates/level", list(g.nupd), "parity", err)
+    print("C5 full size, 1 coarse step: updates/level", list(g.nupd), "parity", err)
     assert (err <= TOL1).all(), err
+    assert p.nsteps == 5
+    g.advance(p.nsteps - 1, 1)
+    o.advance(p.nsteps - 1, 1)
+    assert np.array_equal(o.nupd, g.nupd), (o.nupd, g.nupd)
+    assert abs(g.t.value - o.t.value) <= 1e-13 * o.t.value
+    assert o.status() == 0 and g.status() == 0
+    err = parity_errors(g.get_state().cpu().numpy(), o.get_state(), p.gamma)
+    print("C5 full size, %d coarse steps: updates/level" % p.nsteps, list(g.nupd), "parity", err)
+    assert (err <= TOL10).all(), err
 
 
 def test_c3_full_size_every_cell_one_step():
@@ -216,3 +230,86 @@ def test_c3_full_size_every_cell_one_step():
     for v in range(5):
         d = np.abs(Ug[:, v][good] - Uo[:, v][good]).max() / scale[v]
         assert d <= TOL1, (v, d)
+
+
+def global_grid(p, A):
+    """Per-cell block array A[nb][8][8][8] of the uniform problem p on the global grid [z][y][x]."""
+    nb = p.nb0[0]
+    order = np.lexsort((p.ijk[:, 0], p.ijk[:, 1], p.ijk[:, 2]))          # z slowest
+    G = A[order].reshape(nb, nb, nb, 8, 8, 8)                            # [bz][by][bx][k][j][i]
+    return np.ascontiguousarray(G.transpose(0, 3, 1, 4, 2, 5)).reshape(nb * 8, nb * 8, nb * 8)
+
+
+def dilate_periodic(mask, r):
+    """Every cell within r cells (per axis: a cube, which contains one step's stencil reach) of a marked cell."""
+    for ax in range(3):
+        acc = mask.copy()
+        for s in range(1, r + 1):
+            acc |= np.roll(mask, s, axis=ax)
+            acc |= np.roll(mask, -s, axis=ax)
+        mask = acc
+    return mask
+
+
+def not_positive(U, gamma):
+    rho, E = U[:, 0], U[:, 4]
+    with np.errstate(all="ignore"):
+        P = (gamma - 1.0) * (E - 0.5 * (U[:, 1] ** 2 + U[:, 2] ** 2 + U[:, 3] ** 2) / rho)
+        return ~(np.isfinite(U).all(axis=1) & (rho > 0.0) & (P > 0.0))
+
+
+def test_c3_full_size_every_cell_ten_steps_outside_the_reach_of_bad_cells():
+    """All of C3's configured 10 steps against the oracle in every cell that the oracle's non-positive cells cannot
+    have reached.  The Mach-10 input leaves a few cells at non-positive pressure from the first step on (DESIGN.md
+    R28: no floors on either side; such a cell's content is undefined and spreads 3 cells per step: 1 through the
+    predictor, 2 through the corrector).  A cell is left out when, at any step, it lay within 3 cells per later step
+    of a cell that was not positive and finite on either side; everything else (the fraction is printed and must be
+    >= 0.9) is compared at 1e-10.  Both sides step with the oracle's CFL steps."""
+    import os
+    ram_gb = os.sysconf("SC_PAGE_SIZE") * os.sysconf("SC_PHYS_PAGES") / 2 ** 30
+    if ram_gb < 110:
+        pytest.skip("the oracle's three ghosted copies of C3 need 54 GB (+ inputs): host has %.0f GB" % ram_gb)
+    p = make_config("C3")
+    assert p.nsteps == 10
+    o = oracle_for(p)
+    g = gpu_for(p)
+    reach, n_only_g = 3, 0
+    mask = np.zeros((p.nb0[0] * 8,) * 3, dtype=bool)
+    for step in range(1, p.nsteps + 1):
+        dt = o.cfl_dt()
+        if step == 1:
+            assert abs(g.cfl_dt() - dt) <= TOLDT * dt
+        o.advance(1, 0, dt)
+        g.advance(1, 0, dt)
+        if step > 1:
+            mask = dilate_periodic(mask, reach)                  # what the marked cells reached in this step
+        Uo = o.get_state()
+        bad = not_positive(Uo, p.gamma)
+        if step < p.nsteps:
+            # a cell that goes bad on the CUDA side only, OUTSIDE the reach of earlier bad cells (where the two sides
+            # agreed to round-off a step ago), can only be a pressure within round-off of zero: left out too, but
+            # counted and bounded, so that this mask cannot hide a fault of the CUDA path
+            only_g = global_grid(p, not_positive(g.get_state().cpu().numpy(), p.gamma) & ~bad) & ~mask
+            n_only_g += int(only_g.sum())
+            mask |= only_g
+        mask |= global_grid(p, bad)
+        print("C3 step %d: %d oracle cells not positive, %d cells left out so far, %d bad on the CUDA side only"
+              % (step, int(bad.sum()), int(mask.sum()), n_only_g))
+    assert n_only_g <= 10
+    Ug = g.get_state().cpu().numpy()
+    keep = ~mask
+    frac = keep.mean()
+    print("C3 full size, %d steps: compared %.4f of %d cells; oracle status %d, CUDA status %d"
+          % (p.nsteps, frac, keep.size, o.status(), g.status()))
+    assert frac >= 0.9
+    Go = [global_grid(p, Uo[:, v])[keep] for v in range(5)]
+    Gg = [global_grid(p, Ug[:, v])[keep] for v in range(5)]
+    assert all(np.isfinite(a).all() for a in Gg)
+    rho, E = Go[0], Go[4]
+    P = (p.gamma - 1.0) * (E - 0.5 * (Go[1] ** 2 + Go[2] ** 2 + Go[3] ** 2) / rho)
+    cs = np.sqrt(p.gamma * P / rho)
+    mscale = max((np.abs(Go[v]) + rho * cs).max() for v in (1, 2, 3))     # DESIGN.md "Parity norm"
+    scale = [np.abs(rho).max(), mscale, mscale, mscale, np.abs(E).max()]
+    err = [float(np.abs(Gg[v] - Go[v]).max() / scale[v]) for v in range(5)]
+    print("C3 full size, %d steps: parity" % p.nsteps, err)
+    assert max(err) <= TOL10, err
