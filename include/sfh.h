@@ -166,9 +166,10 @@ int sfh_refine_indicator(sfh_mesh* m, int which, int criterion, double G, double
  * on the device and brought to the host, where the library builds the new block list (the lists are
  * managed on the hosts):
  *   - every root block;
- *   - the 8 children of every block of level < max_level that is in `m`, is in the new tree, and whose indicator is
- *     >= threshold (eq. 33 is written with >=): a regrid deepens the tree by at most one level anywhere and drops
- *     the children of blocks that are no longer flagged;
+ *   - the 8 children of every block of level < max_level that is in `m`, is in the new tree, and is flagged: its
+ *     indicator is >= threshold (eq. 33 is written with >=) or one of its descendants in `m` is flagged (a feature
+ *     smaller than a coarse cell does not show in the restricted data of the blocks above it).  A regrid deepens the
+ *     tree by at most one level anywhere and drops the children of blocks that are no longer flagged;
  *   - closed under proper nesting over the 26 neighbours (reading R25): missing blocks are added with their 7
  *     siblings and, recursively, their ancestors.
  * *out is a new, UNBOUND mesh with the same configuration and Riemann solver (destroy it with sfh_destroy_mesh); its

@@ -782,9 +782,10 @@ int orc_transfer_state(const Mesh* src, int src_which, Mesh* dst, int dst_which)
 // PAPER.md:96 ("a block is refined ... subdivided into eight child blocks"), :277-285 (eq. 33-34), :641 (Jeans), :100
 // (lists built on the host).  The new tree, from the indicator of copy `which` (ghosts filled here):
 //   * every root block;
-//   * the 8 children of every block B of level < max_level that is in the OLD mesh, is in the NEW tree, and whose
-//     indicator is >= threshold (eq. 33 is written with >=) -- so a regrid deepens the tree by at most one level
-//     anywhere and drops the children of blocks that are no longer flagged;
+//   * the 8 children of every block B of level < max_level that is in the OLD mesh, is in the NEW tree, and is
+//     flagged: its indicator is >= threshold (eq. 33 is written with >=) or one of its descendants in the old mesh is
+//     flagged -- so a regrid deepens the tree by at most one level anywhere, drops the children of blocks that are
+//     no longer flagged, and keeps the refinement above every flagged block;
 //   * closed under proper nesting (reading R25): every one of the 26 neighbour positions of a level-l block that lies
 //     inside the domain (periodic wrap applied; positions beyond an outflow face are skipped) is covered at level
 //     l-1; missing blocks are created with their 7 siblings and, recursively, their ancestors.
@@ -799,10 +800,18 @@ int orc_regrid(Mesh* m, int which, int criterion, double Gc, double threshold, M
   typedef std::array<int, 3> C3;
   std::vector<std::set<C3>> tree(m->nlev);
   for (int64_t b = 0; b < m->nb; ++b) if (m->lev[b] == 0) tree[0].insert(C3{m->bx[b], m->by[b], m->bz[b]});
+  // a block counts as flagged when its own indicator is >= threshold or when any of its descendants in the OLD mesh
+  // is flagged (reading R33: a feature smaller than a coarse cell is invisible in the restricted data of the coarse
+  // block above it, and must not lose its refinement for that)
+  std::vector<char> flag(m->nb);
+  for (int64_t b = 0; b < m->nb; ++b) flag[b] = ind[b] >= threshold;
+  for (int l = m->nlev - 1; l >= 1; --l)
+    for (int b : m->of_level[l])
+      if (flag[b]) flag[find(*m, l - 1, m->bx[b] >> 1, m->by[b] >> 1, m->bz[b] >> 1)] = 1;
   for (int l = 0; l + 1 < m->nlev; ++l)
     for (int b : m->of_level[l]) {
       const C3 c{m->bx[b], m->by[b], m->bz[b]};
-      if (!tree[l].count(c) || !(ind[b] >= threshold)) continue;
+      if (!tree[l].count(c) || !flag[b]) continue;
       for (int q = 0; q < 8; ++q) tree[l + 1].insert(C3{2 * c[0] + (q & 1), 2 * c[1] + ((q >> 1) & 1), 2 * c[2] + ((q >> 2) & 1)});
     }
   // make the octet that holds block c of level l exist (and its ancestors)

@@ -255,8 +255,8 @@ int build_host_mesh(const sfh_config& cfg_in, int64_t nblocks_in, const int32_t*
 
 // ---- regrid: the block list of the new tree (reading R31) ----------------
 // ind[slot]: refinement indicator of every block of the old mesh (library order).  New tree: all root blocks; the
-// octet under every old block of level < max_level that is still in the new tree and has ind >= threshold (eq. 33 is
-// written with >=); then the closure under proper nesting over the 26 neighbours (reading R25), adding whole octets
+// octet under every old block of level < max_level that is still in the new tree and is flagged -- ind >= threshold
+// (eq. 33 is written with >=) or a flagged descendant in the old mesh (reading R33) --; then the closure under proper nesting over the 26 neighbours (reading R25), adding whole octets
 // and their ancestors.  Output: level-major, (bx, by, bz) lexicographic within a level.
 int regrid_block_list(const HostMesh& old, const double* ind, double threshold, std::vector<int32_t>& level,
                       std::vector<int32_t>& ijk) {
@@ -274,9 +274,15 @@ int regrid_block_list(const HostMesh& old, const double* ind, double threshold, 
     return any;
   };
   for (int64_t s = 0; s < old.nb && old.lev[s] == 0; ++s) add(0, old.coord[3 * s], old.coord[3 * s + 1], old.coord[3 * s + 2]);
+  // flagged: own indicator >= threshold, or a flagged descendant in the old mesh (slots are level-major, so one
+  // pass from the back reaches every ancestor)
+  std::vector<char> flag(size_t(old.nb));
+  for (int64_t s = 0; s < old.nb; ++s) flag[size_t(s)] = ind[s] >= threshold;
+  for (int64_t s = old.nb - 1; s >= 0; --s)
+    if (flag[size_t(s)] && old.parent[size_t(s)] >= 0) flag[size_t(old.parent[size_t(s)])] = 1;
   for (int64_t s = 0; s < old.nb; ++s) {                          // slots are level-major: parents come first
     const int l = old.lev[s];
-    if (l + 1 >= nlev || !(ind[s] >= threshold)) continue;
+    if (l + 1 >= nlev || !flag[size_t(s)]) continue;
     const int x = old.coord[3 * s], y = old.coord[3 * s + 1], z = old.coord[3 * s + 2];
     if (have[l].count(hkey(l, x, y, z))) add_octet(l + 1, x, y, z);
   }

@@ -121,7 +121,7 @@ def test_compute_calls_fail_loudly_without_binding():
 
 def test_regrid_block_list_host_logic_matches_the_stated_rules():
     """sfh_regrid_from_indicator (host only): the same block list as the dense-array construction of
-    sfh_inputs.Tree (children of flagged blocks present in the new tree, 2:1 closure), in the documented order."""
+    sfh_inputs.Tree (children of blocks that are flagged or have a flagged descendant, 2:1 closure), in the documented order."""
     from sfh_inputs import Tree
     rng = np.random.default_rng(5)
     for periodic, offset in (((True, True, True), (0, 0, 0)), ((False, True, False), (-1, 0, 1))):
@@ -132,11 +132,16 @@ def test_regrid_block_list_host_logic_matches_the_stated_rules():
             ind = rng.random(len(level))
             new = m.regrid_from_indicator(ind, thr)
             ref = Tree(t.nb0, t.max_level, periodic)
-            for l in range(t.max_level):
-                f = np.zeros_like(ref.exists[l])
+            f = []
+            for l in range(t.max_level + 1):
+                f.append(np.zeros_like(ref.exists[l]))
                 sel = (level == l) & (ind >= thr)
-                f[ijk[sel, 0], ijk[sel, 1], ijk[sel, 2]] = True
-                ref.refine(l, f)
+                f[l][ijk[sel, 0], ijk[sel, 1], ijk[sel, 2]] = True
+            for l in range(t.max_level, 0, -1):      # a flagged block flags its ancestors (reading R33)
+                sh = f[l].shape
+                f[l - 1] |= f[l].reshape(sh[0] // 2, 2, sh[1] // 2, 2, sh[2] // 2, 2).any(axis=(1, 3, 5))
+            for l in range(t.max_level):
+                ref.refine(l, f[l])
             lev, ij = ref.pad_2to1().block_list()
             assert np.array_equal(new.level, lev) and np.array_equal(new.ijk, ij)
             assert new.cfg.nscalar == m.cfg.nscalar and new.max_level == m.max_level

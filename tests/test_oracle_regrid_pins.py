@@ -116,13 +116,18 @@ def test_coarsening_keeps_the_restricted_parents_and_two_levels_are_created_at_o
 # ------------------------------------------------------------------ the regrid's block list (orc_regrid)
 def tree_from_flags(p, flagged, periodic):
     """The same rules with an unrelated implementation (dense boolean arrays and dilation, sfh_inputs.Tree): children
-    of flagged blocks that exist in the new tree, then the 2:1 closure."""
+    of blocks that are flagged, or have a flagged descendant, and exist in the new tree; then the 2:1 closure."""
     t = Tree(p.nb0, p.max_level, periodic)
-    for l in range(p.max_level):
-        f = np.zeros_like(t.exists[l])
+    f = []
+    for l in range(p.max_level + 1):
+        f.append(np.zeros_like(t.exists[l]))
         sel = (p.level == l) & flagged
-        f[p.ijk[sel, 0], p.ijk[sel, 1], p.ijk[sel, 2]] = True
-        t.refine(l, f)
+        f[l][p.ijk[sel, 0], p.ijk[sel, 1], p.ijk[sel, 2]] = True
+    for l in range(p.max_level, 0, -1):              # a flagged block flags its ancestors (reading R33)
+        s = f[l].shape
+        f[l - 1] |= f[l].reshape(s[0] // 2, 2, s[1] // 2, 2, s[2] // 2, 2).any(axis=(1, 3, 5))
+    for l in range(p.max_level):
+        t.refine(l, f[l])
     return t.pad_2to1().block_list()
 
 
@@ -195,3 +200,42 @@ def test_regrid_with_nothing_flagged_returns_the_root_grid_and_everything_flagge
     assert (none.level == 0).all() and len(none.level) == 64
     full = m.regrid(0, -1.0)
     assert [int((full.level == l).sum()) for l in range(4)] == [64, 512, 512, 0]       # level 2 under the old level-1 patch only
+
+
+@pytest.mark.parametrize("which_fine", ["all", "one"])
+def test_flagged_fine_block_keeps_its_ancestors(which_fine):
+    """Reading R33: a feature smaller than a coarse cell.  Level-2 blocks carry a density pattern +-delta that averages
+    to zero over every 2 x 2 x 2 cells, so the restricted levels 1 and 0 are exactly uniform (indicator 0) while the
+    level-2 indicator is large.  The refinement above the flagged level-2 blocks must survive the regrid although
+    no block of levels 0 and 1 is flagged by its own data."""
+    p = problem_from_tree(small_amr_tree(), mode=1)
+    assert p.max_level == 2
+    U = np.zeros_like(p.U)
+    U[:, 0] = 1.0
+    U[:, 4] = 1.0 / (p.gamma - 1.0)
+    fine = np.flatnonzero(p.level == 2)
+    marked = fine if which_fine == "all" else fine[:1]
+    k, j, i = np.meshgrid(np.arange(8), np.arange(8), np.arange(8), indexing="ij")
+    U[marked, 0] += 0.125 * (1.0 - 2.0 * ((i + j + k) & 1))
+    m = oracle_for(p, U)
+    m.restrict_all(0)
+    assert (m.get_state()[p.level < 2][:, 0] == 1.0).all()           # the pattern is invisible from above
+    m.fill_ghosts(-1, 0, 0, 0.0)
+    ind = m.refine_indicator(0)
+    thr = 1e-2                                                        # the paper's threshold (PAPER.md:285)
+    assert (ind[p.level < 2] == 0.0).all() and (ind[marked] > 1.0).all()
+    new = m.regrid(0, thr)
+    old = {(int(l), *map(int, c)) for l, c in zip(p.level, p.ijk)}
+    newset = {(int(l), *map(int, c)) for l, c in zip(new.level, new.ijk)}
+    for b in marked:                                                  # every flagged block and its ancestors are there
+        l, c = int(p.level[b]), p.ijk[b]
+        while l >= 0:
+            assert (l, *map(int, c)) in newset
+            l, c = l - 1, c >> 1
+    if which_fine == "all":
+        assert newset == old                                          # nothing above the flagged patch is lost
+    else:
+        assert len(newset) < len(old) and (new.level == 2).sum() == 8  # the other level-2 octets go, this one stays
+    lev, ijk = tree_from_flags(p, ind >= thr, (True, True, True))
+    assert np.array_equal(new.level, lev) and np.array_equal(new.ijk, ijk)
+    assert properly_nested(new.level, new.ijk, p.nb0, (True, True, True), p.max_level)
