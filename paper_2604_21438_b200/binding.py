@@ -348,24 +348,30 @@ class Mesh:
         the old mesh's ghosts of `which` first."""
         self._chk(self.L.sfh_transfer_state(src.h, which, self.h, which, _stream()))
 
+    def _derived(self, handle, bind):
+        """Wrapper of a mesh the library derived from this one (sfh_regrid*).  Such a mesh always has 8^3 blocks: from
+        a mesh of 16^3 blocks the library derives the mesh of the octants (sfh.h, "Blocks of 16^3 cells"), whose root
+        grid counts twice as many blocks per axis; states then cross the interface as [nb][nv][8][8][8]."""
+        c = self.cfg
+        k = self.ncell // N
+        return Mesh(tuple(k * n for n in c.nb0), c.max_level, [tuple(b) for b in c.bc], tuple(c.box_len), c.gamma,
+                    c.cfl, None, None, device=self.device, lib=self.L, nscalar=c.nscalar, handle=handle, bind=bind,
+                    ncell=N)
+
     def regrid_from_indicator(self, indicator, threshold, bind=False):
         """The new mesh from a host indicator array (caller order); host only unless bind=True."""
         ind = np.ascontiguousarray(indicator, dtype=np.float64)
         assert ind.shape == (self.nentries(),)
         h = C.c_void_p()
         self._chk(self.L.sfh_regrid_from_indicator(self.h, ind.ctypes.data, float(threshold), C.byref(h)))
-        c = self.cfg
-        return Mesh(tuple(c.nb0), c.max_level, [tuple(b) for b in c.bc], tuple(c.box_len), c.gamma, c.cfl, None, None,
-                    device=self.device, lib=self.L, nscalar=c.nscalar, handle=h, bind=bind)
+        return self._derived(h, bind)
 
     def regrid(self, criterion, threshold, which=0, G=1.0):
         """The regridded mesh (sfh_regrid: blocks with indicator >= threshold get children, 2:1 closure), bound to new
         buffers, holding the state of copy `which` moved onto it (sfh_transfer_state)."""
         h = C.c_void_p()
         self._chk(self.L.sfh_regrid(self.h, which, criterion, float(G), float(threshold), C.byref(h), _stream()))
-        c = self.cfg
-        new = Mesh(tuple(c.nb0), c.max_level, [tuple(b) for b in c.bc], tuple(c.box_len), c.gamma, c.cfl, None, None,
-                   device=self.device, lib=self.L, nscalar=c.nscalar, handle=h)
+        new = self._derived(h, True)
         new.transfer_from(self, which)
         return new
 

@@ -76,7 +76,11 @@ WorkLayout work_layout(const HostMesh& hm) {
   w.RS = up(w.ghostS + 2 * ncf * ns * NG * FACE * 8);
   w.FHS = up(w.RS + ncf * ns * FACE * 8);
   w.MF = up(w.FHS + size_t(hm.nfh) * ns * FACE * 8);
-  w.scalars = up(w.MF + (ns ? size_t(hm.nb) * 3 * 9 * FACE * 8 : 0));
+  // mass fluxes of ONE stage of ONE level (consumed by the scalar kernel right after the stage that wrote them):
+  // sized by the largest level, indexed by (slot - first slot of the level)
+  int64_t widest = 0;
+  for (int l = 0; l < hm.nlev; ++l) widest = hm.lev_count[l] > widest ? hm.lev_count[l] : widest;
+  w.scalars = up(w.MF + (ns ? size_t(widest) * 3 * 9 * FACE * 8 : 0));
   w.total = w.scalars + 4096;
   return w;
 }
@@ -248,7 +252,9 @@ int stage_level(sfh_mesh* m, int l, int stage, Dt dt, cudaStream_t st) {
   p.use_regs = stage == 1 && (hm.cf_count[l] > 0 || hm.reflux_count[l] > 0);
   p.riemann = m->riemann;
   p.bmax = stage == 1 ? m->bmax : nullptr;
-  p.mf = m->ns > 0 ? m->MF : nullptr;
+  // the kernels index the mass fluxes by slot: shift the base so that the level's first block lands at MF[0]
+  double* const mf_level = m->ns > 0 ? m->MF - size_t(hm.lev_first[l]) * (3 * 9 * FACE) : nullptr;
+  p.mf = mf_level;
   // the corrector overwrites the level's cached maxima with those of U^{n+1}: they stop describing U^n now
   if (stage == 1) { m->bmax_pending[l] = true; m->bmax_valid[l] = false; }
   {
@@ -259,7 +265,7 @@ int stage_level(sfh_mesh* m, int l, int stage, Dt dt, cudaStream_t st) {
   if (m->ns > 0) {      // the scalars ride on the mass fluxes the stage has just exported
     ScalarStageParams q;
     q.Qsrc = role_q(m, l, src_role); q.Qn = role_q(m, l, 0); q.Qdst = role_q(m, l, stage == 0 ? 1 : 2);
-    q.Hsrc = p.Usrc; q.ghostH = p.ghost; q.ghostS = stage == 0 ? m->ghostS : m->ghostS1; q.mf = m->MF;
+    q.Hsrc = p.Usrc; q.ghostH = p.ghost; q.ghostS = stage == 0 ? m->ghostS : m->ghostS1; q.mf = mf_level;
     q.RS = m->RS; q.FHS = m->FHS; q.face_src = m->d_face_src; q.fslot = m->d_fslot;
     q.dt_dev = dt.dev; q.dt = dt.host; q.h = hm.h[l]; q.first = p.first; q.count = p.count; q.ns = m->ns;
     Timed tmr(m, 6, st);

@@ -25,7 +25,7 @@ struct StageParams {
   int use_regs;          // corrector: the level has flux-register faces
   int riemann;           // 0 HLLC, 1 Roe
   double* bmax;          // corrector: per-block maximum CFL speed of U^{n+1} (or null)
-  double* mf;            // if non-null: mass flux of every face, [nb][3 axes][9 faces][64 pencils] (passive scalars)
+  double* mf;            // if non-null: mass flux of every face, [blocks of the level][3 axes][9 faces][64 pencils], base shifted so that slots index it (passive scalars)
 };
 
 struct TensorMaps {      // tensor maps of ONE state buffer seen as [5 nb][8][8][8]
@@ -139,7 +139,7 @@ struct ScalarStageParams {
   const double* Hsrc;    // hydro copy of the same state as Qsrc (variable 0 = rho in both its forms)
   const double* ghostH;  // its coarse-fine slabs
   const double* ghostS;  // coarse-fine slabs of Qsrc  [ncf][ns][128]
-  const double* mf;      // mass fluxes written by the hydro stage  [nb][3][9][64]
+  const double* mf;      // mass fluxes written by the hydro stage  [blocks of the level][3][9][64], indexed by slot (shifted base)
   double* RS;            // fine-side scalar flux registers [ncf][ns][64]
   double* FHS;           // coarse-side                     [nfh][ns][64]
   const int32_t* face_src;

@@ -447,6 +447,37 @@ def test_dynamic_regrid_cycle_matches_the_oracle(criterion):
     compare(o, g, p.gamma, TOL10)
 
 
+def test_regrid_from_a_mesh_of_16_cell_blocks():
+    """sfh_regrid on a mesh of 16^3 blocks gives the mesh of 8^3 blocks that the same cells handed over as octants
+    give (refinement is decided per octant, sfh.h "Blocks of 16^3 cells"): same block list, same state bit for bit,
+    and a wrapper whose geometry (root grid doubled, 8 cells per edge) is that of the library's mesh, so that it
+    can be stepped and regridded again."""
+    from sfh_inputs import tree16_problem
+    p16, p8 = tree16_problem(amr16_tree((True, True, True)), mode=1)
+    g16, g8 = sfh.Mesh.from_problem(p16), sfh.Mesh.from_problem(p8)
+    for m, p in ((g16, p16), (g8, p8)):
+        m.set_state(p.U)
+        m.restrict_all(0)
+        m.advance(1, 1)
+    ind = g8.refine_indicator(0).cpu().numpy()
+    assert np.array_equal(g16.refine_indicator(0).cpu().numpy(), ind)       # entry e = 8 * block + octant
+    s = np.sort(ind)
+    k = int(0.6 * len(s))
+    k = k + int(np.argmax(np.diff(s[k:k + 12])))
+    thr = 0.5 * (s[k] + s[k + 1])
+    n16, n8 = g16.regrid(0, thr), g8.regrid(0, thr)
+    assert n16.ncell == 8 and tuple(n16.cfg.nb0) == tuple(n8.cfg.nb0) == tuple(2 * n for n in p16.nb0)
+    assert n16.nb == n8.nb == n16.nentries() and n16.nb != g8.nb
+    assert np.array_equal(n16.level, n8.level) and np.array_equal(n16.ijk, n8.ijk)
+    assert n16.cell_width(0) == n8.cell_width(0) == g8.cell_width(0)
+    assert np.array_equal(n16.get_state().cpu().numpy(), n8.get_state().cpu().numpy())
+    for m in (n16, n8):
+        m.advance(2, 1)
+    assert np.array_equal(n16.get_state().cpu().numpy(), n8.get_state().cpu().numpy())
+    again = n16.regrid(0, thr)                                                 # and the derived wrapper regrids again
+    assert again.ncell == 8 and again.nb == again.nentries() and again.status() == 0
+
+
 def test_calls_run_on_the_callers_stream():
     """Every call takes the stream the caller passes (torch's current stream in the binding): the same run on
     a side stream gives the same bits, and work queued on that stream is ordered with it."""
