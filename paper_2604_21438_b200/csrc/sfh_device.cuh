@@ -143,10 +143,12 @@ __device__ __forceinline__ double sound_speed(double gamma, double P, double rho
 // produces a block's maximum speed calls this, so the cached per-block maxima and the reduction over
 // whole states agree bit for bit.
 __device__ __forceinline__ double cell_speed(const double u[5], double gamma, double gm1) {
-  double w[5];
-  cons_to_prim(u, gm1, w);
-  const double cs = sound_speed(gamma, w[4], w[0]);
-  return fmax(fmax(fabs(w[1]), fabs(w[2])), fabs(w[3])) + cs;
+  // (max_d |m_d| + sqrt(gamma (gamma-1) (rho E - |m|^2 / 2))) / rho: c_s rho = sqrt(gamma P rho) without forming P
+  // or the velocities (19 fp64 instructions instead of 26; the corrector's helpers evaluate this for every cell)
+  const double m2 = fma(u[3], u[3], fma(u[2], u[2], u[1] * u[1]));
+  const double x = (gamma * gm1) * fma(-0.5, m2, u[0] * u[4]);
+  const double mm = fmax(fmax(fabs(u[1]), fabs(u[2])), fabs(u[3]));
+  return fma(x, rsqrt_fast(x), mm) * rcp_fast(u[0]);
 }
 
 __device__ __forceinline__ double warp_max(double x) {
@@ -158,13 +160,14 @@ __device__ __forceinline__ double warp_max(double x) {
 // HLLC flux (Toro et al. 1994 as cited; Davis wave speeds, reading R6) in the face
 // frame: u = normal velocity, v, w = the two tangential ones; Fn = (mass, normal momentum, tangential
 // momenta, energy).  cL, cR = sound speeds of the two states; igm1 = 1/(gamma-1).
-// Branch-free.  With K the upwind side (L if S_L >= 0, or if S_L < 0 < S_R and S* >= 0; else R),
-//   F = F_K + s (U*_K - U_K),  s = S_K inside the star region (S_L < 0 < S_R), else 0,
+// Branch-free.  With K the upwind side (L if S* >= 0, else R: S_L < S* < S_R holds strictly for Davis speeds and
+// positive rho, P, so S_L >= 0 implies S* > 0 and S_R <= 0 implies S* < 0),
+//   F = F_K + s (U*_K - U_K),  s = S_K clipped at zero (min(S_L, 0) or max(S_R, 0): zero in the supersonic cases),
 // and with d = S* - u_K, g = d/(S_K - S*), A = rho_K g the oracle's star state
 //   U*_K = q (rho, rho S*, rho v, rho w, E + rho d (S* + P/(rho (S_K-u))))_K,  q = (S_K-u_K)/(S_K-S*) = 1 + g
 // gives  U*_K - U_K = (A, rho d + A S*, A v, A w, g (E + P + rho d S*) + rho d S*).
 // The denominator m_L - m_R of S* is strictly negative for positive rho (m_L < 0 < m_R), whatever
-// the wave pattern, so S* is always finite; S_K - S* is replaced by 1 outside the star region.
+// the wave pattern, so S* is always finite, and S_K - S* never vanishes.
 // HAVE_E: the total energies of the two states are known (cell-centred states: the conserved E).
 template <bool HAVE_E>
 __device__ __forceinline__ void hllc_flux(double rL, double uL, double vL, double wL, double PL, double cL, double EL,
@@ -173,15 +176,30 @@ __device__ __forceinline__ void hllc_flux(double rL, double uL, double vL, doubl
   const double SL = dmin(uL - cL, uR - cR);
   const double SR = dmax(uL + cL, uR + cR);
   const double mL = rL * (SL - uL), mR = rR * (SR - uR);
+#ifdef SFH_V_ILP
+  const double num = ((PR - PL) + mL * uL) - mR * uR, den = mL - mR;
+  const double Ss = num * rcp_fast(den);
+#else
   const double Ss = (((PR - PL) + mL * uL) - mR * uR) * rcp_fast(mL - mR);
-  const bool star = SL < 0.0 && SR > 0.0;
-  const bool left = !(SL < 0.0) || (SR > 0.0 && Ss >= 0.0);
+#endif
+  // S_L < S* < S_R strictly (Davis speeds, positive rho and P), so the upwind side is the sign of S* alone, and
+  // clipping the chosen wave speed at zero drops the star term in the supersonic cases
+#ifdef SFH_V_ILP
+  const bool left = !(num > 0.0);            // S* = num / den >= 0 with den < 0: known before the reciprocal lands
+#else
+  const bool left = Ss >= 0.0;
+#endif
   const double r = left ? rL : rR, u = left ? uL : uR, v = left ? vL : vR, w = left ? wL : wR;
   const double P = left ? PL : PR, S = left ? SL : SR;
   const double E = HAVE_E ? (left ? EL : ER) : fma(P, igm1, (0.5 * r) * fma(w, w, fma(v, v, u * u)));
   const double ru = r * u, EP = E + P;
-  const double inv = rcp_fast(star ? S - Ss : 1.0);
-  const double s = star ? S : 0.0;
+#ifdef SFH_V_ILP
+  const double inv = den * rcp_fast(fma(S, den, -num));   // 1 / (S - S*) = den / (S den - num): independent of the first reciprocal
+#else
+  const double inv = rcp_fast(S - Ss);
+#endif
+  const bool in = left ? SL < 0.0 : SR > 0.0;
+  const double s = in ? S : 0.0;
   const double d = Ss - u, g = d * inv, rd = r * d, A = rd * inv, rdS = rd * Ss;
   Fn[0] = fma(s, A, ru);
   Fn[1] = fma(s, fma(A, Ss, rd), fma(ru, u, P));
