@@ -176,28 +176,16 @@ __device__ __forceinline__ void hllc_flux(double rL, double uL, double vL, doubl
   const double SL = dmin(uL - cL, uR - cR);
   const double SR = dmax(uL + cL, uR + cR);
   const double mL = rL * (SL - uL), mR = rR * (SR - uR);
-#ifdef SFH_V_ILP
-  const double num = ((PR - PL) + mL * uL) - mR * uR, den = mL - mR;
+  const double num = ((PR - PL) + mL * uL) - mR * uR, den = mL - mR;   // S* = num / den, den < 0
   const double Ss = num * rcp_fast(den);
-#else
-  const double Ss = (((PR - PL) + mL * uL) - mR * uR) * rcp_fast(mL - mR);
-#endif
   // S_L < S* < S_R strictly (Davis speeds, positive rho and P), so the upwind side is the sign of S* alone, and
   // clipping the chosen wave speed at zero drops the star term in the supersonic cases
-#ifdef SFH_V_ILP
   const bool left = !(num > 0.0);            // S* = num / den >= 0 with den < 0: known before the reciprocal lands
-#else
-  const bool left = Ss >= 0.0;
-#endif
   const double r = left ? rL : rR, u = left ? uL : uR, v = left ? vL : vR, w = left ? wL : wR;
   const double P = left ? PL : PR, S = left ? SL : SR;
   const double E = HAVE_E ? (left ? EL : ER) : fma(P, igm1, (0.5 * r) * fma(w, w, fma(v, v, u * u)));
   const double ru = r * u, EP = E + P;
-#ifdef SFH_V_ILP
   const double inv = den * rcp_fast(fma(S, den, -num));   // 1 / (S - S*) = den / (S den - num): independent of the first reciprocal
-#else
-  const double inv = rcp_fast(S - Ss);
-#endif
   const bool in = left ? SL < 0.0 : SR > 0.0;
   const double s = in ? S : 0.0;
   const double d = Ss - u, g = d * inv, rd = r * d, A = rd * inv, rdS = rd * Ss;
