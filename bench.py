@@ -35,7 +35,7 @@ STEP_BYTES_PER_CELL_UPDATE = 200.0  # predictor 80 + corrector 1
 # fp64 instructions the two stage kernels execute per cell-update.  Written by
 #   ncu -i <report> --page raw --csv | python ncu_summary.py --json
 # (the full command is in the file) and tracked under profiles/.
-NCU_FIGURES = os.path.join(ROOT, "profiles", "r2_c2_stage_figures.json")
+NCU_FIGURES = os.path.join(ROOT, "profiles", "r3_c2_stage_figures.json")
 
 
 def parse():
